@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the PIVOT implied-volatility hot path on B200 (contract in the task prompt).
+
+Workload (BASELINE.json `metric`: "fp64 forward LBR IV/s at 2^26 rows; fwd+bwd rows/s; max rel err vs oracle"):
+config 4 at n = 2^26 rows per GPU (inputs as config 1: x~U[-5,5], s log-U[1e-4,5], call/put 50/50, Black-76 D = 1),
+seeded and generated on the device.  One "step" = one pass of the whole hot path over the batch: the fused forward
+kernel (sigma, vega, status) + the gated backward kernel (MASK, vega_floor 1e-8).  `value` = rows/s through fwd+bwd,
+whole job; the forward-only IV/s and the error vs the oracle ride along as extra keys.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--rows R] [--impl ours|reference]
+
+N > 1 is launched by torchrun (one rank per GPU); rows are sharded (weak scaling), there is no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fp64 forward LBR IV/s at 2^26 rows; fwd+bwd rows/s; max rel err vs oracle"
+VEGA_FLOOR = 1e-8
+KEYS = ("SorF", "K", "tau", "P", "flag")
+
+# fp64-pipe peak of one B200, derived from unit counts and clocks:
+# 148 SMs x 64 fp64 FMA lanes per SM per clock x 2 flops x 1.965 GHz (clocks.max.sm) = 37.2 TFLOP/s.
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# algorithmic bytes per row: forward Black-76 5x8 in + 8+8+1 out; backward 8+8+1 in + 8 out
+FWD_BYTES_PER_ROW = 57
+BWD_BYTES_PER_ROW = 25
+# per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
+# CUDA 12.9 builtins); "/" and sqrt count 1 flop each
+CALL_FLOPS = {"exp": 31, "log": 47, "log1p": 109, "erfc": 113, "erfcx": 165, "ninv": 315, "cbrt": 16}
+# fallback algorithmic flops/row per class (zone 0..3, non-OK), used only when the oracle leg is not run (ranks of an
+# N > 1 job); produced by oracle/pyoracle.count_ops on config 1 and the table above
+FALLBACK_FLOPS_PER_CLASS = (2557.0, 1796.0, 1818.0, 2359.0, 6.0)
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def _flops_per_row_from_counts(counts, rows):
+    names = ("add", "mul", "div", "sqrt", "exp", "log", "log1p", "erfc", "erfcx", "ninv", "cbrt")
+    tot_plain = tot_calls = 0.0
+    for c in range(5):
+        for i, nm in enumerate(names):
+            v = float(counts[c][i])
+            if nm in CALL_FLOPS:
+                tot_calls += v * CALL_FLOPS[nm]
+            else:
+                tot_plain += v
+    n = float(rows.sum())
+    return tot_plain / n, (tot_plain + tot_calls) / n
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import pyoracle as po
+    from paper_2606_17065_b200 import workloads as wl
+    m = min(args.rows, 1 << 22)
+    cfg = wl.config4(m, device="cpu")
+    c = {k: cfg[k].numpy() for k in KEYS}
+    gs = np.random.default_rng(4).standard_normal(m)
+    def step():
+        s, v, st = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"])
+        po.backward(gs, v, st, VEGA_FLOOR, 0)
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    val = m / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "rows/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config 4 (inputs as config 1), bounded sample of {m} rows per step, fwd+bwd, CPU oracle"},
+            "cpu_baseline": {"value": val, "unit": "rows/s", "cores": po.max_threads(), "kind": "oracle",
+                             "sample": f"{m} rows of config 4 per step, forward + MASK backward"},
+            "e2e": {"value": val, "unit": "rows/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--rows", type=int, default=1 << 26, help="rows per GPU")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import paper_2606_17065_b200 as pv
+    from paper_2606_17065_b200 import workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the PIVOT path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    n = args.rows
+    K, W = args.steps, max(args.warmup, 3)
+
+    # --- inputs resident in HBM (row shard of this rank; seeds differ per rank)
+    cfg = wl.config4(n, seed=4 + rank, device="cuda")
+    a = [cfg[k] for k in KEYS]
+    g = torch.Generator(device="cuda"); g.manual_seed(1000 + rank)
+    gsig = torch.randn(n, dtype=torch.float64, device="cuda", generator=g)
+    out = (torch.empty(n, dtype=torch.float64, device="cuda"), torch.empty(n, dtype=torch.float64, device="cuda"),
+           torch.empty(n, dtype=torch.uint8, device="cuda"))
+    gP = torch.empty(n, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        pv.pivot_iv_forward(*a, out=out, stream=stream)
+        pv.pivot_iv_backward(gsig, out[1], out[2], VEGA_FLOOR, pv.GATE_MASK, out=gP, stream=stream)
+
+    for _ in range(W):
+        step()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
+    barrier()
+    sampler.start()
+    t_begin = torch.cuda.Event(enable_timing=True); t_end = torch.cuda.Event(enable_timing=True)
+    t_begin.record(stream)
+    for i in range(K):
+        ev[i][0].record(stream)
+        pv.pivot_iv_forward(*a, out=out, stream=stream)
+        ev[i][1].record(stream)
+        pv.pivot_iv_backward(gsig, out[1], out[2], VEGA_FLOOR, pv.GATE_MASK, out=gP, stream=stream)
+        ev[i][2].record(stream)
+    t_end.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = t_begin.elapsed_time(t_end)
+    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    bwd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    if dist is not None:
+        t = torch.tensor([total_ms, fwd_ms, bwd_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, fwd_ms, bwd_ms = (float(x) for x in t.tolist())
+    ms_per_step = total_ms / K
+    value = world * n / (ms_per_step * 1e-3)
+
+    # --- e2e: the same step through the C-ABI host entry point (pinned host buffers, H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        host = [t_.cpu().pin_memory() for t_ in a]
+        hgs = gsig.cpu().pin_memory()
+        hout = (torch.empty(n, dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory(),
+                torch.empty(n, dtype=torch.uint8).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory())
+        pipe = pv.Pipeline(chunk_rows=1 << 21, n_slots=4)
+        ke = max(1, min(K, 5))
+        pipe.forward_backward_host(*host, hgs, VEGA_FLOOR, pv.GATE_MASK, out=hout)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            pipe.forward_backward_host(*host, hgs, VEGA_FLOOR, pv.GATE_MASK, out=hout)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) / ke
+        pipe.close()
+        t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+        if dist is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        e2e = {"value": world * n / dt, "unit": "rows/s", "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 25 * n,
+               "ms_per_step": dt * 1e3, "steps": ke, "api": "pivot_iv_forward_backward_host (pinned host buffers)"}
+        del host, hgs, hout
+
+    # --- zone mix of this workload (diagnostic kernel variant; not timed)
+    zsig, zveg, zst, zone = pv.pivot_iv_forward_zones(*a)
+    mix = [int(((zone == z) & (zst == 0)).sum().item()) for z in range(4)] + [int((zst != 0).sum().item())]
+    del zsig, zveg, zone
+
+    # --- cpu_baseline + parity sample + algorithmic flop count: the oracle, rank 0 at N = 1 only
+    cpu = None
+    err = {}
+    flops_plain = flops_all = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import pyoracle as po
+        m = min(n, 1 << 24)
+        c = {k: cfg[k][:m].cpu().numpy() for k in KEYS}
+        hg = gsig[:m].cpu().numpy()
+        t0 = time.perf_counter()
+        os_, ov, ost = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"])
+        og = po.backward(hg, ov, ost, VEGA_FLOOR, 0)
+        dt = time.perf_counter() - t0
+        cpu = {"value": m / dt, "unit": "rows/s", "cores": po.max_threads(), "kind": "oracle",
+               "sample": f"first {m} rows of the same workload, forward + MASK backward, one pass"}
+        gs_, gv_, gst_ = (t_[:m].cpu().numpy() for t_ in out)
+        ok = (ost == 0) & (gst_ == 0)
+        err["status_mismatches"] = int((ost != gst_).sum())
+        err["max_rel_err_sigma"] = float(np.max(np.abs(gs_[ok] / os_[ok] - 1))) if ok.any() else None
+        on = ok & (ov > VEGA_FLOOR) & (np.abs(ov / VEGA_FLOOR - 1) > 1e-12) & (og != 0)
+        err["max_rel_err_grad_P"] = float(np.max(np.abs(gP[:m].cpu().numpy()[on] / og[on] - 1))) if on.any() else None
+        err["parity_sample_rows"] = m
+        mc = min(m, 1 << 18)
+        counts, rows = po.count_ops(*[c[k][:mc] for k in KEYS])
+        flops_plain, flops_all = _flops_per_row_from_counts(counts, rows)
+    if flops_all is None:
+        tot = float(sum(mix))
+        flops_all = sum(f * k for f, k in zip(FALLBACK_FLOPS_PER_CLASS, mix)) / tot
+
+    peaks, peak_src = _peaks()
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    fwd_tflops = flops_all * n / (fwd_ms * 1e-3) / 1e12
+    roofline = {"kernel": "forward_kernel_vec2<false,false>", "bound": "alu", "achieved": fwd_tflops,
+                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": fwd_tflops / FP64_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md s7); DFMA probe measures ~35.7",
+                "flops_per_row": flops_all, "flops_per_row_excl_transcendental_internals": flops_plain,
+                "avg_launch_ms": fwd_ms,
+                "hbm": {"achieved": FWD_BYTES_PER_ROW * n / (fwd_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": FWD_BYTES_PER_ROW * n / (fwd_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src}}
+    bwd_gbs = BWD_BYTES_PER_ROW * n / (bwd_ms * 1e-3) / 1e9
+    roofline_bwd = {"kernel": "backward_kernel_vec4<MASK>", "bound": "hbm", "achieved": bwd_gbs, "peak": hbm_peak,
+                    "unit": "GB/s", "frac": bwd_gbs / hbm_peak, "traffic": None, "avg_launch_ms": bwd_ms,
+                    "peak_source": peak_src}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": "rows/s", "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "config 4 @ n=2^26 rows/GPU (inputs as config 1: x~U[-5,5], s log-U[1e-4,5], "
+                                       "call/put 50/50, Black-76 D=1); step = fused forward + MASK backward (floor 1e-8)",
+                           "rows_per_gpu": n, "l2": "inputs+outputs 5.5 GB per step >> 126 MB L2, no flush needed",
+                           "zone_mix_rows[z0,z1,z2,z3,non_ok]": mix},
+                "fwd_iv_per_s": world * n / (fwd_ms * 1e-3), "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+                "bwd_rows_per_s": world * n / (bwd_ms * 1e-3),
+                "solved_rows_per_s_fwd": world * sum(mix[:4]) / (fwd_ms * 1e-3),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": K * (pv.load_library().pivot_iv_launches_per_forward() + pv.load_library().pivot_iv_launches_per_backward()),
+                "roofline": roofline, "roofline_backward": roofline_bwd, "cpu_baseline": cpu}
+        line.update(err)
+        line["paper_context"] = {"h100_triton_fused_iv_per_s": 1.79e9, "h100_max_rel_err": 9.3e-14,
+                                 "h100_label_pipeline_per_s": 48.9e6, "source": "PAPER.md:156,175 (1e5 rows; not the target)"}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,134 @@
+/* include/pivot_iv.h -- C ABI of the PIVOT implied-volatility hot path for NVIDIA B200 (sm_100a).
+ *
+ * One data-parallel path (arxiv/paper_2606_17065, "PIVOT"): batched, row-independent fp64 inversion of
+ * Black-76 / Black-Scholes-Merton prices to implied volatility with the "Let's Be Rational" construction in
+ * the forward pass, fused with the Black vega and a status byte; and a separate fused elementwise backward
+ * pass  grad_P = gate * grad_sigma / vega  by implicit differentiation (never through the solver branches).
+ * Citations are /root/reference/PAPER.md line numbers (section / equation given alongside).
+ *
+ * Conventions for every entry point
+ *   - plain C, no C++ exceptions cross the boundary; returns 0 (PIVOT_OK) or a negative PIVOT_ERR_* code;
+ *   - per-row numerical problems are never error codes, they are `status` values;
+ *   - the library never allocates, frees or retains caller memory, keeps no global mutable state (except inside an
+ *     explicit pivot_iv_pipeline object), and the device entry points never synchronise the host:
+ *     work is enqueued on `stream` (a cudaStream_t passed as an opaque pointer; NULL = the legacy default stream);
+ *   - all arrays are SoA, contiguous, length n, fp64 unless stated; pointers need only their natural alignment
+ *     (8 B for double): a 16-B-aligned fast path and a scalar path exist on the GPU, there is no CPU fallback;
+ *   - n == 0 is a successful no-op.
+ */
+#ifndef PIVOT_IV_H_
+#define PIVOT_IV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PIVOT_IV_VERSION 100 /* major*10000 + minor*100 + patch */
+
+/* error codes */
+#define PIVOT_OK 0
+#define PIVOT_ERR_NULL (-1)      /* a required pointer is NULL */
+#define PIVOT_ERR_BAD_N (-2)     /* n < 0 */
+#define PIVOT_ERR_BAD_MODE (-3)  /* mode not PIVOT_GATE_MASK / PIVOT_GATE_ATTENUATE */
+#define PIVOT_ERR_BAD_FLOOR (-4) /* vega_floor is NaN or negative */
+#define PIVOT_ERR_MIXED_RQ (-5)  /* exactly one of r, q is NULL */
+#define PIVOT_ERR_CUDA (-6)      /* CUDA runtime error (launch, copy, allocation inside a pipeline) */
+#define PIVOT_ERR_BAD_ARG (-7)   /* other invalid argument (pipeline geometry, device index) */
+
+/* per-row status byte written by the forward pass (PAPER.md:98 Alg.1 l.3, :125, :363; readings in DESIGN.md) */
+#define PIVOT_ST_OK 0              /* sigma, vega valid */
+#define PIVOT_ST_BELOW_INTRINSIC 1 /* undiscounted price < max(theta (F-K), 0)        -> sigma = NaN, vega = 0 */
+#define PIVOT_ST_ABOVE_MAX 2       /* undiscounted price >= F (call) or >= K (put)     -> sigma = NaN, vega = 0 */
+#define PIVOT_ST_BAD_INPUT 3       /* tau <= 0, non-finite or non-positive S|F, K, non-finite P, r, q, flag not +-1,
+                                      or |ln(F/K)| > 693                               -> sigma = NaN, vega = 0 */
+#define PIVOT_ST_AT_INTRINSIC 4    /* time value is zero or subnormal after normalisation -> sigma = +0, vega = 0 */
+
+/* gate modes of the backward pass (eq.(9), :148-150 eq.(10)) */
+#define PIVOT_GATE_MASK 0      /* hard mask 1{|V| > vega_floor} */
+#define PIVOT_GATE_ATTENUATE 1 /* smooth gate w(V) = V^2 / (V^2 + vega_floor^2) */
+
+/* Row tuple as parallel arrays (PAPER.md:123 "every input is treated as a tensor"; :51 xi = (S,K,tau,r,q), theta).
+ * For the device entry points these are DEVICE pointers; for the *_host entry points HOST pointers. */
+typedef struct pivot_iv_inputs {
+  const double* S_or_F; /* spot S (BSM mode) or forward F (Black-76 mode) */
+  const double* K;      /* strike */
+  const double* tau;    /* time to expiry in years */
+  const double* r;      /* risk-free rate;   r and q both NULL => Black-76 with discount factor 1 */
+  const double* q;      /* dividend yield;   r and q both non-NULL => BSM: F = S e^{(r-q) tau}, D = e^{-r tau} */
+  const double* P;      /* observed (discounted) option price P* */
+  const double* flag;   /* theta: +1.0 call, -1.0 put; anything else => PIVOT_ST_BAD_INPUT */
+} pivot_iv_inputs;
+
+typedef struct CUstream_st* pivot_iv_stream; /* == cudaStream_t */
+
+/* Forward pass, one fused kernel (PAPER.md:94-98 Alg.1 l.1-3; :359-363 A.5 stages 1-5; :322 eq.(14)).
+ * Per row: normalise (F = S e^{(r-q)tau}, x = ln(F/K), beta = e^{r tau} P / sqrt(FK)); validity -> status; reduce to an
+ * OTM call (x <= 0); LBR boundary point and four-zone rational initial guess; two Householder(3) steps on the zone's
+ * transformed objective; sigma = s / sqrt(tau); vega = dP/dsigma = D sqrt(FK) phi0 exp(-(h^2+t^2)/2) sqrt(tau).
+ *   in      device pointers (see pivot_iv_inputs), read only
+ *   n       number of rows, >= 0
+ *   sigma   [out, device, n doubles] implied volatility; canonical quiet NaN (0x7ff8000000000000) for status 1-3, +0 for 4
+ *   vega    [out, device, n doubles] Black vega (per unit of sigma, not per 1%); 0 when status != 0
+ *   status  [out, device, n bytes]   PIVOT_ST_*
+ *   stream  CUDA stream the kernel is enqueued on
+ * Outputs must not alias inputs.  Returns PIVOT_ERR_NULL / _BAD_N / _MIXED_RQ / _CUDA. */
+int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                     pivot_iv_stream stream);
+
+/* As pivot_iv_forward, additionally writing the LBR zone taken by each OK row (0 lower tail, 1 lower middle,
+ * 2 upper middle, 3 upper tail; -1 when status != 0).  Diagnostics only: zone edges are transcendental, so this
+ * byte is not bit-reproducible across implementations and is not part of `status`. */
+int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                           int8_t* zone, pivot_iv_stream stream);
+
+/* Backward pass, one fused elementwise kernel (PAPER.md:100-103 Alg.1 l.4-6; :107 eq.(7); :131 eq.(8) first half;
+ * :144 eq.(9); :150 eq.(10)).  Reads only what the forward emitted: 25 B per row.
+ *   MASK:      grad_P = grad_sigma / vega                              if status == OK and |vega| > vega_floor (strict)
+ *   ATTENUATE: grad_P = grad_sigma * vega / (vega^2 + vega_floor^2)    if status == OK   (= w(V) grad_sigma / V)
+ *   otherwise  grad_P = +0.0 exactly (by select, so 0*NaN never leaks).
+ *   grad_sigma, vega [in, device, n doubles]; status [in, device, n bytes]; grad_P [out, device, n doubles], may
+ *   alias grad_sigma.  Returns PIVOT_ERR_NULL / _BAD_N / _BAD_MODE / _BAD_FLOOR / _CUDA. */
+int pivot_iv_backward(const double* grad_sigma, const double* vega, const uint8_t* status, double vega_floor,
+                      int mode, int64_t n, double* grad_P, pivot_iv_stream stream);
+
+/* ---- host-buffer pipeline (the streaming label-generation setting: batches of rows, H2D included) ----
+ * A pipeline owns `n_slots` device staging slots of `chunk_rows` rows each, one CUDA stream per slot and pinned
+ * bounce buffers are NOT used: host arrays are copied directly (pin them for full PCIe speed).  The *_host calls split
+ * the n rows into chunks, overlap H2D copy, kernels and D2H copy across slots, and return after the last byte of
+ * output is in host memory (they synchronise).  Not thread-safe per pipeline object. */
+typedef struct pivot_iv_pipeline pivot_iv_pipeline;
+
+/* Creates a pipeline on CUDA device `device` (-1 = current).  chunk_rows > 0, 1 <= n_slots <= 8. */
+int pivot_iv_pipeline_create(pivot_iv_pipeline** out, int device, int64_t chunk_rows, int n_slots);
+int pivot_iv_pipeline_destroy(pivot_iv_pipeline* p);
+
+/* Forward on HOST arrays: `in`, sigma, vega, status are host pointers (length n). */
+int pivot_iv_forward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega,
+                          uint8_t* status);
+
+/* Forward + backward on HOST arrays: additionally reads grad_sigma (host, n) and writes grad_P (host, n). */
+int pivot_iv_forward_backward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* grad_sigma,
+                                   double vega_floor, int mode, int64_t n, double* sigma, double* vega,
+                                   uint8_t* status, double* grad_P);
+
+/* ---- measurement helpers ---- */
+/* Dependent-DFMA-chain microbenchmark on `stream`: every thread of a full-occupancy grid runs `iters` rounds of 8
+ * independent fused multiply-adds.  Writes the number of fp64 FMA instructions (per thread, summed over threads)
+ * to *fma_count_out (host); the caller times it with CUDA events to obtain the fp64-pipe peak.
+ * `sink` is a device buffer of at least 8 bytes. */
+int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivot_iv_stream stream);
+
+/* Number of kernels a call launches (for bench.py's `gpu_launches` bookkeeping). */
+int pivot_iv_launches_per_forward(void);
+int pivot_iv_launches_per_backward(void);
+
+const char* pivot_iv_strerror(int code);
+int pivot_iv_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIVOT_IV_H_ */

@@ -9,7 +9,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(HERE, "liblbr_oracle.so")
-SOURCES = [os.path.join(HERE, "oracle_capi.cpp")]
+SOURCES = [os.path.join(HERE, "oracle_capi.cpp"), os.path.join(HERE, "opcount.cpp")]
 DEPS = SOURCES + [os.path.join(HERE, "lbr_oracle.hpp")]
 
 

@@ -175,3 +175,19 @@ def f_up_end(x, s):
     out = (C.c_double * 3)()
     lib().oracle_f_up_end(C.c_double(x), C.c_double(s), out)
     return tuple(out)
+
+
+OP_NAMES = ("add", "mul", "div", "sqrt", "exp", "log", "log1p", "erfc", "erfcx", "ninv", "cbrt")
+
+
+def count_ops(SorF, K, tau, P, flag, r=None, q=None, fixed_iters=2):
+    """Algorithmic fp64 operation counts of the oracle (op-counting scalar type), per LBR zone.
+    Returns (counts[5, 11] uint64, rows[5]): classes 0..3 = zone of OK rows, 4 = non-OK rows; columns OP_NAMES."""
+    SorF, K, tau, P, flag = map(_d, (SorF, K, tau, P, flag))
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    nc = int(lib().oracle_count_ops_ncounters())
+    counts = np.zeros((5, nc), dtype=np.uint64); rows = np.zeros(5, dtype=np.uint64)
+    lib().oracle_count_ops(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(P), _p(flag),
+                           C.c_int(fixed_iters), counts.ctypes.data_as(C.c_void_p), rows.ctypes.data_as(C.c_void_p))
+    return counts, rows

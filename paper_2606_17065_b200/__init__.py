@@ -1,0 +1,27 @@
+"""paper_2606_17065_b200 -- B200-native (sm_100a) PIVOT implied-volatility hot path.
+
+Thin Python binding over the C-ABI library `libpivot_iv.so` (include/pivot_iv.h).  Every step of the path runs in
+the hand-written CUDA kernels; Python only marshals arguments.  PyTorch is used for device memory and streams.
+There is no CPU fallback: calling any entry point without the built library or without a CUDA device raises.
+"""
+from .binding import (  # noqa: F401
+    GATE_ATTENUATE,
+    GATE_MASK,
+    PivotError,
+    Pipeline,
+    library_path,
+    load_library,
+    pivot_iv_backward,
+    pivot_iv_forward,
+    pivot_iv_forward_zones,
+    pivot_iv_probe_dfma,
+    pivot_iv_strerror,
+    pivot_iv_version,
+    EXPORTS,
+)
+
+__all__ = [
+    "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "Pipeline", "pivot_iv_probe_dfma",
+    "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
+    "GATE_ATTENUATE", "EXPORTS",
+]

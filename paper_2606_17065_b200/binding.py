@@ -1,0 +1,210 @@
+"""ctypes binding of include/pivot_iv.h: argument marshalling only (same names as the C entry points)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Tuple
+
+import torch  # loads libcudart first, so the library shares torch's CUDA runtime / primary context
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(HERE, "libpivot_iv.so")
+
+GATE_MASK = 0
+GATE_ATTENUATE = 1
+
+# every symbol include/pivot_iv.h declares
+EXPORTS = (
+    "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_pipeline_create",
+    "pivot_iv_pipeline_destroy", "pivot_iv_forward_host", "pivot_iv_forward_backward_host", "pivot_iv_probe_dfma",
+    "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
+)
+
+
+class PivotError(RuntimeError):
+    pass
+
+
+class _Inputs(C.Structure):
+    _fields_ = [(name, C.c_void_p) for name in ("S_or_F", "K", "tau", "r", "q", "P", "flag")]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _SO
+
+
+def load_library():
+    """Loads libpivot_iv.so; raises (never falls back) if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise PivotError(f"{_SO} is missing: build it with `python paper_2606_17065_b200/build.py` "
+                         "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = C.CDLL(_SO)
+    vp, i64, dbl, cint = C.c_void_p, C.c_int64, C.c_double, C.c_int
+    lib.pivot_iv_forward.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
+    lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
+    lib.pivot_iv_backward.argtypes = [vp, vp, vp, dbl, cint, i64, vp, vp]
+    lib.pivot_iv_pipeline_create.argtypes = [C.POINTER(vp), cint, i64, cint]
+    lib.pivot_iv_pipeline_destroy.argtypes = [vp]
+    lib.pivot_iv_forward_host.argtypes = [vp, C.POINTER(_Inputs), i64, vp, vp, vp]
+    lib.pivot_iv_forward_backward_host.argtypes = [vp, C.POINTER(_Inputs), vp, dbl, cint, i64, vp, vp, vp, vp]
+    lib.pivot_iv_probe_dfma.argtypes = [i64, vp, C.POINTER(dbl), vp]
+    lib.pivot_iv_strerror.argtypes = [cint]
+    lib.pivot_iv_strerror.restype = C.c_char_p
+    for name in EXPORTS:
+        if name != "pivot_iv_strerror":
+            getattr(lib, name).restype = cint
+    _lib = lib
+    return lib
+
+
+def pivot_iv_strerror(code: int) -> str:
+    return load_library().pivot_iv_strerror(int(code)).decode()
+
+
+def pivot_iv_version() -> int:
+    return int(load_library().pivot_iv_version())
+
+
+def _check(code: int):
+    if code != 0:
+        raise PivotError(f"pivot_iv error {code}: {pivot_iv_strerror(code)}")
+
+
+def _dev(t: Optional[torch.Tensor], name: str, dtype=torch.float64) -> Optional[int]:
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.dim() == 1):
+        raise PivotError(f"{name}: expected a contiguous 1-D CUDA tensor of {dtype}")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise PivotError("no CUDA device: the PIVOT path runs only on the GPU (no CPU fallback)")
+
+
+def _forward(SorF, K, tau, P, flag, r, q, out, stream, zones):
+    _require_cuda()
+    lib = load_library()
+    n = SorF.numel()
+    for nm, t in (("K", K), ("tau", tau), ("P", P), ("flag", flag), ("r", r), ("q", q)):
+        if t is not None and t.numel() != n:
+            raise PivotError(f"{nm}: length {t.numel()} != {n}")
+    inp = _Inputs(_dev(SorF, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P, "P"),
+                  _dev(flag, "flag"))
+    if out is None:
+        sigma = torch.empty(n, dtype=torch.float64, device=SorF.device)
+        vega = torch.empty(n, dtype=torch.float64, device=SorF.device)
+        status = torch.empty(n, dtype=torch.uint8, device=SorF.device)
+    else:
+        sigma, vega, status = out[:3]
+    sp = _stream_ptr(stream)
+    with torch.cuda.device(SorF.device):
+        if zones:
+            zone = torch.empty(n, dtype=torch.int8, device=SorF.device) if out is None or len(out) < 4 else out[3]
+            _check(lib.pivot_iv_forward_zones(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
+                                              _dev(status, "status", torch.uint8), _dev(zone, "zone", torch.int8), sp))
+            return sigma, vega, status, zone
+        _check(lib.pivot_iv_forward(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
+                                    _dev(status, "status", torch.uint8), sp))
+    return sigma, vega, status
+
+
+def pivot_iv_forward(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None
+                     ) -> Tuple[torch.Tensor, torch.Tensor, torch.Tensor]:
+    """(sigma, vega, status) = pivot_iv_forward(...) on CUDA fp64 tensors; r = q = None selects Black-76 with D = 1.
+    `out` = (sigma, vega, status) preallocated tensors; `stream` = torch.cuda.Stream (default: current)."""
+    return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, False)
+
+
+def pivot_iv_forward_zones(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None):
+    """As pivot_iv_forward, also returning the LBR zone per row (diagnostics)."""
+    return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, True)
+
+
+def pivot_iv_backward(grad_sigma, vega, status, vega_floor: float, mode: int, out=None, stream=None) -> torch.Tensor:
+    """grad_P = gate * grad_sigma / vega (mode GATE_MASK or GATE_ATTENUATE); `out` may alias grad_sigma."""
+    _require_cuda()
+    lib = load_library()
+    n = grad_sigma.numel()
+    if vega.numel() != n or status.numel() != n:
+        raise PivotError("grad_sigma, vega, status must have the same length")
+    gP = torch.empty_like(grad_sigma) if out is None else out
+    with torch.cuda.device(grad_sigma.device):
+        _check(lib.pivot_iv_backward(_dev(grad_sigma, "grad_sigma"), _dev(vega, "vega"),
+                                     _dev(status, "status", torch.uint8), float(vega_floor), int(mode), n,
+                                     _dev(gP, "grad_P"), _stream_ptr(stream)))
+    return gP
+
+
+def pivot_iv_probe_dfma(iters: int, stream=None) -> float:
+    """Enqueues the DFMA-chain probe; returns the number of fp64 FMAs it executes (time it with CUDA events)."""
+    _require_cuda()
+    sink = torch.zeros(8, dtype=torch.float64, device="cuda")
+    cnt = C.c_double(0.0)
+    _check(load_library().pivot_iv_probe_dfma(int(iters), sink.data_ptr(), C.byref(cnt), _stream_ptr(stream)))
+    return float(cnt.value)
+
+
+def _host(t: Optional[torch.Tensor], name: str, dtype=torch.float64) -> Optional[int]:
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != dtype or not t.is_contiguous() or t.dim() != 1:
+        raise PivotError(f"{name}: expected a contiguous 1-D CPU tensor of {dtype}")
+    return t.data_ptr()
+
+
+class Pipeline:
+    """Host-buffer pipeline (pivot_iv_pipeline_*): chunked H2D -> kernels -> D2H over `n_slots` streams.
+    Pass pinned CPU tensors for full PCIe bandwidth."""
+
+    def __init__(self, chunk_rows: int = 1 << 20, n_slots: int = 3, device: int = -1):
+        _require_cuda()
+        self._lib = load_library()
+        self._h = C.c_void_p()
+        _check(self._lib.pivot_iv_pipeline_create(C.byref(self._h), int(device), int(chunk_rows), int(n_slots)))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.pivot_iv_pipeline_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def forward_host(self, S_or_F, K, tau, P, flag, r=None, q=None, out=None):
+        n = S_or_F.numel()
+        if out is None:
+            out = (torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.float64),
+                   torch.empty(n, dtype=torch.uint8))
+        sigma, vega, status = out
+        inp = _Inputs(_host(S_or_F, "S_or_F"), _host(K, "K"), _host(tau, "tau"), _host(r, "r"), _host(q, "q"),
+                      _host(P, "P"), _host(flag, "flag"))
+        _check(self._lib.pivot_iv_forward_host(self._h, C.byref(inp), n, _host(sigma, "sigma"), _host(vega, "vega"),
+                                               _host(status, "status", torch.uint8)))
+        return sigma, vega, status
+
+    def forward_backward_host(self, S_or_F, K, tau, P, flag, grad_sigma, vega_floor, mode, r=None, q=None, out=None):
+        n = S_or_F.numel()
+        if out is None:
+            out = (torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.float64),
+                   torch.empty(n, dtype=torch.uint8), torch.empty(n, dtype=torch.float64))
+        sigma, vega, status, gP = out
+        inp = _Inputs(_host(S_or_F, "S_or_F"), _host(K, "K"), _host(tau, "tau"), _host(r, "r"), _host(q, "q"),
+                      _host(P, "P"), _host(flag, "flag"))
+        _check(self._lib.pivot_iv_forward_backward_host(self._h, C.byref(inp), _host(grad_sigma, "grad_sigma"),
+                                                        float(vega_floor), int(mode), n, _host(sigma, "sigma"),
+                                                        _host(vega, "vega"), _host(status, "status", torch.uint8),
+                                                        _host(gP, "grad_P")))
+        return sigma, vega, status, gP

@@ -1,0 +1,31 @@
+"""Builds paper_2606_17065_b200/libpivot_iv.so (hand-written CUDA, sm_100a only) in-tree with nvcc.
+
+nvcc cross-compiles without a GPU; the built .so travels to the GPU box with the repo snapshot.
+"""
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+ROOT = os.path.dirname(HERE)
+SO = os.path.join(HERE, "libpivot_iv.so")
+SRC = [os.path.join(HERE, "csrc", "pivot_iv.cu")]
+DEPS = SRC + [os.path.join(HERE, "csrc", "lbr_device.cuh"), os.path.join(ROOT, "include", "pivot_iv.h")]
+NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+         "-shared", "-cudart", "shared"]
+
+
+def needs_build() -> bool:
+    return not os.path.exists(SO) or any(os.path.getmtime(SO) < os.path.getmtime(d) for d in DEPS)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and not needs_build():
+        return SO
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SRC
+    subprocess.check_call(cmd)
+    return SO
+
+
+if __name__ == "__main__":
+    print(build(force=True, verbose=True))

@@ -1,0 +1,405 @@
+// pivot_iv.cu -- kernels and C ABI (include/pivot_iv.h) of the PIVOT implied-volatility hot path, sm_100a.
+//
+// Forward: one fused kernel; every intermediate of the per-row LBR solve lives in registers, HBM is touched once per
+// element (57 B/row Black-76, 73 B/row BSM).  Backward: one streaming elementwise kernel (25 B/row).
+// No tensor cores: the path is an fp64 transcendental chain, not a contraction.
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <new>
+
+#include "../../include/pivot_iv.h"
+#include "lbr_device.cuh"
+
+namespace pivot {
+
+constexpr int kFwdThreads = 128;
+constexpr int kBwdThreads = 256;
+constexpr int kHouseholderSteps = 2;  // north_star: two Householder(3) steps
+
+// ---------------------------------------------------------------------------------------------------------------
+// Forward kernel.  ROWS rows per thread: ROWS = 2 reads each input array with one 16-byte load (double2) per thread,
+// a warp covering 512 contiguous bytes per array; ROWS = 1 is the 8-byte-aligned fallback and the tail.
+// ---------------------------------------------------------------------------------------------------------------
+template <bool BSM, bool ZONES>
+__device__ __forceinline__ void solve_and_store(int64_t i, double S, double K, double tau, double r, double q, double P,
+                                                double flag, double* __restrict__ sigma, double* __restrict__ vega,
+                                                uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
+  const RowOut o = lbr_row<BSM, kHouseholderSteps>(S, K, tau, r, q, P, flag);
+  __stcs(sigma + i, o.sigma);
+  __stcs(vega + i, o.vega);
+  status[i] = o.status;
+  if (ZONES) zone[i] = o.zone;
+}
+
+template <bool BSM, bool ZONES>
+__global__ void __launch_bounds__(kFwdThreads)
+forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __restrict__ sigma,
+                      double* __restrict__ vega, uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
+  const int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+  solve_and_store<BSM, ZONES>(i, __ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(in.P + i),
+                              __ldcs(in.flag + i), sigma, vega, status, zone);
+}
+
+// 2 rows per thread, 16-byte loads / stores.  n2 = number of row pairs.
+template <bool BSM, bool ZONES>
+__global__ void __launch_bounds__(kFwdThreads)
+forward_kernel_vec2(pivot_iv_inputs in, int64_t n2, double* __restrict__ sigma, double* __restrict__ vega,
+                    uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n2) return;
+  const double2 S = __ldcs(reinterpret_cast<const double2*>(in.S_or_F) + j);
+  const double2 K = __ldcs(reinterpret_cast<const double2*>(in.K) + j);
+  const double2 T = __ldcs(reinterpret_cast<const double2*>(in.tau) + j);
+  const double2 P = __ldcs(reinterpret_cast<const double2*>(in.P) + j);
+  const double2 f = __ldcs(reinterpret_cast<const double2*>(in.flag) + j);
+  double2 r = make_double2(0.0, 0.0), q = make_double2(0.0, 0.0);
+  if (BSM) {
+    r = __ldcs(reinterpret_cast<const double2*>(in.r) + j);
+    q = __ldcs(reinterpret_cast<const double2*>(in.q) + j);
+  }
+  const RowOut a = lbr_row<BSM, kHouseholderSteps>(S.x, K.x, T.x, r.x, q.x, P.x, f.x);
+  const RowOut b = lbr_row<BSM, kHouseholderSteps>(S.y, K.y, T.y, r.y, q.y, P.y, f.y);
+  __stcs(reinterpret_cast<double2*>(sigma) + j, make_double2(a.sigma, b.sigma));
+  __stcs(reinterpret_cast<double2*>(vega) + j, make_double2(a.vega, b.vega));
+  reinterpret_cast<uchar2*>(status)[j] = make_uchar2(a.status, b.status);
+  if (ZONES) reinterpret_cast<char2*>(zone)[j] = make_char2(a.zone, b.zone);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Backward kernel: grad_P = gate * grad_sigma / vega  (eq.(8)-(10)); 25 B/row, HBM-bound.
+// ---------------------------------------------------------------------------------------------------------------
+template <int MODE>
+__device__ __forceinline__ double backward_row(double gs, double V, uint8_t st, double floor_, double floor2) {
+  if (MODE == PIVOT_GATE_MASK) {
+    const bool on = (st == PIVOT_ST_OK) && (fabs(V) > floor_);
+    return on ? __ddiv_rn(gs, V) : 0.0;
+  } else {
+    const double den = __dadd_rn(__dmul_rn(V, V), floor2);
+    const bool on = (st == PIVOT_ST_OK) && (den > 0.0);
+    return on ? __ddiv_rn(__dmul_rn(gs, V), den) : 0.0;
+  }
+}
+
+// 4 rows per thread per iteration (two 16-byte loads per fp64 array, one 4-byte status load), grid-stride.
+template <int MODE>
+__global__ void __launch_bounds__(kBwdThreads)
+backward_kernel_vec4(const double* __restrict__ gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
+                     double floor_, int64_t n4, double* __restrict__ gP) {
+  const double floor2 = __dmul_rn(floor_, floor_);
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n4; j += stride) {
+    const double2 g0 = __ldcs(reinterpret_cast<const double2*>(gs) + 2 * j);
+    const double2 g1 = __ldcs(reinterpret_cast<const double2*>(gs) + 2 * j + 1);
+    const double2 v0 = __ldcs(reinterpret_cast<const double2*>(vega) + 2 * j);
+    const double2 v1 = __ldcs(reinterpret_cast<const double2*>(vega) + 2 * j + 1);
+    const uchar4 st = __ldcs(reinterpret_cast<const uchar4*>(status) + j);
+    double2 o0, o1;
+    o0.x = backward_row<MODE>(g0.x, v0.x, st.x, floor_, floor2);
+    o0.y = backward_row<MODE>(g0.y, v0.y, st.y, floor_, floor2);
+    o1.x = backward_row<MODE>(g1.x, v1.x, st.z, floor_, floor2);
+    o1.y = backward_row<MODE>(g1.y, v1.y, st.w, floor_, floor2);
+    __stcs(reinterpret_cast<double2*>(gP) + 2 * j, o0);
+    __stcs(reinterpret_cast<double2*>(gP) + 2 * j + 1, o1);
+  }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(kBwdThreads)
+backward_kernel_scalar(const double* __restrict__ gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
+                       double floor_, int64_t begin, int64_t n, double* __restrict__ gP) {
+  const double floor2 = __dmul_rn(floor_, floor_);
+  const int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) gP[i] = backward_row<MODE>(gs[i], vega[i], status[i], floor_, floor2);
+}
+
+// fp64-pipe probe: 8 independent DFMA chains per thread
+__global__ void __launch_bounds__(256) dfma_probe_kernel(int64_t iters, double* sink) {
+  double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1e-3, a2 = a0 + 2e-3, a3 = a0 + 3e-3, a4 = a0 + 4e-3, a5 = a0 + 5e-3,
+         a6 = a0 + 6e-3, a7 = a0 + 7e-3;
+  const double m = 0.999999999, c = 1e-9;
+  for (int64_t i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  const double sum = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (sum == 123.456) sink[0] = sum;  // never true; keeps the chains alive
+}
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+}  // namespace pivot
+
+// ===============================================================================================================
+// C ABI
+// ===============================================================================================================
+using namespace pivot;
+
+namespace {
+
+template <bool BSM, bool ZONES>
+int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
+                     cudaStream_t st) {
+  const bool vec = aligned16(in.S_or_F) && aligned16(in.K) && aligned16(in.tau) && aligned16(in.P) &&
+                   aligned16(in.flag) && aligned16(sigma) && aligned16(vega) &&
+                   (!BSM || (aligned16(in.r) && aligned16(in.q))) &&
+                   ((reinterpret_cast<uintptr_t>(status) & 1u) == 0) &&
+                   (!ZONES || (reinterpret_cast<uintptr_t>(zone) & 1u) == 0);
+  int64_t done = 0;
+  if (vec && n >= 2) {
+    const int64_t n2 = n / 2;
+    const int64_t blocks = (n2 + kFwdThreads - 1) / kFwdThreads;
+    forward_kernel_vec2<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, n2, sigma, vega, status, zone);
+    done = 2 * n2;
+  }
+  if (done < n) {
+    const int64_t rem = n - done;
+    const int64_t blocks = (rem + kFwdThreads - 1) / kFwdThreads;
+    forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, done, n, sigma, vega, status, zone);
+  }
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
+                 bool zones, cudaStream_t st) {
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (n == 0) return PIVOT_OK;
+  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status || (zones && !zone))
+    return PIVOT_ERR_NULL;
+  if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;  // grid.x limit at 2 rows/thread
+  const bool bsm = in->r != nullptr;
+  if (bsm) return zones ? launch_forward_t<true, true>(*in, n, sigma, vega, status, zone, st)
+                        : launch_forward_t<true, false>(*in, n, sigma, vega, status, zone, st);
+  return zones ? launch_forward_t<false, true>(*in, n, sigma, vega, status, zone, st)
+               : launch_forward_t<false, false>(*in, n, sigma, vega, status, zone, st);
+}
+
+int g_sm_count = 0;
+int sm_count() {
+  if (g_sm_count == 0) {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+      sms = 148;
+    g_sm_count = sms;
+  }
+  return g_sm_count;
+}
+
+template <int MODE>
+int launch_backward_t(const double* gs, const double* vega, const uint8_t* status, double floor_, int64_t n, double* gP,
+                      cudaStream_t st) {
+  const bool vec = aligned16(gs) && aligned16(vega) && aligned16(gP) && ((reinterpret_cast<uintptr_t>(status) & 3u) == 0);
+  int64_t done = 0;
+  if (vec && n >= 4) {
+    const int64_t n4 = n / 4;
+    int64_t blocks = (n4 + kBwdThreads - 1) / kBwdThreads;
+    const int64_t cap = (int64_t)sm_count() * 8 * 4;  // 8 resident CTAs of 256 threads per SM, 4 waves' worth
+    if (blocks > cap) blocks = cap;
+    backward_kernel_vec4<MODE><<<(unsigned)blocks, kBwdThreads, 0, st>>>(gs, vega, status, floor_, n4, gP);
+    done = 4 * n4;
+  }
+  if (done < n) {
+    const int64_t rem = n - done;
+    const int64_t blocks = (rem + kBwdThreads - 1) / kBwdThreads;
+    backward_kernel_scalar<MODE><<<(unsigned)blocks, kBwdThreads, 0, st>>>(gs, vega, status, floor_, done, n, gP);
+  }
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int backward_impl(const double* gs, const double* vega, const uint8_t* status, double floor_, int mode, int64_t n,
+                  double* gP, cudaStream_t st) {
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE) return PIVOT_ERR_BAD_MODE;
+  if (!(floor_ >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
+  if (n == 0) return PIVOT_OK;
+  if (!gs || !vega || !status || !gP) return PIVOT_ERR_NULL;
+  if (n > ((int64_t)1 << 38)) return PIVOT_ERR_BAD_N;
+  return mode == PIVOT_GATE_MASK ? launch_backward_t<PIVOT_GATE_MASK>(gs, vega, status, floor_, n, gP, st)
+                                 : launch_backward_t<PIVOT_GATE_ATTENUATE>(gs, vega, status, floor_, n, gP, st);
+}
+
+}  // namespace
+
+extern "C" {
+
+int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                     pivot_iv_stream stream) {
+  return forward_impl(in, n, sigma, vega, status, nullptr, false, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                           int8_t* zone, pivot_iv_stream stream) {
+  return forward_impl(in, n, sigma, vega, status, zone, true, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int pivot_iv_backward(const double* grad_sigma, const double* vega, const uint8_t* status, double vega_floor, int mode,
+                      int64_t n, double* grad_P, pivot_iv_stream stream) {
+  return backward_impl(grad_sigma, vega, status, vega_floor, mode, n, grad_P, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivot_iv_stream stream) {
+  if (!sink || !fma_count_out) return PIVOT_ERR_NULL;
+  if (iters <= 0) return PIVOT_ERR_BAD_ARG;
+  const int blocks = sm_count() * 8, threads = 256;
+  dfma_probe_kernel<<<blocks, threads, 0, reinterpret_cast<cudaStream_t>(stream)>>>(iters, sink);
+  *fma_count_out = (double)iters * 8.0 * (double)blocks * (double)threads;
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int pivot_iv_launches_per_forward(void) { return 1; }
+int pivot_iv_launches_per_backward(void) { return 1; }
+
+const char* pivot_iv_strerror(int code) {
+  switch (code) {
+    case PIVOT_OK: return "ok";
+    case PIVOT_ERR_NULL: return "a required pointer is NULL";
+    case PIVOT_ERR_BAD_N: return "n is negative or too large";
+    case PIVOT_ERR_BAD_MODE: return "mode must be PIVOT_GATE_MASK (0) or PIVOT_GATE_ATTENUATE (1)";
+    case PIVOT_ERR_BAD_FLOOR: return "vega_floor must be a non-negative number";
+    case PIVOT_ERR_MIXED_RQ: return "r and q must both be NULL (Black-76) or both non-NULL (BSM)";
+    case PIVOT_ERR_CUDA: return "CUDA runtime error";
+    case PIVOT_ERR_BAD_ARG: return "invalid argument";
+    default: return "unknown pivot_iv error code";
+  }
+}
+
+int pivot_iv_version(void) { return PIVOT_IV_VERSION; }
+
+}  // extern "C"
+
+// ===============================================================================================================
+// Host-buffer pipeline: chunked H2D -> forward [-> backward] -> D2H, one stream per slot so that the copy engines
+// and the SMs overlap across chunks (streaming label generation over batches of rows).
+// ===============================================================================================================
+struct pivot_iv_pipeline {
+  int device = 0;
+  int64_t chunk = 0;
+  int nslots = 0;
+  cudaStream_t streams[8] = {};
+  double* dbl[8] = {};   // per slot: 11 fp64 arrays of `chunk` rows: S,K,tau,r,q,P,flag,sigma,vega,gs,gP
+  uint8_t* st[8] = {};   // per slot: status bytes
+};
+
+namespace {
+
+#define PIVOT_CUDA_TRY(expr)                    \
+  do {                                          \
+    if ((expr) != cudaSuccess) {                \
+      (void)cudaGetLastError();                 \
+      return PIVOT_ERR_CUDA;                    \
+    }                                           \
+  } while (0)
+
+int pipeline_run(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* gs, double floor_, int mode, bool bwd,
+                 int64_t n, double* sigma, double* vega, uint8_t* status, double* gP) {
+  if (!p || !in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (bwd) {
+    if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE) return PIVOT_ERR_BAD_MODE;
+    if (!(floor_ >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
+  }
+  if (n == 0) return PIVOT_OK;
+  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status) return PIVOT_ERR_NULL;
+  if (bwd && (!gs || !gP)) return PIVOT_ERR_NULL;
+  int prev = 0;
+  PIVOT_CUDA_TRY(cudaGetDevice(&prev));
+  PIVOT_CUDA_TRY(cudaSetDevice(p->device));
+  const bool bsm = in->r != nullptr;
+  const int64_t C = p->chunk;
+  int rc = PIVOT_OK;
+  int64_t c = 0;
+  for (int64_t off = 0; off < n && rc == PIVOT_OK; off += C, ++c) {
+    const int slot = (int)(c % p->nslots);
+    const int64_t m = (n - off < C) ? (n - off) : C;
+    cudaStream_t s = p->streams[slot];
+    double* base = p->dbl[slot];
+    double* d[11];
+    for (int k = 0; k < 11; ++k) d[k] = base + (int64_t)k * C;
+    const size_t bytes = (size_t)m * sizeof(double);
+    const double* src[7] = {in->S_or_F, in->K, in->tau, in->r, in->q, in->P, in->flag};
+    for (int k = 0; k < 7; ++k) {
+      if (!src[k]) continue;
+      if (cudaMemcpyAsync(d[k], src[k] + off, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = PIVOT_ERR_CUDA;
+    }
+    if (bwd && cudaMemcpyAsync(d[9], gs + off, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = PIVOT_ERR_CUDA;
+    if (rc != PIVOT_OK) break;
+    pivot_iv_inputs din{d[0], d[1], d[2], bsm ? d[3] : nullptr, bsm ? d[4] : nullptr, d[5], d[6]};
+    rc = forward_impl(&din, m, d[7], d[8], p->st[slot], nullptr, false, s);
+    if (rc == PIVOT_OK && bwd) rc = backward_impl(d[9], d[8], p->st[slot], floor_, mode, m, d[10], s);
+    if (rc != PIVOT_OK) break;
+    if (cudaMemcpyAsync(sigma + off, d[7], bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaMemcpyAsync(vega + off, d[8], bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaMemcpyAsync(status + off, p->st[slot], (size_t)m, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        (bwd && cudaMemcpyAsync(gP + off, d[10], bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess))
+      rc = PIVOT_ERR_CUDA;
+  }
+  for (int k = 0; k < p->nslots; ++k)
+    if (cudaStreamSynchronize(p->streams[k]) != cudaSuccess) rc = PIVOT_ERR_CUDA;
+  if (rc == PIVOT_ERR_CUDA) (void)cudaGetLastError();
+  (void)cudaSetDevice(prev);
+  return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pivot_iv_pipeline_create(pivot_iv_pipeline** out, int device, int64_t chunk_rows, int n_slots) {
+  if (!out) return PIVOT_ERR_NULL;
+  *out = nullptr;
+  if (chunk_rows <= 0 || n_slots < 1 || n_slots > 8) return PIVOT_ERR_BAD_ARG;
+  int prev = 0;
+  PIVOT_CUDA_TRY(cudaGetDevice(&prev));
+  if (device < 0) device = prev;
+  if (cudaSetDevice(device) != cudaSuccess) { (void)cudaGetLastError(); return PIVOT_ERR_BAD_ARG; }
+  pivot_iv_pipeline* p = new (std::nothrow) pivot_iv_pipeline();
+  if (!p) { (void)cudaSetDevice(prev); return PIVOT_ERR_CUDA; }
+  p->device = device;
+  p->chunk = (chunk_rows + 1) & ~(int64_t)1;  // even, keeps every array of a slot 16-byte aligned
+  p->nslots = n_slots;
+  int rc = PIVOT_OK;
+  for (int k = 0; k < n_slots && rc == PIVOT_OK; ++k) {
+    if (cudaStreamCreateWithFlags(&p->streams[k], cudaStreamNonBlocking) != cudaSuccess ||
+        cudaMalloc(&p->dbl[k], (size_t)p->chunk * 11 * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&p->st[k], (size_t)p->chunk) != cudaSuccess)
+      rc = PIVOT_ERR_CUDA;
+  }
+  (void)cudaSetDevice(prev);
+  if (rc != PIVOT_OK) { (void)cudaGetLastError(); pivot_iv_pipeline_destroy(p); return rc; }
+  *out = p;
+  return PIVOT_OK;
+}
+
+int pivot_iv_pipeline_destroy(pivot_iv_pipeline* p) {
+  if (!p) return PIVOT_OK;
+  int prev = 0;
+  (void)cudaGetDevice(&prev);
+  (void)cudaSetDevice(p->device);
+  for (int k = 0; k < 8; ++k) {
+    if (p->streams[k]) { (void)cudaStreamSynchronize(p->streams[k]); (void)cudaStreamDestroy(p->streams[k]); }
+    if (p->dbl[k]) (void)cudaFree(p->dbl[k]);
+    if (p->st[k]) (void)cudaFree(p->st[k]);
+  }
+  (void)cudaSetDevice(prev);
+  delete p;
+  return PIVOT_OK;
+}
+
+int pivot_iv_forward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega,
+                          uint8_t* status) {
+  return pipeline_run(p, in, nullptr, 0.0, 0, false, n, sigma, vega, status, nullptr);
+}
+
+int pivot_iv_forward_backward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* grad_sigma,
+                                   double vega_floor, int mode, int64_t n, double* sigma, double* vega,
+                                   uint8_t* status, double* grad_P) {
+  return pipeline_run(p, in, grad_sigma, vega_floor, mode, true, n, sigma, vega, status, grad_P);
+}
+
+}  // extern "C"

@@ -1,0 +1,224 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI (ctypes binding), against the CPU oracle on
+the same seeded inputs, element by element.  Sizes: what the oracle finishes in seconds, spanning many tiles and ragged
+tails; and at the bench's full size (2^26 rows) on sampled rows."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_17065_b200 import workloads as wl
+import paper_2606_17065_b200 as pv
+from oracle import pyoracle as po
+from tests.parity_util import KEYS, compare_backward, compare_forward, gpu_forward, oracle_forward, to_device, to_numpy
+
+pytestmark = pytest.mark.gpu
+
+
+def _fwd_both(cfg):
+    d = to_device(cfg)
+    g = tuple(t.cpu().numpy() for t in gpu_forward(d))
+    c = to_numpy(cfg)
+    o = oracle_forward(c)
+    return d, c, g, o
+
+
+def test_config0_black76_with_invalid_rows():
+    cfg = wl.config0()
+    d, c, g, o = _fwd_both(cfg)
+    st = compare_forward(g, o, c)
+    pert = c["perturbed"]
+    assert np.all(np.isin(g[2][pert], (1, 2))) and np.isnan(g[0][pert]).all()      # perturbed rows -> NaN
+    assert st["ok"] > 0.8 * st["n"]
+    # sanity against the drawn sigma on OTM rows with a healthy vega
+    m = (g[2] == 0) & (g[1] > 1.0) & (((c["flag"] > 0) & (c["K"] >= c["SorF"])) | ((c["flag"] < 0) & (c["K"] <= c["SorF"])))
+    assert np.max(np.abs(g[0][m] / c["sigma_true"][m] - 1)) < 1e-8
+
+
+@pytest.mark.parametrize("solve_only", [False, True])
+def test_config1_four_zone_stress(solve_only):
+    cfg = wl.config1(1 << 22, solve_only=solve_only)
+    d, c, g, o = _fwd_both(cfg)
+    st = compare_forward(g, o, c)
+    _, _, _, zone = pv.pivot_iv_forward_zones(*[d[k] for k in KEYS])
+    z = zone.cpu().numpy()
+    ok = g[2] == 0
+    assert all((z[ok] == k).sum() > 1000 for k in range(4)), "all four LBR zones must be exercised"
+    assert np.all(z[~ok] == -1)
+    if solve_only:
+        assert st["ok"] > 0.6 * st["n"]
+
+
+def test_config2_bsm_chains():
+    cfg = wl.config2(days=96)   # 96 x 40 x 400 = 1,536,000 rows
+    d, c, g, o = _fwd_both(cfg)
+    st = compare_forward(g, o, c)
+    assert st["ok"] > 0.7 * st["n"]
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_config3_forward_backward(mode):
+    cfg = wl.config3(1 << 20)
+    d, c, g, o = _fwd_both(cfg)
+    compare_forward(g, o, c)
+    sig, vega, status = gpu_forward(d)
+    gP = pv.pivot_iv_backward(d["grad_sigma"], vega, status, 1e-8, mode).cpu().numpy()
+    st = compare_backward(gP, c["grad_sigma"], g[1], g[2], o[1], 1e-8, mode)
+    low = c["low_vega"] & (g[2] == 0)
+    assert (g[1][low] < 1e-8).mean() > 0.9       # the low-vega slice really is below the floor
+    assert st["gate_on"] > 0.5 * gP.size
+    if mode == 0:
+        assert np.all(gP[low & (g[1] <= 1e-8)] == 0.0)
+        # implicit identity: grad_P * vega == grad_sigma on gate-on rows (eq.(7))
+        on = (g[2] == 0) & (g[1] > 1e-8)
+        assert np.max(np.abs(gP[on] * g[1][on] / c["grad_sigma"][on] - 1)) < 1e-15 * 4
+    # in place (grad_P aliasing grad_sigma) gives the same bits
+    buf = d["grad_sigma"].clone()
+    pv.pivot_iv_backward(buf, vega, status, 1e-8, mode, out=buf)
+    assert np.array_equal(buf.cpu().numpy().view(np.uint64), gP.view(np.uint64))
+
+
+def test_backward_bit_exact_given_same_inputs():
+    """Fed the oracle's own vega/status, the backward kernel reproduces the oracle's grad_P bit for bit."""
+    rng = np.random.default_rng(7)
+    n = 1_000_003
+    vega = np.exp(rng.uniform(np.log(1e-30), np.log(1e3), n)); vega[::97] = 0.0; vega[5::101] = 1e-8
+    status = rng.integers(0, 5, n).astype(np.uint8); status[rng.random(n) < 0.7] = 0
+    gs = rng.standard_normal(n); gs[::89] = 0.0; gs[3::1013] = np.nan
+    for floor in (0.0, 1e-8, 1e-4):
+        for mode in (0, 1):
+            ref = po.backward(gs, vega, status, floor, mode)
+            got = pv.pivot_iv_backward(torch.from_numpy(gs).cuda(), torch.from_numpy(vega).cuda(),
+                                       torch.from_numpy(status).cuda(), floor, mode).cpu().numpy()
+            assert np.array_equal(got.view(np.uint64), ref.view(np.uint64))
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 127, 128, 129, 255, 257, 65537])
+def test_ragged_sizes_and_unaligned_pointers(n):
+    """Empty and ragged inputs; odd element offsets force the 8-byte-aligned scalar path; results identical."""
+    cfg = wl.config1(n + 3, seed=11) if n else wl.config1(4, seed=11)
+    d = to_device(cfg)
+    if n == 0:
+        e = torch.empty(0, dtype=torch.float64, device="cuda")
+        s, v, st = pv.pivot_iv_forward(e, e, e, e, e)
+        assert s.numel() == 0
+        assert pv.pivot_iv_backward(e, e, torch.empty(0, dtype=torch.uint8, device="cuda"), 1e-8, 0).numel() == 0
+        return
+    full = gpu_forward(d)
+    for off in (0, 1):
+        sl = {k: d[k][off:off + n] for k in KEYS}
+        # out buffers with the same misalignment
+        so = torch.empty(n + 1, dtype=torch.float64, device="cuda")[off:off + n]
+        vo = torch.empty(n + 1, dtype=torch.float64, device="cuda")[off:off + n]
+        sto = torch.empty(n + 1, dtype=torch.uint8, device="cuda")[off:off + n]
+        s, v, st = pv.pivot_iv_forward(*[sl[k].contiguous() if False else sl[k] for k in KEYS], out=(so, vo, sto))
+        assert torch.equal(st, full[2][off:off + n])
+        assert np.array_equal(s.cpu().numpy().view(np.uint64), full[0][off:off + n].cpu().numpy().view(np.uint64))
+        assert np.array_equal(v.cpu().numpy().view(np.uint64), full[1][off:off + n].cpu().numpy().view(np.uint64))
+        gs = torch.randn(n + 1, dtype=torch.float64, device="cuda")[off:off + n]
+        a = pv.pivot_iv_backward(gs, v, st, 1e-8, 0)
+        b = pv.pivot_iv_backward(gs.clone(), v.clone(), st.clone(), 1e-8, 0)
+        assert torch.equal(a, b)
+    c = to_numpy({k: d[k][:n] for k in KEYS})
+    o = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"])
+    compare_forward(tuple(t[:n].cpu().numpy() for t in full), o, c)
+
+
+def test_edge_rows_match_oracle():
+    """The degenerate cases of the method: ATM (x = 0), prices at / next to the bounds, bad inputs, extreme moneyness."""
+    nan, inf = float("nan"), float("inf")
+    rows = [  # F, K, T, P, flag
+        (100, 100, 1.0, 5.0, 1), (100, 100, 0.25, 1e-9, -1), (100, 100, 2.0, 99.9999, 1),
+        (100, 90, 1.0, 9.999, 1), (100, 90, 1.0, 10.0, 1), (100, 90, 1.0, np.nextafter(10.0, 11), 1), (100, 90, 1.0, 99.99, 1),
+        (100, 90, 1.0, 100.0, 1), (100, 90, 1.0, 0.0, -1), (100, 90, 1.0, 1e-320, -1), (100, 90, 1.0, -1e-9, -1),
+        (100, 90, 1.0, 89.9, -1), (100, 90, 1.0, 90.0, -1), (100, 90, 0.0, 12.0, 1), (100, 90, -1.0, 12.0, 1),
+        (100, 90, nan, 12.0, 1), (100, 90, inf, 12.0, 1), (0.0, 90, 1.0, 12.0, 1), (100, -90, 1.0, 12.0, 1),
+        (nan, 90, 1.0, 12.0, 1), (100, 90, 1.0, nan, 1), (100, 90, 1.0, inf, 1), (100, 90, 1.0, 12.0, 0), (100, 90, 1.0, 12.0, 2),
+        (1e-300, 1e300, 1.0, 1e-301, 1), (1e300, 1e-300, 1.0, 1e299, -1), (1e-130, 1e130, 1.0, 1e-135, 1),
+        (100, 100 * (1 + 1e-15), 1.0, 3.0, 1), (100, 100.0001, 1e-4, 0.01, 1), (100, 150, 1 / 365, 1e-200, 1),
+        (100, 101, 1.0, 1e-300, 1), (100, 3000, 1.0, 99.0, 1),
+    ]
+    a = np.array(rows, dtype=np.float64)
+    cols = [np.ascontiguousarray(a[:, j]) for j in range(5)]
+    o = po.forward(*cols)
+    g = pv.pivot_iv_forward(*[torch.from_numpy(x).cuda() for x in cols])
+    g = tuple(t.cpu().numpy() for t in g)
+    c = dict(zip(KEYS, cols)); c["r"] = None; c["q"] = None
+    compare_forward(g, o, c)
+    assert set(np.unique(g[2])) == {0, 1, 2, 3, 4}
+
+
+def test_bsm_bad_rates_and_mixed_rq_error():
+    d = to_device(wl.config2(days=1, expiries=2, strikes=50))
+    r = d["r"].clone(); r[3] = float("nan")
+    q = d["q"].clone(); q[7] = float("inf")
+    s, v, st = pv.pivot_iv_forward(d["SorF"], d["K"], d["tau"], d["P"], d["flag"], r=r, q=q)
+    assert st[3].item() == 3 and st[7].item() == 3
+    with pytest.raises(pv.PivotError):
+        pv.pivot_iv_forward(d["SorF"], d["K"], d["tau"], d["P"], d["flag"], r=r, q=None)
+    with pytest.raises(pv.PivotError):
+        pv.pivot_iv_backward(s, v, st, -1.0, 0)
+    with pytest.raises(pv.PivotError):
+        pv.pivot_iv_backward(s, v, st, 1e-8, 2)
+
+
+def test_full_size_headline_sampled():
+    """BASELINE.json's full size (2^26 rows, inputs as config 1/4), in the launch configuration bench.py times:
+    sampled rows against the oracle one by one, plus properties that hold at any size."""
+    n = 1 << 26
+    cfg = wl.config4(n, device="cuda")
+    d = cfg
+    sig, vega, status = gpu_forward(d)
+    gsg = torch.randn(n, dtype=torch.float64, device="cuda")
+    gP = pv.pivot_iv_backward(gsg, vega, status, 1e-8, 0)
+    g = torch.Generator(device="cuda"); g.manual_seed(123)
+    idx = torch.randint(0, n, (300_000,), device="cuda", generator=g)
+    idx = torch.cat([idx, torch.arange(0, 4096, device="cuda"), torch.arange(n - 4096, n, device="cuda")])
+    c = to_numpy({k: d[k] for k in KEYS}, idx)
+    c["r"] = None; c["q"] = None
+    o = oracle_forward(c)
+    gsub = (sig[idx].cpu().numpy(), vega[idx].cpu().numpy(), status[idx].cpu().numpy())
+    st = compare_forward(gsub, o, c)
+    compare_backward(gP[idx].cpu().numpy(), gsg[idx].cpu().numpy(), gsub[1], gsub[2], o[1], 1e-8, 0)
+    # any-size properties: NaN iff status in 1..3; vega >= 0; off-gate gradient exactly 0
+    assert torch.equal(torch.isnan(sig), (status >= 1) & (status <= 3))
+    assert bool((vega >= 0).all()) and bool((vega[status != 0] == 0).all())
+    off = (status != 0) | (vega <= 1e-8)
+    assert bool((gP[off] == 0).all())
+    assert st["ok"] > 0.2 * idx.numel()
+
+
+def test_host_pipeline_matches_device_path():
+    """pivot_iv_forward_host / _forward_backward_host (chunked H2D -> kernels -> D2H) give the device path's bits."""
+    cfg = wl.config3(300_001, seed=9)
+    d = to_device(cfg)
+    sig, vega, status = gpu_forward(d)
+    gP = pv.pivot_iv_backward(d["grad_sigma"], vega, status, 1e-8, 1)
+    pipe = pv.Pipeline(chunk_rows=65_536, n_slots=3)
+    hs = {k: cfg[k].pin_memory() for k in KEYS}
+    s2, v2, st2 = pipe.forward_host(*[hs[k] for k in KEYS])
+    assert torch.equal(st2, status.cpu())
+    assert np.array_equal(s2.numpy().view(np.uint64), sig.cpu().numpy().view(np.uint64))
+    assert np.array_equal(v2.numpy().view(np.uint64), vega.cpu().numpy().view(np.uint64))
+    s3, v3, st3, g3 = pipe.forward_backward_host(*[hs[k] for k in KEYS], cfg["grad_sigma"].pin_memory(), 1e-8, 1)
+    assert np.array_equal(g3.numpy().view(np.uint64), gP.cpu().numpy().view(np.uint64))
+    # BSM through the pipeline
+    c2 = wl.config2(days=2, expiries=5, strikes=401)
+    d2 = to_device(c2)
+    ref = gpu_forward(d2)
+    out = pipe.forward_host(*[c2[k] for k in KEYS], r=c2["r"], q=c2["q"])
+    assert np.array_equal(out[0].numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
+    pipe.close()
+
+
+def test_streams_and_preallocated_outputs():
+    cfg = wl.config0(10_000)
+    d = to_device(cfg)
+    ref = gpu_forward(d)
+    s = torch.cuda.Stream()
+    out = tuple(torch.empty_like(t) for t in ref)
+    with torch.cuda.stream(s):
+        pv.pivot_iv_forward(*[d[k] for k in KEYS], out=out, stream=s)
+    s.synchronize()
+    assert np.array_equal(out[0].cpu().numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
+    assert torch.equal(out[2], ref[2])
