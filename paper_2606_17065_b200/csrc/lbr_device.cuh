@@ -136,15 +136,17 @@ __device__ __forceinline__ double rc_control(int side, double H, double yl, doub
 }
 
 struct NormSolve {
-  double s;
-  double E;   // (h^2+t^2)/2 is NOT returned at the final s; the caller evaluates vega itself
+  double s;     // total volatility after NITER Householder steps
+  double vfin;  // b'(x, s) = phi0 exp(-(h^2+t^2)/2) at that s (for vega)
   int zone;
 };
 
 // Solve b(x,s) = beta, x <= 0, 0 < beta < bmax; bbar = bmax - beta supplied exactly.
-// Stage 0: boundary point s_c.  Stage 1: zone node (s_l or s_u) and the rational seed.  Stages 2..1+NITER: Householder(3).
+// Stage 0: boundary point s_c.  Stage 1: zone node (s_l or s_u) and the rational seed.  Stages 2..1+NITER:
+// Householder(3).  Stage 2+NITER: b' at the final s.  One copy of the erfcx pair, of exp and of log serves all stages.
 template <int NITER>
 __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bmax, double bbar) {
+  constexpr int kLast = 2 + NITER;
   const double a = -x;
   const double sc = sqrt(2.0 * a);
   const double vc = kPhi0 * bmax;  // b'(x, s_c) = phi0 e^{-|x|/2}
@@ -152,11 +154,13 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
   double s = (a == 0.0) ? su : sc;  // evaluation point of the current stage, then the iterate (x = 0: no stage 0)
   bool lower = false;
   int zone = 2, kind = KIND_LINEAR;
-  double ln_beta = 0.0, ln_bbar = 0.0;
+  double ln_target = 0.0;  // ln beta (lower tail) or ln(b_max - beta) (upper tail)
+  double vfin = 0.0;
 
 #pragma unroll 1
-  for (int stage = (a == 0.0) ? 1 : 0; stage < 2 + NITER; ++stage) {
+  for (int stage = (a == 0.0) ? 1 : 0; stage <= kLast; ++stage) {
     // ---------------- common part: W (or Wbar) and E at the point s ----------------
+    const bool fin = stage == kLast;
     const double rs = 1.0 / s;
     const double h = (a == 0.0) ? 0.0 : x * rs;   // <= 0
     const double t = 0.5 * s;
@@ -165,45 +169,50 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
     const bool small = t < kSmallT;
     const double z1 = (stage == 0) ? 0.0 : (ah - t) * kInvSqrt2;   // at s_c, |h| = t exactly (rounding must not flip it)
     const bool neg = z1 < 0.0;
-    double e1, e2;
-    erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
-    double Wd;          // z1 >= 0 or small: W;  z1 < 0: Wbar
-    bool have_W;        // Wd holds W (true) or Wbar (false)
-    if (small) {
-      const double w0 = kSqrtPiOver2 * e1;
-      const double w1 = fma(h, w0, 1.0);
-      const double w2 = fma(h, w1, w0);
-      const double w3 = fma(h, w2, 2.0 * w1);
-      const double w4 = fma(h, w3, 3.0 * w2);
-      const double w5 = fma(h, w4, 4.0 * w3);
-      const double w6 = fma(h, w5, 5.0 * w4);
-      const double w7 = fma(h, w6, 6.0 * w5);
-      const double w8 = fma(h, w7, 7.0 * w6);
-      const double w9 = fma(h, w8, 8.0 * w7);
-      const double w10 = fma(h, w9, 9.0 * w8);
-      const double w11 = fma(h, w10, 10.0 * w9);
-      const double t2 = t * t;
-      double acc = w11 * (1.0 / 39916800.0);
-      acc = fma(acc, t2, w9 * (1.0 / 362880.0));
-      acc = fma(acc, t2, w7 * (1.0 / 5040.0));
-      acc = fma(acc, t2, w5 * (1.0 / 120.0));
-      acc = fma(acc, t2, w3 * (1.0 / 6.0));
-      acc = fma(acc, t2, w1);
-      Wd = s * acc;  // 2 t acc
-      have_W = true;
-    } else if (!neg) {
-      Wd = kSqrtPiOver2 * (e1 - e2);
-      have_W = true;
-    } else {
-      Wd = kSqrtPiOver2 * (e1 + e2);
-      have_W = false;
+    double Wd = 0.0;        // z1 >= 0 or small: W;  z1 < 0: Wbar
+    bool have_W = true;     // Wd holds W (true) or Wbar (false)
+    if (!fin) {
+      double e1, e2;
+      erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
+      if (small) {
+        const double w0 = kSqrtPiOver2 * e1;
+        const double w1 = fma(h, w0, 1.0);
+        const double w2 = fma(h, w1, w0);
+        const double w3 = fma(h, w2, 2.0 * w1);
+        const double w4 = fma(h, w3, 3.0 * w2);
+        const double w5 = fma(h, w4, 4.0 * w3);
+        const double w6 = fma(h, w5, 5.0 * w4);
+        const double w7 = fma(h, w6, 6.0 * w5);
+        const double w8 = fma(h, w7, 7.0 * w6);
+        const double w9 = fma(h, w8, 8.0 * w7);
+        const double w10 = fma(h, w9, 9.0 * w8);
+        const double w11 = fma(h, w10, 10.0 * w9);
+        const double t2 = t * t;
+        double acc = w11 * (1.0 / 39916800.0);
+        acc = fma(acc, t2, w9 * (1.0 / 362880.0));
+        acc = fma(acc, t2, w7 * (1.0 / 5040.0));
+        acc = fma(acc, t2, w5 * (1.0 / 120.0));
+        acc = fma(acc, t2, w3 * (1.0 / 6.0));
+        acc = fma(acc, t2, w1);
+        Wd = s * acc;  // 2 t acc
+      } else if (!neg) {
+        Wd = kSqrtPiOver2 * (e1 - e2);
+      } else {
+        Wd = kSqrtPiOver2 * (e1 + e2);
+        have_W = false;
+      }
     }
-    // 1/b' = sqrt(2 pi) e^{E}: needed by the node stage, by the b - beta objective, and when the available ratio is
-    // not the one the objective wants
+    // the one exp: 1/b' = sqrt(2 pi) e^{E} (node stage, b - beta objective, or when the available ratio is not the
+    // one the objective wants), or b' itself at the final s
     const bool want_W = (stage < 2) || (kind != KIND_UPPER);
-    const bool need_exp = (stage == 1) || (stage >= 2 && kind == KIND_LINEAR) || (stage >= 2 && want_W != have_W);
-    double inv_v = 0.0;
-    if (need_exp) inv_v = kSqrt2Pi * exp(E);
+    const bool need_exp = fin || (stage == 1) || (stage >= 2 && (kind == KIND_LINEAR || want_W != have_W));
+    double ex = 0.0;
+    if (need_exp) ex = exp(fin ? -E : E);
+    if (fin) {
+      vfin = kPhi0 * ex;
+      break;
+    }
+    const double inv_v = kSqrt2Pi * ex;
 
     if (stage == 0) {
       // ---------------- boundary: tangent at the inflection point hits 0 at s_l and b_max at s_u ----------------
@@ -221,6 +230,8 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
       s = lower ? sl : su;
       continue;
     }
+    double larg = 1.0;      // argument of the one log
+    bool need_log = false;
     if (stage == 1) {
       // ---------------- node (s_l or s_u) and the zone's rational seed ----------------
       const double sn = s, hn = h, tn = t;
@@ -281,14 +292,25 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
       }
       if (!(s > 0.0) || !is_fin(s)) s = sn;
       kind = (zone == 0) ? KIND_LOWER : ((zone == 3 && beta > 0.5 * bmax) ? KIND_UPPER : KIND_LINEAR);
-      if (kind == KIND_LOWER) ln_beta = log(beta);
-      if (kind == KIND_UPPER) ln_bbar = log(bbar);
+      if (kind != KIND_LINEAR) {
+        larg = (kind == KIND_LOWER) ? beta : bbar;
+        need_log = true;
+      }
+    } else if (kind != KIND_LINEAR) {
+      // the ratio this objective wants: W (lower tail) or Wbar (upper tail)
+      larg = (want_W == have_W) ? Wd : fma(bmax, inv_v, -Wd);
+      need_log = true;
+    }
+    double lg = 0.0;
+    if (need_log) lg = log(larg);
+    if (stage == 1) {
+      ln_target = lg;
       continue;
     }
     // ---------------- Householder(3) step on the zone's objective ----------------
     const double hr = h * rs;
-    const double B2 = fma(h, hr, -0.25 * s);                    // b''/b'
-    const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // b'''/b'
+    const double B2 = fma(h, hr, -0.25 * s);                    // b2 = b''/b'
+    const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // b3 = third derivative of b over b'
     double nu, h2, h3;
     if (kind == KIND_LINEAR) {
       // g = b - beta:  nu = (beta - b)/b'
@@ -297,19 +319,19 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
       h3 = B3;
     } else if (kind == KIND_LOWER) {
       // g = 1/ln b - 1/ln beta,  ln b = ln phi0 - E + ln W
-      const double W = have_W ? Wd : fma(bmax, inv_v, -Wd);
-      const double L = kLnPhi0 - E + log(W);
+      const double W = larg;
+      const double L = kLnPhi0 - E + lg;
       const double rLW = 1.0 / (L * W);
       const double lam = rLW * W, ub = rLW * L;  // 1/L, b'/b = 1/W
       const double k2 = fma(2.0, lam, 1.0);
-      nu = (ln_beta - L) * (L / ln_beta) * W;
+      nu = (ln_target - L) * (L / ln_target) * W;
       h2 = fma(-ub, k2, B2);
       h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
     } else {
       // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar
-      const double Wb = have_W ? fma(bmax, inv_v, -Wd) : Wd;
+      const double Wb = larg;
       const double gp = 1.0 / Wb;
-      nu = (kLnPhi0 - E + log(Wb) - ln_bbar) * Wb;
+      nu = (kLnPhi0 - E + lg - ln_target) * Wb;
       h2 = B2 + gp;
       h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
     }
@@ -317,7 +339,7 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
     if (!(ds > -0.5 * s)) ds = -0.5 * s;
     s += ds;
   }
-  return NormSolve{s, 0.0, zone};
+  return NormSolve{s, vfin, zone};
 }
 
 struct RowOut {
@@ -368,11 +390,9 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
     const double x = -log1p(__ddiv_rn(__dsub_rn(hi, lo), lo));
     const double bbar = __ddiv_rn(__dsub_rn(U, B), rootFK);
     const NormSolve ns = lbr_solve<NITER>(x, beta, bmax, bbar);
-    const double s = ns.s;
     const double rt = sqrt(tau);
-    const double h = (x == 0.0) ? 0.0 : x / s;
-    o.sigma = s / rt;
-    o.vega = D * rootFK * kPhi0 * exp(-0.5 * fma(h, h, 0.25 * s * s)) * rt;
+    o.sigma = ns.s / rt;
+    o.vega = D * rootFK * ns.vfin * rt;
     o.zone = (int8_t)ns.zone;
   }
   return o;

@@ -7,6 +7,7 @@
 
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <new>
 
 #include "../../include/pivot_iv.h"
@@ -16,6 +17,7 @@ namespace pivot {
 
 constexpr int kFwdThreads = 128;
 constexpr int kBwdThreads = 256;
+constexpr int kDefaultFwdRows = 1;
 constexpr int kHouseholderSteps = 2;  // north_star: two Householder(3) steps
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -140,6 +142,16 @@ using namespace pivot;
 
 namespace {
 
+// Tuning knob for the ncu A/B studies: PIVOT_IV_FWD_ROWS=1|2 selects rows per thread
+// (2 = 16-byte double2 loads, 1 = 8-byte loads).  Read once.
+int fwd_rows_per_thread() {
+  static const int v = [] {
+    const char* e = std::getenv("PIVOT_IV_FWD_ROWS");
+    return (e && e[0] == '2') ? 2 : ((e && e[0] == '1') ? 1 : kDefaultFwdRows);
+  }();
+  return v;
+}
+
 template <bool BSM, bool ZONES>
 int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
                      cudaStream_t st) {
@@ -149,7 +161,7 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
                    ((reinterpret_cast<uintptr_t>(status) & 1u) == 0) &&
                    (!ZONES || (reinterpret_cast<uintptr_t>(zone) & 1u) == 0);
   int64_t done = 0;
-  if (vec && n >= 2) {
+  if (vec && n >= 2 && fwd_rows_per_thread() == 2) {
     const int64_t n2 = n / 2;
     const int64_t blocks = (n2 + kFwdThreads - 1) / kFwdThreads;
     forward_kernel_vec2<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, n2, sigma, vega, status, zone);
