@@ -138,7 +138,7 @@ def main():
         f.write(f"// ninv tail : -Phi^-1(p) = u - R(1/(1+u)), u = sqrt(-2 ln p), p <= 0.345 (z >= 0.4), degree 7, max rel err {en:.2e}\n")
         f.write("#pragma once\nnamespace pivot {\n")
         f.write(f"constexpr double kErfcxC = {C64};\nconstexpr int kErfcxN = {N64};\n")
-        f.write("__device__ constexpr double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
+        f.write("__constant__ double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
         f.write(f"constexpr float kErfcxCf = {C32}f;\nconstexpr int kErfcxNf = {N32};\n")
         f.write("__device__ constexpr float kErfcxQf[kErfcxNf + 1] = {\n" + fmt(a32, 4, True) + "};\n")
         f.write("constexpr int kNinvN = 7;\n")

@@ -342,22 +342,22 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
   return NormSolve{s, vfin, zone};
 }
 
-struct RowOut {
-  double sigma, vega;
-  uint8_t status;
-  int8_t zone;
-};
-
-// Full row (Alg.1 l.1-3).  BSM = true: (S,K,tau,r,q,P,flag); false: Black-76 with discount factor 1.
+// Row prelude (Alg.1 l.1 and l.3; A.5 stages 1-2): normalisation, validity, reduction to an OTM call.
 // The status decision uses only correctly rounded IEEE operations issued through intrinsics, so it cannot be
 // contracted into FMAs and is bit-reproducible against any IEEE-754 implementation of the same sequence.
-template <bool BSM, int NITER>
-__device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, double r, double q, double P, double flag) {
-  RowOut o;
-  o.sigma = canonical_nan();
-  o.vega = 0.0;
-  o.zone = -1;
-  o.status = 3;
+struct Prelude {
+  double qrel;    // (hi - lo)/lo, hi = max(F,K), lo = min(F,K):  x = -log1p(qrel)
+  double beta;    // time value / sqrt(FK)
+  double bbar;    // (U - B)/sqrt(FK) = b_max - beta, formed without cancellation
+  double bmax;    // lo / sqrt(FK) = e^{x/2}
+  double scale;   // D sqrt(FK): vega = scale * b'(x,s) * sqrt(tau)
+  int status;
+};
+
+template <bool BSM>
+__device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau, double r, double q, double P,
+                                               double flag) {
+  Prelude p;
   bool bad = !(is_fin(SorF) && SorF > 0.0) || !(is_fin(K) && K > 0.0) || !(is_fin(tau) && tau > 0.0) || !is_fin(P) ||
              !(flag == 1.0 || flag == -1.0);
   double F = SorF, D = 1.0, B = P;
@@ -372,27 +372,45 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
   }
   const double rootFK = __dsqrt_rn(__dmul_rn(F, K));
   const double lo = fmin(F, K), hi = fmax(F, K);
-  const double bmax = __ddiv_rn(lo, rootFK);
-  if (!(is_fin(rootFK) && rootFK > 0.0) || !(bmax >= 0x1p-500)) bad = true;
+  p.bmax = __ddiv_rn(lo, rootFK);
+  if (!(is_fin(rootFK) && rootFK > 0.0) || !(p.bmax >= 0x1p-500)) bad = true;
   const bool call = flag > 0.0;
   const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
   const double U = call ? F : K;
   const double tv = __dsub_rn(B, iota);
-  const double beta = __ddiv_rn(tv, rootFK);
+  p.beta = __ddiv_rn(tv, rootFK);
   int st = 0;
   if (bad) st = 3;
   else if (B < iota) st = 1;
   else if (B >= U) st = 2;
-  else if (beta < 2.2250738585072014e-308) st = 4;
-  o.status = (uint8_t)st;
-  if (st == 4) o.sigma = 0.0;
-  if (st == 0) {
-    const double x = -log1p(__ddiv_rn(__dsub_rn(hi, lo), lo));
-    const double bbar = __ddiv_rn(__dsub_rn(U, B), rootFK);
-    const NormSolve ns = lbr_solve<NITER>(x, beta, bmax, bbar);
-    const double rt = sqrt(tau);
-    o.sigma = ns.s / rt;
-    o.vega = D * rootFK * ns.vfin * rt;
+  else if (p.beta < 2.2250738585072014e-308) st = 4;
+  p.status = st;
+  p.qrel = __ddiv_rn(__dsub_rn(hi, lo), lo);
+  p.bbar = __ddiv_rn(__dsub_rn(U, B), rootFK);
+  p.scale = BSM ? D * rootFK : rootFK;
+  return p;
+}
+
+struct RowOut {
+  double sigma, vega;
+  uint8_t status;
+  int8_t zone;
+};
+
+// Full row (Alg.1 l.1-3).  BSM = true: (S,K,tau,r,q,P,flag); false: Black-76 with discount factor 1.
+template <bool BSM, int NITER>
+__device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, double r, double q, double P, double flag) {
+  RowOut o;
+  const Prelude p = lbr_prelude<BSM>(SorF, K, tau, r, q, P, flag);
+  o.sigma = (p.status == 4) ? 0.0 : canonical_nan();
+  o.vega = 0.0;
+  o.zone = -1;
+  o.status = (uint8_t)p.status;
+  if (p.status == 0) {
+    const NormSolve ns = lbr_solve<NITER>(-log1p(p.qrel), p.beta, p.bmax, p.bbar);
+    const double rinv = rsqrt(tau);
+    o.sigma = ns.s * rinv;
+    o.vega = p.scale * ns.vfin * (tau * rinv);
     o.zone = (int8_t)ns.zone;
   }
   return o;

@@ -17,7 +17,6 @@ namespace pivot {
 
 constexpr int kFwdThreads = 128;
 constexpr int kBwdThreads = 256;
-constexpr int kDefaultFwdRows = 1;
 constexpr int kHouseholderSteps = 2;  // north_star: two Householder(3) steps
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -46,29 +45,109 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __re
                               __ldcs(in.flag + i), sigma, vega, status, zone);
 }
 
-// 2 rows per thread, 16-byte loads / stores.  n2 = number of row pairs.
+// ---------------------------------------------------------------------------------------------------------------
+// Forward kernel v4, "tile compaction".  A CTA owns a tile of kTileRows consecutive rows.
+//   Phase A (all rows, coalesced 8-byte loads): prelude -> status.  Rows that need the solver are appended to a
+//            compact queue in shared memory (warp ballot + one shared atomic per warp); the others get their final
+//            sigma / vega straight away.  For queued rows the staged output slots carry tau and D sqrt(FK) meanwhile.
+//   Phase B (queued rows only, DENSE warps): x = -log1p(qrel), the four-stage LBR solve, sigma and vega into the
+//            staged output slots of the row's tile position.
+//   Phase C: the staged sigma, vega and status of the tile are streamed out with coalesced stores.
+// Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); the partition by "needs the solver" costs
+// shared-memory traffic only.  The ncu capture of v3 (profiles/r1a_*) showed 10.45 of 32 lanes active because ~2/3 of
+// config 1/4 rows leave at the validity check; here the solver's warps are full.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kTileThreads = 256;
+constexpr int kTileRowsPerThread = 8;
+constexpr int kTileRows = kTileThreads * kTileRowsPerThread;  // 2048 rows, 104 KB of shared memory, 2 CTAs per SM
+
+struct TileSmem {
+  double sig[kTileRows];    // phase A: tau (queued rows) or final sigma;  phase B: final sigma
+  double veg[kTileRows];    // phase A: D sqrt(FK) (queued rows) or 0;      phase B: final vega
+  double qrel[kTileRows];   // compact queue
+  double beta[kTileRows];
+  double bbar[kTileRows];
+  double bmax[kTileRows];
+  uint16_t pos[kTileRows];  // tile position of the queued row
+  uint8_t status[kTileRows];
+  int count;
+};
+
 template <bool BSM, bool ZONES>
-__global__ void __launch_bounds__(kFwdThreads)
-forward_kernel_vec2(pivot_iv_inputs in, int64_t n2, double* __restrict__ sigma, double* __restrict__ vega,
+__global__ void __launch_bounds__(kTileThreads, 2)
+forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                     uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
-  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= n2) return;
-  const double2 S = __ldcs(reinterpret_cast<const double2*>(in.S_or_F) + j);
-  const double2 K = __ldcs(reinterpret_cast<const double2*>(in.K) + j);
-  const double2 T = __ldcs(reinterpret_cast<const double2*>(in.tau) + j);
-  const double2 P = __ldcs(reinterpret_cast<const double2*>(in.P) + j);
-  const double2 f = __ldcs(reinterpret_cast<const double2*>(in.flag) + j);
-  double2 r = make_double2(0.0, 0.0), q = make_double2(0.0, 0.0);
-  if (BSM) {
-    r = __ldcs(reinterpret_cast<const double2*>(in.r) + j);
-    q = __ldcs(reinterpret_cast<const double2*>(in.q) + j);
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  TileSmem& sm = *reinterpret_cast<TileSmem*>(smem_raw);
+  const int tid = threadIdx.x;
+  const int lane = tid & 31;
+  const int64_t base = (int64_t)blockIdx.x * kTileRows;
+  const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
+  if (tid == 0) sm.count = 0;
+  __syncthreads();
+
+  // ---- phase A
+#pragma unroll 2
+  for (int k = 0; k < kTileRowsPerThread; ++k) {
+    const int p = k * kTileThreads + tid;
+    const bool live = p < rows;
+    bool queued = false;
+    Prelude pr;
+    double tau = 0.0;
+    if (live) {
+      const int64_t i = base + p;
+      const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+      tau = __ldcs(in.tau + i);
+      pr = lbr_prelude<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), tau, r, q, __ldcs(in.P + i), __ldcs(in.flag + i));
+      queued = pr.status == 0;
+      sm.status[p] = (uint8_t)pr.status;
+      sm.sig[p] = queued ? tau : (pr.status == 4 ? 0.0 : canonical_nan());
+      sm.veg[p] = queued ? pr.scale : 0.0;
+      if (ZONES && !queued) zone[i] = -1;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, queued);
+    if (m) {
+      int slot = 0;
+      if (lane == 0) slot = atomicAdd(&sm.count, __popc(m));
+      slot = __shfl_sync(0xffffffffu, slot, 0) + __popc(m & ((1u << lane) - 1u));
+      if (queued) {
+        sm.qrel[slot] = pr.qrel;
+        sm.beta[slot] = pr.beta;
+        sm.bbar[slot] = pr.bbar;
+        sm.bmax[slot] = pr.bmax;
+        sm.pos[slot] = (uint16_t)p;
+      }
+    }
   }
-  const RowOut a = lbr_row<BSM, kHouseholderSteps>(S.x, K.x, T.x, r.x, q.x, P.x, f.x);
-  const RowOut b = lbr_row<BSM, kHouseholderSteps>(S.y, K.y, T.y, r.y, q.y, P.y, f.y);
-  __stcs(reinterpret_cast<double2*>(sigma) + j, make_double2(a.sigma, b.sigma));
-  __stcs(reinterpret_cast<double2*>(vega) + j, make_double2(a.vega, b.vega));
-  reinterpret_cast<uchar2*>(status)[j] = make_uchar2(a.status, b.status);
-  if (ZONES) reinterpret_cast<char2*>(zone)[j] = make_char2(a.zone, b.zone);
+  __syncthreads();
+
+  // ---- phase B
+  const int cnt = sm.count;
+  for (int j = tid; j < cnt; j += kTileThreads) {
+    const int p = sm.pos[j];
+    const NormSolve ns = lbr_solve<kHouseholderSteps>(-log1p(sm.qrel[j]), sm.beta[j], sm.bmax[j], sm.bbar[j]);
+    const double tau = sm.sig[p];
+    const double rinv = rsqrt(tau);
+    sm.sig[p] = ns.s * rinv;
+    sm.veg[p] = sm.veg[p] * ns.vfin * (tau * rinv);
+    if (ZONES) zone[base + p] = (int8_t)ns.zone;
+  }
+  __syncthreads();
+
+  // ---- phase C
+#pragma unroll 4
+  for (int k = 0; k < kTileRowsPerThread; ++k) {
+    const int p = k * kTileThreads + tid;
+    if (p < rows) {
+      __stcs(sigma + base + p, sm.sig[p]);
+      __stcs(vega + base + p, sm.veg[p]);
+    }
+  }
+  if (rows == kTileRows && ((reinterpret_cast<uintptr_t>(status + base) & 15u) == 0)) {
+    if (tid < kTileRows / 16) __stcs(reinterpret_cast<uint4*>(status + base) + tid, reinterpret_cast<const uint4*>(sm.status)[tid]);
+  } else {
+    for (int p = tid; p < rows; p += kTileThreads) status[base + p] = sm.status[p];
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -142,12 +221,12 @@ using namespace pivot;
 
 namespace {
 
-// Tuning knob for the ncu A/B studies: PIVOT_IV_FWD_ROWS=1|2 selects rows per thread
-// (2 = 16-byte double2 loads, 1 = 8-byte loads).  Read once.
-int fwd_rows_per_thread() {
-  static const int v = [] {
-    const char* e = std::getenv("PIVOT_IV_FWD_ROWS");
-    return (e && e[0] == '2') ? 2 : ((e && e[0] == '1') ? 1 : kDefaultFwdRows);
+// Tuning knob for the ncu A/B studies: PIVOT_IV_FWD_KERNEL=rowwise selects the v3 kernel
+// (one row per thread, no compaction); anything else (default) the tile-compaction kernel.  Read once.
+bool fwd_rowwise() {
+  static const bool v = [] {
+    const char* e = std::getenv("PIVOT_IV_FWD_KERNEL");
+    return e && e[0] == 'r';
   }();
   return v;
 }
@@ -155,22 +234,15 @@ int fwd_rows_per_thread() {
 template <bool BSM, bool ZONES>
 int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
                      cudaStream_t st) {
-  const bool vec = aligned16(in.S_or_F) && aligned16(in.K) && aligned16(in.tau) && aligned16(in.P) &&
-                   aligned16(in.flag) && aligned16(sigma) && aligned16(vega) &&
-                   (!BSM || (aligned16(in.r) && aligned16(in.q))) &&
-                   ((reinterpret_cast<uintptr_t>(status) & 1u) == 0) &&
-                   (!ZONES || (reinterpret_cast<uintptr_t>(zone) & 1u) == 0);
-  int64_t done = 0;
-  if (vec && n >= 2 && fwd_rows_per_thread() == 2) {
-    const int64_t n2 = n / 2;
-    const int64_t blocks = (n2 + kFwdThreads - 1) / kFwdThreads;
-    forward_kernel_vec2<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, n2, sigma, vega, status, zone);
-    done = 2 * n2;
-  }
-  if (done < n) {
-    const int64_t rem = n - done;
-    const int64_t blocks = (rem + kFwdThreads - 1) / kFwdThreads;
-    forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, done, n, sigma, vega, status, zone);
+  if (fwd_rowwise()) {
+    const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
+    forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, 0, n, sigma, vega, status, zone);
+  } else {
+    static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES>,
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
+    if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
+    const int64_t blocks = (n + kTileRows - 1) / kTileRows;
+    forward_kernel_tile<BSM, ZONES><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem), st>>>(in, n, sigma, vega, status, zone);
   }
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
@@ -183,7 +255,7 @@ int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* ve
   if (n == 0) return PIVOT_OK;
   if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status || (zones && !zone))
     return PIVOT_ERR_NULL;
-  if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;  // grid.x limit at 2 rows/thread
+  if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;  // grid.x limit
   const bool bsm = in->r != nullptr;
   if (bsm) return zones ? launch_forward_t<true, true>(*in, n, sigma, vega, status, zone, st)
                         : launch_forward_t<true, false>(*in, n, sigma, vega, status, zone, st);
