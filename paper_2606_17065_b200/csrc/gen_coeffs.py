@@ -112,6 +112,43 @@ def fit_ninv_tail(deg):
     return coef, float(rel.max())
 
 
+
+def fit_exp(N):
+    """exp(r) on |r| <= ln2/2 as a degree-N polynomial in r (Chebyshev interpolant, monomial basis)."""
+    half = mp.log(2) / 2
+    a = cheb_to_monomial(cheb_coeffs(lambda y: mp.exp(half * y), N))
+    a = [v / half ** k for k, v in enumerate(a)]
+    worst = 0.0
+    for r in np.linspace(-float(half), float(half), 2001):
+        val = horner([float(v) for v in a], np.float64(r), np.float64)
+        worst = max(worst, abs(float(mp.mpf(float(val)) / mp.exp(mp.mpf(float(r))) - 1)))
+    return a, worst
+
+
+def fit_atanh(N, fmax):
+    """atanh(f) = f (1 + w G(w)), w = f^2 <= fmax^2;  G = degree-N polynomial in w."""
+    wmax = mp.mpf(fmax) ** 2
+
+    def G(y):
+        w = wmax * (1 + y) / 2
+        if w < mp.mpf(10) ** -30:
+            return mp.mpf(1) / 3
+        f = mp.sqrt(w)
+        return (mp.atanh(f) / f - 1) / w
+    a = cheb_to_monomial(cheb_coeffs(G, N))
+    # y = 2 w / wmax - 1  ->  monomial in w
+    out = [mp.mpf(0)] * (N + 1)
+    import math
+    for k, ck in enumerate(a):
+        for j in range(k + 1):
+            out[j] += ck * math.comb(k, j) * (2 / wmax) ** j * (-1) ** (k - j)
+    worst = 0.0
+    for f in np.linspace(1e-6, float(fmax), 1001):
+        w = np.float64(f) ** 2
+        val = np.float64(f) * (1 + w * horner([float(v) for v in out], w, np.float64))
+        worst = max(worst, abs(float(mp.mpf(float(val)) / mp.atanh(mp.mpf(float(f))) - 1)))
+    return out, worst
+
 def fmt(vals, per_line=3, f32=False):
     out = []
     for i in range(0, len(vals), per_line):
@@ -131,12 +168,24 @@ def main():
     print(f"erfcx fp64: C={C64} N={N64} max rel err (fp64 Horner, no FMA) = {e64:.3e}")
     print(f"erfcx fp32: C={C32} N={N32} max rel err (fp32 Horner) = {e32:.3e}")
     print(f"ninv tail : deg 7 in w=1/(1+u), max rel err = {en:.3e}")
+    NEXP, NATH = 11, 8
+    aexp, eexp = fit_exp(NEXP)
+    FMAX = (mp.sqrt(2) - 1) / (mp.sqrt(2) + 1) * mp.mpf("1.02")
+    aath, eath = fit_atanh(NATH, FMAX)
+    print(f"exp       : degree {NEXP} on |r| <= ln2/2, max rel err (fp64 Horner) = {eexp:.3e}")
+    print(f"atanh     : f(1 + w G(w)), G degree {NATH}, |f| <= {float(FMAX):.4f}, max rel err = {eath:.3e}")
     with open(os.path.join(HERE, "coeffs.cuh"), "w") as f:
         f.write("// coeffs.cuh -- GENERATED by gen_coeffs.py (mpmath, 40 digits); do not edit by hand.\n")
         f.write(f"// erfcx fp64: erfcx(z) = (2C/(z+C)) Q((z-C)/(z+C)), C = {C64}, degree {N64}, max rel err {e64:.2e}\n")
         f.write(f"// erfcx fp32: same form, C = {C32}, degree {N32}, max rel err {e32:.2e}\n")
         f.write(f"// ninv tail : -Phi^-1(p) = u - R(1/(1+u)), u = sqrt(-2 ln p), p <= 0.345 (z >= 0.4), degree 7, max rel err {en:.2e}\n")
+        f.write(f"// exp       : degree {NEXP} polynomial on |r| <= ln2/2, max rel err {eexp:.2e}\n")
+        f.write(f"// atanh     : atanh(f) = f (1 + w G(w)), w = f^2, G degree {NATH}, |f| <= {float(FMAX):.4f}, max rel err {eath:.2e}\n")
         f.write("#pragma once\nnamespace pivot {\n")
+        f.write(f"constexpr int kExpN = {NEXP};\n")
+        f.write("__constant__ double kExpP[kExpN + 1] = {\n" + fmt(aexp) + "};\n")
+        f.write(f"constexpr int kAtanhN = {NATH};\n")
+        f.write("__constant__ double kAtanhG[kAtanhN + 1] = {\n" + fmt(aath) + "};\n")
         f.write(f"constexpr double kErfcxC = {C64};\nconstexpr int kErfcxN = {N64};\n")
         f.write("__constant__ double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
         f.write(f"constexpr float kErfcxCf = {C32}f;\nconstexpr int kErfcxNf = {N32};\n")

@@ -21,33 +21,113 @@
 
 namespace pivot {
 
-__device__ constexpr double kInvSqrt2 = 0.70710678118654752440;       // 1/sqrt(2)
-__device__ constexpr double kSqrtPiOver2 = 1.2533141373155002512;      // sqrt(pi/2)
-__device__ constexpr double kSqrt2Pi = 2.5066282746310005024;          // sqrt(2 pi)
-__device__ constexpr double kPhi0 = 0.39894228040143267794;            // 1/sqrt(2 pi)
-__device__ constexpr double kLnPhi0 = -0.91893853320467274178;         // ln(1/sqrt(2 pi))
-__device__ constexpr double kSqrt3 = 1.7320508075688772935;            // sqrt(3)
-__device__ constexpr double kInvSqrt3 = 0.57735026918962576451;        // 1/sqrt(3)
-__device__ constexpr double kTwoPi = 6.2831853071795864769;            // 2 pi
-__device__ constexpr double kTwoPiOver3Sqrt3 = 1.2091995761561452337;  // 2 pi / (3 sqrt 3)
-__device__ constexpr double kPiOver6 = 0.52359877559829887308;         // pi/6
-__device__ constexpr double kLog2e = 1.4426950408889634074;            // 1/ln 2
-__device__ constexpr double kLn2 = 0.69314718055994530942;             // ln 2
-__device__ constexpr double kSmallT = 0.1;                              // series / erfcx switch-over
+// Scalar constants live in constant memory: an fp64 instruction takes a c[bank][offset] operand for free, whereas a
+// 64-bit immediate costs two extra MOV/UMOV issue slots (16.6 % of all issued instructions in the v3 capture,
+// profiles/r1a_forward_v3_ncu_full.md).
+__constant__ double kInvSqrt2 = 0.70710678118654752440;       // 1/sqrt(2)
+__constant__ double kSqrtPiOver2 = 1.2533141373155002512;      // sqrt(pi/2)
+__constant__ double kSqrt2Pi = 2.5066282746310005024;          // sqrt(2 pi)
+__constant__ double kPhi0 = 0.39894228040143267794;            // 1/sqrt(2 pi)
+__constant__ double kLnPhi0 = -0.91893853320467274178;         // ln(1/sqrt(2 pi))
+__constant__ double kSqrt3 = 1.7320508075688772935;            // sqrt(3)
+__constant__ double kInvSqrt3 = 0.57735026918962576451;        // 1/sqrt(3)
+__constant__ double kTwoPi = 6.2831853071795864769;            // 2 pi
+__constant__ double kTwoPiOver3Sqrt3 = 1.2091995761561452337;  // 2 pi / (3 sqrt 3)
+__constant__ double kPiOver6 = 0.52359877559829887308;         // pi/6
+__constant__ double kLog2e = 1.4426950408889634074;            // 1/ln 2
+__constant__ double kLn2 = 0.69314718055994530942;             // ln 2 (nearest double)
+__constant__ double kLn2Lo = 2.3190468138462995584e-17;        // ln 2 - (double)ln 2
+__constant__ double kSmallT = 0.1;                              // series / erfcx switch-over
+__constant__ double kSqrt2m1 = 0.41421356237309504880;         // sqrt(2) - 1
+__constant__ double kEightSqrt3 = 13.856406460551018348;       // 8 sqrt 3
+__constant__ double kSeriesC[5] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0};
 
 enum : int { KIND_LOWER = 0, KIND_LINEAR = 1, KIND_UPPER = 2 };
 
 __device__ __forceinline__ bool is_fin(double v) { return fabs(v) < __longlong_as_double(0x7ff0000000000000LL); }
 __device__ __forceinline__ double canonical_nan() { return __longlong_as_double(0x7ff8000000000000LL); }
 
-// 1/x for x > 0 well inside the fp32 exponent range: MUFU.RCP seed + two Newton steps (error ~1 ulp, no slow path).
-__device__ __forceinline__ double rcp_pos(double x) {
-  float r0f;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r0f) : "f"(__double2float_rn(x)));
-  double r = (double)r0f;
-  r = fma(r, fma(-x, r, 1.0), r);
+// 1/x from MUFU.RCP64H (about 20 bits, full fp64 exponent range, no slow path) plus Newton steps.
+__device__ __forceinline__ double rcp_raw(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  return r;
+}
+__device__ __forceinline__ double rcp_nr1(double x) {  // relative error ~1e-12: seeds only
+  double r = rcp_raw(x);
   r = fma(r, fma(-x, r, 1.0), r);
   return r;
+}
+__device__ __forceinline__ double rcp_nr2(double x) {  // relative error ~1 ulp
+  double r = rcp_nr1(x);
+  r = fma(r, fma(-x, r, 1.0), r);
+  return r;
+}
+__device__ __forceinline__ double rcp_pos(double x) { return rcp_nr2(x); }
+// a/b to ~1 ulp (b normal, finite, non-zero)
+__device__ __forceinline__ double div_fast(double a, double b) {
+  const double r = rcp_nr2(b);
+  const double q = a * r;
+  return fma(fma(-b, q, a), r, q);
+}
+
+// exp(a), |a| < ~745; error ~1 ulp.  n = rint(a log2 e) through the 1.5*2^52 shift, Cody-Waite reduction by fma,
+// degree-11 polynomial (coeffs.cuh), exponent add.
+__device__ __forceinline__ double exp_fast(double a) {
+  const double sh = 6755399441055744.0;
+  const double tt = fma(a, kLog2e, sh);
+  const int n = __double2loint(tt);
+  const double nf = tt - sh;
+  double r = fma(nf, -kLn2, a);
+  r = fma(nf, -kLn2Lo, r);
+  double p = kExpP[kExpN];
+#pragma unroll
+  for (int k = kExpN - 1; k >= 0; --k) p = fma(p, r, kExpP[k]);
+  if ((unsigned)(n + 1020) > 2040u) {  // result leaves the normal range: two-step scaling / saturation
+    if (n > 1020)
+      return (n > 1024) ? __longlong_as_double(0x7ff0000000000000LL)
+                        : p * 0x1p512 * __hiloint2double((n - 512 + 1023) << 20, 0);
+    if (n < -1080) return 0.0;
+    return p * __hiloint2double((n + 128 + 1023) << 20, 0) * 0x1p-128;
+  }
+  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+}
+
+// ef ln2 + 2 atanh(num/den), |num/den| <= 0.175
+__device__ __forceinline__ double log_core(double num, double den, double ef) {
+  const double r = rcp_nr2(den);
+  const double f0 = num * r;
+  const double f = fma(fma(-den, f0, num), r, f0);
+  const double w = f * f;
+  double G = kAtanhG[kAtanhN];
+#pragma unroll
+  for (int k = kAtanhN - 1; k >= 0; --k) G = fma(G, w, kAtanhG[k]);
+  const double two_f = f + f;
+  const double tail = fma(ef, kLn2Lo, two_f * w * G);
+  return fma(ef, kLn2, two_f) + tail;
+}
+
+// ln(v), v positive and normal; error ~1 ulp
+__device__ __forceinline__ double log_fast(double v) {
+  int hi = __double2hiint(v);
+  int e = (hi >> 20) - 1023;
+  hi = (hi & 0x000fffff) | 0x3ff00000;
+  if (hi > 0x3ff6a09e) { hi -= 0x00100000; e += 1; }  // m in (sqrt2/2, sqrt2]
+  const double m = __hiloint2double(hi, __double2loint(v));
+  const double num = m - 1.0;
+  return log_core(num, num + 2.0, (double)e);
+}
+
+// ln(1 + q), q >= 0 finite; relative error ~1 ulp also for tiny q
+__device__ __forceinline__ double log1p_fast(double q) {
+  const double u = 1.0 + q;
+  int hi = __double2hiint(u);
+  int e = (hi >> 20) - 1023;
+  hi = (hi & 0x000fffff) | 0x3ff00000;
+  if (hi > 0x3ff6a09e) { hi -= 0x00100000; e += 1; }
+  const double m = __hiloint2double(hi, __double2loint(u));
+  const double num = (q < kSqrt2m1) ? q : m - 1.0;  // q < sqrt2 - 1  =>  e == 0 and q itself is the exact numerator
+  return log_core(num, num + 2.0, (double)e);
 }
 
 // erfcx(z1), erfcx(z2) for z1, z2 >= 0:  erfcx(z) = (2C/(z+C)) Q((z-C)/(z+C)), one shared reciprocal.
@@ -188,11 +268,11 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
         const double w10 = fma(h, w9, 9.0 * w8);
         const double w11 = fma(h, w10, 10.0 * w9);
         const double t2 = t * t;
-        double acc = w11 * (1.0 / 39916800.0);
-        acc = fma(acc, t2, w9 * (1.0 / 362880.0));
-        acc = fma(acc, t2, w7 * (1.0 / 5040.0));
-        acc = fma(acc, t2, w5 * (1.0 / 120.0));
-        acc = fma(acc, t2, w3 * (1.0 / 6.0));
+        double acc = w11 * kSeriesC[4];
+        acc = fma(acc, t2, w9 * kSeriesC[3]);
+        acc = fma(acc, t2, w7 * kSeriesC[2]);
+        acc = fma(acc, t2, w5 * kSeriesC[1]);
+        acc = fma(acc, t2, w3 * kSeriesC[0]);
         acc = fma(acc, t2, w1);
         Wd = s * acc;  // 2 t acc
       } else if (!neg) {
@@ -207,7 +287,7 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
     const bool want_W = (stage < 2) || (kind != KIND_UPPER);
     const bool need_exp = fin || (stage == 1) || (stage >= 2 && (kind == KIND_LINEAR || want_W != have_W));
     double ex = 0.0;
-    if (need_exp) ex = exp(fin ? -E : E);
+    if (need_exp) ex = exp_fast(fin ? -E : E);
     if (fin) {
       vfin = kPhi0 * ex;
       break;
@@ -252,7 +332,7 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
           yr = kTwoPiOver3Sqrt3 * a * Phz * Phz * Phz;
           dr = kTwoPi * z * z * Yp * Yp * B;
           dd = kPiOver6 * (z * z / (sn2 * sn)) * Yp *
-               fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, 8.0 * kSqrt3 * sn * a) * (B * B) / (A * A * A);
+               fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, kEightSqrt3 * sn * a) * (B * B) / (A * A * A);
           side = 1;
         } else {
           zone = 1;  // s(beta) on [b_l, b_c], s'' = 0 at b_c
@@ -302,7 +382,7 @@ __device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bma
       need_log = true;
     }
     double lg = 0.0;
-    if (need_log) lg = log(larg);
+    if (need_log) lg = log_fast(larg);
     if (stage == 1) {
       ln_target = lg;
       continue;
@@ -407,7 +487,7 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
   o.zone = -1;
   o.status = (uint8_t)p.status;
   if (p.status == 0) {
-    const NormSolve ns = lbr_solve<NITER>(-log1p(p.qrel), p.beta, p.bmax, p.bbar);
+    const NormSolve ns = lbr_solve<NITER>(-log1p_fast(p.qrel), p.beta, p.bmax, p.bbar);
     const double rinv = rsqrt(tau);
     o.sigma = ns.s * rinv;
     o.vega = p.scale * ns.vfin * (tau * rinv);

@@ -125,7 +125,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const int cnt = sm.count;
   for (int j = tid; j < cnt; j += kTileThreads) {
     const int p = sm.pos[j];
-    const NormSolve ns = lbr_solve<kHouseholderSteps>(-log1p(sm.qrel[j]), sm.beta[j], sm.bmax[j], sm.bbar[j]);
+    const NormSolve ns = lbr_solve<kHouseholderSteps>(-log1p_fast(sm.qrel[j]), sm.beta[j], sm.bmax[j], sm.bbar[j]);
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
     sm.sig[p] = ns.s * rinv;
