@@ -8,10 +8,10 @@
 //   z1 >= 0:  W    = c [erfcx(z1) - erfcx(z2)]                       Wbar = b_max/b' - W
 //   z1 <  0:  Wbar = c [erfcx(-z1) + erfcx(z2)]                      W    = b_max/b' - Wbar
 //   t < 0.1:  W    = 2 sum_j w^(2j+1)(h) t^(2j+1)/(2j+1)!,  w(z) = Phi(z)/phi(z) = c erfcx(-z/sqrt2)   (no cancellation)
-// The kernel is organised for a SMALL INSTRUCTION FOOTPRINT (the first version was 213 KB of SASS and stalled on
-// instruction fetch): one non-unrolled loop of four "evaluate W at s" stages (boundary point, zone node, two
-// Householder(3) steps) shares a single copy of the erfcx pair, of exp and of log; the zone seeds, which need only
-// ~1e-5 relative accuracy, use fp32-grade exp / log / erfcx / Phi^-1 built on MUFU.  See DESIGN.md section 5.
+// The solve is split in two passes so that the kernel can regroup rows in shared memory between them (pivot_iv.cu):
+// lbr_seed (boundary point, zone, rational seed; seed-grade arithmetic) and lbr_refine (Householder(3) steps at full
+// precision).  exp / log / log1p / erfcx / reciprocals are this file's own, with coefficients in constant memory
+// (gen_coeffs.py): no slow paths, no 64-bit immediates.  See DESIGN.md section 5.
 // This file shares nothing with oracle/ (the CPU checker).
 #pragma once
 #include <cstdint>
@@ -191,235 +191,281 @@ __device__ __forceinline__ double ninv_tail_seed(double lnp) {
   return (double)(u - R);
 }
 
+// erfcx(z), z >= 0 (single evaluation, same polynomial as erfcx_pair)
+__device__ __forceinline__ double erfcx_one(double z) {
+  const double r = rcp_nr2(z + kErfcxC);
+  const double y = fma(-2.0 * kErfcxC, r, 1.0);
+  double q = kErfcxQ[kErfcxN];
+#pragma unroll
+  for (int k = kErfcxN - 1; k >= 0; --k) q = fma(q, y, kErfcxQ[k]);
+  return (2.0 * kErfcxC) * r * q;
+}
+
+// sqrt(v), v >= 0, relative error ~1e-12 (MUFU.RSQ64H + one Newton step); seeds only
+__device__ __forceinline__ double sqrt_nr1(double v) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(v));
+  y = y * fma(-0.5 * v, y * y, 1.5);
+  return (v > 0.0) ? v * y : 0.0;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// W-evaluation shared by the node stage and the Householder stages: at the point s returns
+//   have_W = true : Wd = W = b/b'            (z1 >= 0, or the small-t series)
+//   have_W = false: Wd = Wbar = (b_max-b)/b' (z1 < 0)
+// together with h = x/s, 1/s and E = (h^2+t^2)/2.
+// ---------------------------------------------------------------------------------------------------------------
+struct WEval {
+  double Wd, E, h, rs;
+  bool have_W;
+};
+
+__device__ __forceinline__ WEval eval_W(double x, double s) {
+  WEval w;
+  w.rs = rcp_nr2(s);
+  w.h = x * w.rs;  // <= 0
+  const double t = 0.5 * s;
+  const double ah = -w.h;
+  w.E = 0.5 * fma(w.h, w.h, t * t);
+  const bool small = t < kSmallT;
+  const double z1 = (ah - t) * kInvSqrt2;
+  const bool neg = z1 < 0.0;
+  double e1, e2;
+  erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
+  w.have_W = small || !neg;
+  if (small) {
+    const double h = w.h;
+    const double w0 = kSqrtPiOver2 * e1;
+    const double w1 = fma(h, w0, 1.0);
+    const double w2 = fma(h, w1, w0);
+    const double w3 = fma(h, w2, 2.0 * w1);
+    const double w4 = fma(h, w3, 3.0 * w2);
+    const double w5 = fma(h, w4, 4.0 * w3);
+    const double w6 = fma(h, w5, 5.0 * w4);
+    const double w7 = fma(h, w6, 6.0 * w5);
+    const double w8 = fma(h, w7, 7.0 * w6);
+    const double w9 = fma(h, w8, 8.0 * w7);
+    const double w10 = fma(h, w9, 9.0 * w8);
+    const double w11 = fma(h, w10, 10.0 * w9);
+    const double t2 = t * t;
+    double acc = w11 * kSeriesC[4];
+    acc = fma(acc, t2, w9 * kSeriesC[3]);
+    acc = fma(acc, t2, w7 * kSeriesC[2]);
+    acc = fma(acc, t2, w5 * kSeriesC[1]);
+    acc = fma(acc, t2, w3 * kSeriesC[0]);
+    acc = fma(acc, t2, w1);
+    w.Wd = s * acc;  // 2 t acc
+  } else {
+    w.Wd = kSqrtPiOver2 * (neg ? e1 + e2 : e1 - e2);
+  }
+  return w;
+}
+
 // Rational cubic on [0,1] (Delbourgo-Gregory form), H = interval width, u and omu = 1-u both supplied.
+// Seed-grade arithmetic: reciprocals carry ~1e-12.
 __device__ __forceinline__ double rc_eval(double u, double omu, double H, double yl, double yr, double dl, double dr,
                                           double r) {
   if (!(r < 1e300)) return fma(yr, u, yl * omu);
   const double c2 = fma(r, yr, -H * dr), c1 = fma(r, yl, H * dl);
   const double num = fma(u * u, fma(yr, u, c2 * omu), omu * omu * fma(c1, u, yl * omu));
-  return num / fma(r - 3.0, u * omu, 1.0);
+  return num * rcp_nr1(fma(r - 3.0, u * omu, 1.0));
 }
 
 // control parameter: fit the second derivative `dd` at the left (side = 0) or right (side = 1) end, floored by the
-// monotonicity / convexity bounds
-__device__ __forceinline__ double rc_control(int side, double H, double yl, double yr, double dl, double dr, double dd) {
-  const double Delta = (yr - yl) / H;
-  const double den = side ? (dr - Delta) : (Delta - dl);
+// monotonicity / convexity bounds.  rH = 1/H.
+__device__ __forceinline__ double rc_control(int side, double H, double rH, double yl, double yr, double dl, double dr,
+                                             double dd) {
+  const double Delta = (yr - yl) * rH;
+  const double dR = dr - Delta, dL = Delta - dl;
+  const double rR = rcp_nr1(dR), rL = rcp_nr1(dL), rD = rcp_nr1(Delta);
   const double span = dr - dl;
-  double r = fma(0.5 * H, dd, span) / den;
+  const double den = side ? dR : dL;
+  double r = fma(0.5 * H, dd, span) * (side ? rR : rL);
   double rmin = -1.0 + 1e-9;
-  if (Delta != 0.0) rmin = fmax(rmin, (dl + dr) / Delta);
-  if (dr != Delta) rmin = fmax(rmin, fabs(span / (dr - Delta)));
-  if (Delta != dl) rmin = fmax(rmin, fabs(span / (Delta - dl)));
+  if (Delta != 0.0) rmin = fmax(rmin, (dl + dr) * rD);
+  if (dR != 0.0) rmin = fmax(rmin, fabs(span * rR));
+  if (dL != 0.0) rmin = fmax(rmin, fabs(span * rL));
   if (den == 0.0) r = __longlong_as_double(0x7ff0000000000000LL);
   return (r > rmin) ? r : rmin;
 }
 
-struct NormSolve {
-  double s;     // total volatility after NITER Householder steps
-  double vfin;  // b'(x, s) = phi0 exp(-(h^2+t^2)/2) at that s (for vega)
-  int zone;
+// ---------------------------------------------------------------------------------------------------------------
+// Pass 1 of the solve (A.5 stage 4): boundary point, zone, rational seed.
+// In:  qrel = (hi-lo)/lo, beta, bbar = b_max - beta (formed without cancellation), bmax.
+// Out: x = -ln(1+qrel) <= 0, the seed s0, the objective kind and its two parameters
+//        KIND_LOWER : p1 = ln beta,          p2 = b_max      g = 1/ln b - 1/ln beta
+//        KIND_LINEAR: p1 = beta,             p2 = bbar       g = b - beta
+//        KIND_UPPER : p1 = ln(b_max - beta), p2 = b_max      g = ln((b_max - beta)/(b_max - b))
+// Everything here only has to deliver a seed good to ~1e-3 (Householder(3) is fourth order), so reciprocals and
+// square roots carry ~1e-12 and the tail maps use fp32-grade exp / log / erfcx / Phi^-1 on MUFU.
+// ---------------------------------------------------------------------------------------------------------------
+struct Seed {
+  double x, s, p1, p2;
+  int kind, zone;
 };
 
-// Solve b(x,s) = beta, x <= 0, 0 < beta < bmax; bbar = bmax - beta supplied exactly.
-// Stage 0: boundary point s_c.  Stage 1: zone node (s_l or s_u) and the rational seed.  Stages 2..1+NITER:
-// Householder(3).  Stage 2+NITER: b' at the final s.  One copy of the erfcx pair, of exp and of log serves all stages.
-template <int NITER>
-__device__ __forceinline__ NormSolve lbr_solve(double x, double beta, double bmax, double bbar) {
-  constexpr int kLast = 2 + NITER;
+__device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, double bmax) {
+  Seed o;
+  const double x = -log1p_fast(qrel);
   const double a = -x;
-  const double sc = sqrt(2.0 * a);
-  const double vc = kPhi0 * bmax;  // b'(x, s_c) = phi0 e^{-|x|/2}
-  double Wc = 0.0, bc = 0.0, sl = 0.0, su = kSqrt2Pi;
-  double s = (a == 0.0) ? su : sc;  // evaluation point of the current stage, then the iterate (x = 0: no stage 0)
-  bool lower = false;
-  int zone = 2, kind = KIND_LINEAR;
-  double ln_target = 0.0;  // ln beta (lower tail) or ln(b_max - beta) (upper tail)
-  double vfin = 0.0;
+  o.x = x;
+  const double sc = sqrt_nr1(2.0 * a);        // inflection point of b(x, .)
+  const double vc = kPhi0 * bmax;             // b'(x, s_c) = phi0 e^{-|x|/2}
+  const double rvc = kSqrt2Pi * rcp_nr1(bmax);
+  // at s_c: |h| = t, so z1 = 0, z2 = sqrt(|x|):  W_c = c (1 - erfcx(sqrt|x|))
+  const double Wc = (a > 0.0) ? kSqrtPiOver2 * (1.0 - erfcx_one(sc * kInvSqrt2)) : 0.0;
+  const double bc = vc * Wc;
+  const double sl = sc - Wc;                  // tangent at the inflection point hits 0 ...
+  const double su = sc + (kSqrt2Pi - Wc);     // ... and b_max
+  const bool lower = beta < bc;
+  int zone;
+  double s;
+  if (lower && !(sl > 0.0)) {  // rounding guard, |x| below ~1e-30: linear seed
+    s = sc * beta * rcp_nr1(bc);
+    zone = 1;
+  } else {
+    const double sn = lower ? sl : su;
+    const WEval w = eval_W(x, sn);
+    const double vn = kPhi0 * exp_fast(-w.E);  // b'(s_n)
+    const double inv_vn = rcp_nr1(vn);
+    const double bn = w.have_W ? w.Wd * vn : fma(-w.Wd, vn, bmax);
+    double xl, xr, yl, yr, dl, dr, dd;
+    int side;
+    if (lower) {
+      if (beta < bn) {
+        zone = 0;  // f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l]
+        const double z = -w.h * kInvSqrt3;
+        const double Y = kSqrtPiOver2 * (double)erfcx_seed(__double2float_rn(z * kInvSqrt2));  // Phi(-z)/phi(z)
+        const double Yp = Y * kPhi0;
+        const double A = exp_seed(-0.5 * z * z), B = exp_seed(0.125 * sn * sn);
+        const double Phz = Yp * A;
+        const double sn2 = sn * sn;
+        const double rA = rcp_nr1(A);
+        xl = 0.0; xr = bn; yl = 0.0; dl = 1.0;
+        yr = kTwoPiOver3Sqrt3 * a * Phz * Phz * Phz;
+        dr = kTwoPi * z * z * Yp * Yp * B;
+        dd = kPiOver6 * (z * z * w.rs * w.rs * w.rs) * Yp *
+             fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, kEightSqrt3 * sn * a) * (B * B) * (rA * rA * rA);
+        side = 1;
+      } else {
+        zone = 1;  // s(beta) on [b_l, b_c], s'' = 0 at b_c
+        xl = bn; xr = bc; yl = sl; yr = sc; dl = inv_vn; dr = rvc; dd = 0.0; side = 1;
+      }
+    } else {
+      if (beta <= bn) {
+        zone = 2;  // s(beta) on [b_c, b_u], s'' = 0 at b_c
+        xl = bc; xr = bn; yl = sc; yr = su; dl = rvc; dr = inv_vn; dd = 0.0; side = 0;
+      } else {
+        zone = 3;  // f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max]
+        const double hu2 = w.h * w.h;
+        const double tn = 0.5 * sn;
+        const double A = exp_seed(0.5 * hu2), B = exp_seed(0.125 * sn * sn);
+        xl = bn; xr = bmax;
+        yl = 0.5 * (double)erfcx_seed(__double2float_rn(tn * kInvSqrt2)) * rcp_nr1(B);  // Phi(-t)
+        yr = 0.0;
+        dl = -0.5 * A; dr = -0.5;
+        dd = kSqrtPiOver2 * (A * A) * B * hu2 * w.rs;
+        side = 0;
+      }
+    }
+    const double H = xr - xl;
+    const double rH = rcp_nr1(H);
+    const double r = rc_control(side, H, rH, yl, yr, dl, dr, dd);
+    const double u = (beta - xl) * rH;
+    const double omu = ((zone == 3) ? bbar : (xr - beta)) * rH;
+    double y = rc_eval(u, omu, H, yl, yr, dl, dr, r);
+    if (zone == 0) {
+      if (!(y > 0.0)) y = fma(yr, u, xr * omu) * u;
+      // Phi(-z) = (f/c)^{1/3}  ->  ln p = ln(f/c)/3
+      const double lnp = fmin(log_seed(y * rcp_nr1(kTwoPiOver3Sqrt3 * a)) * (1.0 / 3.0), -1.0651);
+      s = a * kInvSqrt3 * rcp_nr1(ninv_tail_seed(lnp));
+    } else if (zone == 3) {
+      if (!(y > 0.0)) y = fma(yl, omu, 0.5 * H * u) * omu;
+      s = 2.0 * ninv_tail_seed(fmin(log_seed(y), -1.0651));
+    } else {
+      s = y;
+    }
+    if (!(s > 0.0) || !is_fin(s)) s = sn;
+  }
+  o.s = s;
+  o.zone = zone;
+  if (zone == 0) {
+    o.kind = KIND_LOWER; o.p1 = log_fast(beta); o.p2 = bmax;
+  } else if (zone == 3 && beta > 0.5 * bmax) {
+    o.kind = KIND_UPPER; o.p1 = log_fast(bbar); o.p2 = bmax;
+  } else {
+    o.kind = KIND_LINEAR; o.p1 = beta; o.p2 = bbar;
+  }
+  return o;
+}
 
+// ---------------------------------------------------------------------------------------------------------------
+// Pass 2 of the solve (A.5 stage 5): NITER Householder(3) steps on the zone's objective, then
+// b'(x, s) = phi0 exp(-E) at the final s for the vega (eq.(14)).
+//   ds = nu (1 + h2 nu / 2) / (1 + nu (h2 + h3 nu / 6)),  nu = -g/g', h2 = g''/g', h3 = g'''/g',  ds >= -s/2.
+// Each step needs W or Wbar (one erfcx pair or the small-t series) and ONE of exp / log:
+//   LINEAR: 1/b' = sqrt(2 pi) e^E;   LOWER: ln W;   UPPER: ln Wbar
+// (plus the exp when the available ratio is not the one the objective wants).
+// ---------------------------------------------------------------------------------------------------------------
+struct NormSolve {
+  double s;     // total volatility after NITER Householder steps
+  double vfin;  // b'(x, s) at that s
+};
+
+template <int NITER>
+__device__ __forceinline__ NormSolve lbr_refine(double x, double s, double p1, double p2, int kind) {
 #pragma unroll 1
-  for (int stage = (a == 0.0) ? 1 : 0; stage <= kLast; ++stage) {
-    // ---------------- common part: W (or Wbar) and E at the point s ----------------
-    const bool fin = stage == kLast;
-    const double rs = 1.0 / s;
-    const double h = (a == 0.0) ? 0.0 : x * rs;   // <= 0
-    const double t = 0.5 * s;
-    const double ah = -h;
-    const double E = 0.5 * fma(h, h, t * t);
-    const bool small = t < kSmallT;
-    const double z1 = (stage == 0) ? 0.0 : (ah - t) * kInvSqrt2;   // at s_c, |h| = t exactly (rounding must not flip it)
-    const bool neg = z1 < 0.0;
-    double Wd = 0.0;        // z1 >= 0 or small: W;  z1 < 0: Wbar
-    bool have_W = true;     // Wd holds W (true) or Wbar (false)
-    if (!fin) {
-      double e1, e2;
-      erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
-      if (small) {
-        const double w0 = kSqrtPiOver2 * e1;
-        const double w1 = fma(h, w0, 1.0);
-        const double w2 = fma(h, w1, w0);
-        const double w3 = fma(h, w2, 2.0 * w1);
-        const double w4 = fma(h, w3, 3.0 * w2);
-        const double w5 = fma(h, w4, 4.0 * w3);
-        const double w6 = fma(h, w5, 5.0 * w4);
-        const double w7 = fma(h, w6, 6.0 * w5);
-        const double w8 = fma(h, w7, 7.0 * w6);
-        const double w9 = fma(h, w8, 8.0 * w7);
-        const double w10 = fma(h, w9, 9.0 * w8);
-        const double w11 = fma(h, w10, 10.0 * w9);
-        const double t2 = t * t;
-        double acc = w11 * kSeriesC[4];
-        acc = fma(acc, t2, w9 * kSeriesC[3]);
-        acc = fma(acc, t2, w7 * kSeriesC[2]);
-        acc = fma(acc, t2, w5 * kSeriesC[1]);
-        acc = fma(acc, t2, w3 * kSeriesC[0]);
-        acc = fma(acc, t2, w1);
-        Wd = s * acc;  // 2 t acc
-      } else if (!neg) {
-        Wd = kSqrtPiOver2 * (e1 - e2);
-      } else {
-        Wd = kSqrtPiOver2 * (e1 + e2);
-        have_W = false;
-      }
-    }
-    // the one exp: 1/b' = sqrt(2 pi) e^{E} (node stage, b - beta objective, or when the available ratio is not the
-    // one the objective wants), or b' itself at the final s
-    const bool want_W = (stage < 2) || (kind != KIND_UPPER);
-    const bool need_exp = fin || (stage == 1) || (stage >= 2 && (kind == KIND_LINEAR || want_W != have_W));
-    double ex = 0.0;
-    if (need_exp) ex = exp_fast(fin ? -E : E);
-    if (fin) {
-      vfin = kPhi0 * ex;
-      break;
-    }
-    const double inv_v = kSqrt2Pi * ex;
-
-    if (stage == 0) {
-      // ---------------- boundary: tangent at the inflection point hits 0 at s_l and b_max at s_u ----------------
-      Wc = Wd;  // z1 = 0 here, so this is W
-      bc = vc * Wc;
-      sl = sc - Wc;
-      su = sc + (kSqrt2Pi - Wc);
-      lower = beta < bc;
-      if (lower && !(sl > 0.0)) {  // rounding guard, |x| below ~1e-30: skip the node, linear seed
-        s = sc * (beta / bc);
-        zone = 1; kind = KIND_LINEAR;
-        stage = 1;
-        continue;
-      }
-      s = lower ? sl : su;
-      continue;
-    }
-    double larg = 1.0;      // argument of the one log
-    bool need_log = false;
-    if (stage == 1) {
-      // ---------------- node (s_l or s_u) and the zone's rational seed ----------------
-      const double sn = s, hn = h, tn = t;
-      const double inv_vn = inv_v;                                             // 1/b'(s_n)
-      const double bn = have_W ? Wd / inv_vn : bmax - Wd / inv_vn;             // b(s_n)
-      double xl, xr, yl, yr, dl, dr, dd;
-      int side;
-      if (lower) {
-        if (beta < bn) {
-          zone = 0;  // f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l]
-          const double z = ah * kInvSqrt3;
-          const double Y = kSqrtPiOver2 * (double)erfcx_seed(__double2float_rn(z * kInvSqrt2));  // Phi(-z)/phi(z)
-          const double Yp = Y * kPhi0;
-          const double A = exp_seed(-0.5 * z * z), B = exp_seed(0.125 * sn * sn);
-          const double Phz = Yp * A;
-          const double sn2 = sn * sn;
-          xl = 0.0; xr = bn; yl = 0.0; dl = 1.0;
-          yr = kTwoPiOver3Sqrt3 * a * Phz * Phz * Phz;
-          dr = kTwoPi * z * z * Yp * Yp * B;
-          dd = kPiOver6 * (z * z / (sn2 * sn)) * Yp *
-               fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, kEightSqrt3 * sn * a) * (B * B) / (A * A * A);
-          side = 1;
-        } else {
-          zone = 1;  // s(beta) on [b_l, b_c], s'' = 0 at b_c
-          xl = bn; xr = bc; yl = sl; yr = sc; dl = inv_vn; dr = 1.0 / vc; dd = 0.0; side = 1;
-        }
-      } else {
-        if (beta <= bn) {
-          zone = 2;  // s(beta) on [b_c, b_u], s'' = 0 at b_c
-          xl = bc; xr = bn; yl = sc; yr = su; dl = 1.0 / vc; dr = inv_vn; dd = 0.0; side = 0;
-        } else {
-          zone = 3;  // f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max]
-          const double hu2 = hn * hn;
-          const double A = exp_seed(0.5 * hu2), B = exp_seed(0.125 * sn * sn);
-          xl = bn; xr = bmax;
-          yl = 0.5 * (double)erfcx_seed(__double2float_rn(tn * kInvSqrt2)) / B;  // Phi(-t) = erfcx(t/sqrt2) e^{-t^2/2}/2, B = e^{t^2/2}
-          yr = 0.0;
-          dl = -0.5 * A; dr = -0.5;
-          dd = kSqrtPiOver2 * (A * A) * B * hu2 / sn;
-          side = 0;
-        }
-      }
-      const double H = xr - xl;
-      const double r = rc_control(side, H, yl, yr, dl, dr, dd);
-      const double u = (beta - xl) / H;
-      const double omu = (zone == 3) ? bbar / H : (xr - beta) / H;
-      double y = rc_eval(u, omu, H, yl, yr, dl, dr, r);
-      if (zone == 0) {
-        if (!(y > 0.0)) y = fma(yr, u, xr * omu) * u;
-        // Phi(-z) = (f/c)^{1/3}  ->  ln p = ln(f/c)/3
-        const double lnp = fmin(log_seed(y / (kTwoPiOver3Sqrt3 * a)) * (1.0 / 3.0), -1.0651);
-        s = a * kInvSqrt3 / ninv_tail_seed(lnp);
-      } else if (zone == 3) {
-        if (!(y > 0.0)) y = fma(yl, omu, 0.5 * H * u) * omu;
-        s = 2.0 * ninv_tail_seed(fmin(log_seed(y), -1.0651));
-      } else {
-        s = y;
-      }
-      if (!(s > 0.0) || !is_fin(s)) s = sn;
-      kind = (zone == 0) ? KIND_LOWER : ((zone == 3 && beta > 0.5 * bmax) ? KIND_UPPER : KIND_LINEAR);
-      if (kind != KIND_LINEAR) {
-        larg = (kind == KIND_LOWER) ? beta : bbar;
-        need_log = true;
-      }
-    } else if (kind != KIND_LINEAR) {
-      // the ratio this objective wants: W (lower tail) or Wbar (upper tail)
-      larg = (want_W == have_W) ? Wd : fma(bmax, inv_v, -Wd);
-      need_log = true;
-    }
-    double lg = 0.0;
-    if (need_log) lg = log_fast(larg);
-    if (stage == 1) {
-      ln_target = lg;
-      continue;
-    }
-    // ---------------- Householder(3) step on the zone's objective ----------------
-    const double hr = h * rs;
-    const double B2 = fma(h, hr, -0.25 * s);                    // b2 = b''/b'
-    const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // b3 = third derivative of b over b'
+  for (int it = 0; it < NITER; ++it) {
+    const WEval w = eval_W(x, s);
+    const double hr = w.h * w.rs;
+    const double B2 = fma(w.h, hr, -0.25 * s);                  // b''/b'
+    const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // b'''/b'
     double nu, h2, h3;
     if (kind == KIND_LINEAR) {
-      // g = b - beta:  nu = (beta - b)/b'
-      nu = have_W ? fma(beta, inv_v, -Wd) : fma(-bbar, inv_v, Wd);
+      // g = b - beta:  nu = (beta - b)/b'  (p1 = beta, p2 = bbar)
+      const double inv_v = kSqrt2Pi * exp_fast(w.E);
+      nu = w.have_W ? fma(p1, inv_v, -w.Wd) : fma(-p2, inv_v, w.Wd);
       h2 = B2;
       h3 = B3;
-    } else if (kind == KIND_LOWER) {
-      // g = 1/ln b - 1/ln beta,  ln b = ln phi0 - E + ln W
-      const double W = larg;
-      const double L = kLnPhi0 - E + lg;
-      const double rLW = 1.0 / (L * W);
-      const double lam = rLW * W, ub = rLW * L;  // 1/L, b'/b = 1/W
-      const double k2 = fma(2.0, lam, 1.0);
-      nu = (ln_target - L) * (L / ln_target) * W;
-      h2 = fma(-ub, k2, B2);
-      h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
     } else {
-      // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar
-      const double Wb = larg;
-      const double gp = 1.0 / Wb;
-      nu = (kLnPhi0 - E + lg - ln_target) * Wb;
-      h2 = B2 + gp;
-      h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
+      const bool want_W = kind == KIND_LOWER;
+      double R = w.Wd;  // the ratio the objective wants: W (lower tail) or Wbar (upper tail); p2 = b_max
+      if (want_W != w.have_W) R = fma(p2 * kSqrt2Pi, exp_fast(w.E), -w.Wd);
+      const double L = kLnPhi0 - w.E + log_fast(R);  // ln b (lower) or ln(b_max - b) (upper)
+      if (want_W) {
+        // g = 1/ln b - 1/ln beta  (p1 = ln beta)
+        const double rLW = rcp_nr2(L * R);
+        const double lam = rLW * R, ub = rLW * L;  // 1/L, b'/b = 1/W
+        const double k2 = fma(2.0, lam, 1.0);
+        nu = (p1 - L) * (L * rcp_nr2(p1)) * R;
+        h2 = fma(-ub, k2, B2);
+        h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
+      } else {
+        // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar  (p1 = ln(b_max - beta))
+        const double gp = rcp_nr2(R);
+        nu = (L - p1) * R;
+        h2 = B2 + gp;
+        h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
+      }
     }
-    double ds = nu * fma(0.5 * h2, nu, 1.0) / fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0);
+    double ds = nu * fma(0.5 * h2, nu, 1.0) * rcp_nr2(fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0));
     if (!(ds > -0.5 * s)) ds = -0.5 * s;
     s += ds;
   }
-  return NormSolve{s, vfin, zone};
+  const double rs = rcp_nr2(s);
+  const double h = x * rs, t = 0.5 * s;
+  NormSolve o;
+  o.s = s;
+  o.vfin = kPhi0 * exp_fast(-0.5 * fma(h, h, t * t));
+  return o;
+}
+
+// one-call form (row-per-thread kernel): seed + refine
+template <int NITER>
+__device__ __forceinline__ NormSolve lbr_solve(double qrel, double beta, double bmax, double bbar, int& zone) {
+  const Seed sd = lbr_seed(qrel, beta, bbar, bmax);
+  zone = sd.zone;
+  return lbr_refine<NITER>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
 }
 
 // Row prelude (Alg.1 l.1 and l.3; A.5 stages 1-2): normalisation, validity, reduction to an OTM call.
@@ -487,11 +533,12 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
   o.zone = -1;
   o.status = (uint8_t)p.status;
   if (p.status == 0) {
-    const NormSolve ns = lbr_solve<NITER>(-log1p_fast(p.qrel), p.beta, p.bmax, p.bbar);
+    int zone;
+    const NormSolve ns = lbr_solve<NITER>(p.qrel, p.beta, p.bmax, p.bbar, zone);
     const double rinv = rsqrt(tau);
     o.sigma = ns.s * rinv;
     o.vega = p.scale * ns.vfin * (tau * rinv);
-    o.zone = (int8_t)ns.zone;
+    o.zone = (int8_t)zone;
   }
   return o;
 }

@@ -58,23 +58,26 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __re
 // config 1/4 rows leave at the validity check; here the solver's warps are full.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
-constexpr int kTileRowsPerThread = 8;
+constexpr int kTileRowsPerThread = 4;
 constexpr int kTileRows = kTileThreads * kTileRowsPerThread;  // 2048 rows, 104 KB of shared memory, 2 CTAs per SM
 
 struct TileSmem {
-  double sig[kTileRows];    // phase A: tau (queued rows) or final sigma;  phase B: final sigma
-  double veg[kTileRows];    // phase A: D sqrt(FK) (queued rows) or 0;      phase B: final vega
-  double qrel[kTileRows];   // compact queue
-  double beta[kTileRows];
-  double bbar[kTileRows];
-  double bmax[kTileRows];
-  uint16_t pos[kTileRows];  // tile position of the queued row
+  double sig[kTileRows];      // phase A: tau (queued rows) or final sigma;  phase B2: final sigma
+  double veg[kTileRows];      // phase A: D sqrt(FK) (queued rows) or 0;      phase B2: final vega
+  double q0[kTileRows];       // compact queue.  after A: qrel, beta, bbar, bmax;  after B1: x, s0, p1, p2 (lbr_seed)
+  double q1[kTileRows];
+  double q2[kTileRows];
+  double q3[kTileRows];
+  uint16_t pos[kTileRows];    // tile position of the queued row
+  uint16_t perm[kTileRows];   // queue indices grouped by objective: LOWER from the front, LINEAR from the back
+  uint16_t permU[kTileRows];  // ... and UPPER
   uint8_t status[kTileRows];
-  int count;
+  int count;                  // queued rows
+  int nkind[3];               // rows per objective kind
 };
 
 template <bool BSM, bool ZONES>
-__global__ void __launch_bounds__(kTileThreads, 2)
+__global__ void __launch_bounds__(kTileThreads, 3)
 forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                     uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -83,7 +86,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const int lane = tid & 31;
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
   const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
-  if (tid == 0) sm.count = 0;
+  if (tid < 4) (&sm.count)[tid] = 0;  // count, nkind[0..2]
   __syncthreads();
 
   // ---- phase A
@@ -111,26 +114,60 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       if (lane == 0) slot = atomicAdd(&sm.count, __popc(m));
       slot = __shfl_sync(0xffffffffu, slot, 0) + __popc(m & ((1u << lane) - 1u));
       if (queued) {
-        sm.qrel[slot] = pr.qrel;
-        sm.beta[slot] = pr.beta;
-        sm.bbar[slot] = pr.bbar;
-        sm.bmax[slot] = pr.bmax;
+        sm.q0[slot] = pr.qrel;
+        sm.q1[slot] = pr.beta;
+        sm.q2[slot] = pr.bbar;
+        sm.q3[slot] = pr.bmax;
         sm.pos[slot] = (uint16_t)p;
       }
     }
   }
   __syncthreads();
 
-  // ---- phase B
+  // ---- phase B1: boundary point, zone, seed; rows regrouped by objective kind
   const int cnt = sm.count;
-  for (int j = tid; j < cnt; j += kTileThreads) {
+  for (int j0 = 0; j0 < cnt; j0 += kTileThreads) {   // j0 is CTA-uniform: every lane reaches the ballots
+    const int j = j0 + tid;
+    const bool act = j < cnt;
+    int kind = -1;
+    if (act) {
+      const Seed sd = lbr_seed(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+      sm.q0[j] = sd.x; sm.q1[j] = sd.s; sm.q2[j] = sd.p1; sm.q3[j] = sd.p2;
+      kind = sd.kind;
+      if (ZONES) zone[base + sm.pos[j]] = (int8_t)sd.zone;
+    }
+    const unsigned mL = __ballot_sync(0xffffffffu, kind == KIND_LOWER);
+    const unsigned mN = __ballot_sync(0xffffffffu, kind == KIND_LINEAR);
+    const unsigned mU = __ballot_sync(0xffffffffu, kind == KIND_UPPER);
+    int bL = 0, bN = 0, bU = 0;
+    if (lane == 0) {
+      if (mL) bL = atomicAdd(&sm.nkind[KIND_LOWER], __popc(mL));
+      if (mN) bN = atomicAdd(&sm.nkind[KIND_LINEAR], __popc(mN));
+      if (mU) bU = atomicAdd(&sm.nkind[KIND_UPPER], __popc(mU));
+    }
+    bL = __shfl_sync(0xffffffffu, bL, 0);
+    bN = __shfl_sync(0xffffffffu, bN, 0);
+    bU = __shfl_sync(0xffffffffu, bU, 0);
+    const unsigned lt = (1u << lane) - 1u;
+    if (kind == KIND_LOWER) sm.perm[bL + __popc(mL & lt)] = (uint16_t)j;
+    else if (kind == KIND_LINEAR) sm.perm[kTileRows - 1 - (bN + __popc(mN & lt))] = (uint16_t)j;
+    else if (kind == KIND_UPPER) sm.permU[bU + __popc(mU & lt)] = (uint16_t)j;
+  }
+  __syncthreads();
+
+  // ---- phase B2: Householder steps; a warp sees one objective kind (except at the two group boundaries)
+  const int nL = sm.nkind[KIND_LOWER], nN = sm.nkind[KIND_LINEAR];
+  for (int k = tid; k < cnt; k += kTileThreads) {
+    int j, kind;
+    if (k < nL) { j = sm.perm[k]; kind = KIND_LOWER; }
+    else if (k < nL + nN) { j = sm.perm[kTileRows - 1 - (k - nL)]; kind = KIND_LINEAR; }
+    else { j = sm.permU[k - nL - nN]; kind = KIND_UPPER; }
+    const NormSolve ns = lbr_refine<kHouseholderSteps>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], kind);
     const int p = sm.pos[j];
-    const NormSolve ns = lbr_solve<kHouseholderSteps>(-log1p_fast(sm.qrel[j]), sm.beta[j], sm.bmax[j], sm.bbar[j]);
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
     sm.sig[p] = ns.s * rinv;
     sm.veg[p] = sm.veg[p] * ns.vfin * (tau * rinv);
-    if (ZONES) zone[base + p] = (int8_t)ns.zone;
   }
   __syncthreads();
 
