@@ -468,16 +468,20 @@ __device__ __forceinline__ NormSolve lbr_solve(double qrel, double beta, double 
   return lbr_refine<NITER>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
 }
 
-// Row prelude (Alg.1 l.1 and l.3; A.5 stages 1-2): normalisation, validity, reduction to an OTM call.
+// Row prelude (Alg.1 l.1 and l.3; A.5 stages 1-2): validity and status for EVERY row, with no division:
+//   beta = RN(tv / rootFK) < DBL_MIN   <=>   tv * 2^1022 < rootFK     (exact: the scaling is exact, and for doubles
+//   bmax = RN(lo / rootFK) >= 2^-500   <=>   lo * 2^500 >= rootFK      a < b implies a <= b - ulp(b) < b (1 - 2^-53))
+// so the status byte equals the one obtained from the correctly rounded quotients, bit for bit, and rows that leave
+// here (64.6 % of config 1/4) cost no division (a zero numerator would even take the divide's slow path).
 // The status decision uses only correctly rounded IEEE operations issued through intrinsics, so it cannot be
 // contracted into FMAs and is bit-reproducible against any IEEE-754 implementation of the same sequence.
 struct Prelude {
-  double qrel;    // (hi - lo)/lo, hi = max(F,K), lo = min(F,K):  x = -log1p(qrel)
-  double beta;    // time value / sqrt(FK)
-  double bbar;    // (U - B)/sqrt(FK) = b_max - beta, formed without cancellation
-  double bmax;    // lo / sqrt(FK) = e^{x/2}
+  double F;       // forward (BSM: S e^{(r-q) tau})
+  double B;       // undiscounted price (BSM: P / D)
+  double rootFK;  // sqrt(F K)
   double scale;   // D sqrt(FK): vega = scale * b'(x,s) * sqrt(tau)
   int status;
+  bool call;
 };
 
 template <bool BSM>
@@ -497,24 +501,44 @@ __device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau
     }
   }
   const double rootFK = __dsqrt_rn(__dmul_rn(F, K));
-  const double lo = fmin(F, K), hi = fmax(F, K);
-  p.bmax = __ddiv_rn(lo, rootFK);
-  if (!(is_fin(rootFK) && rootFK > 0.0) || !(p.bmax >= 0x1p-500)) bad = true;
+  const double lo = fmin(F, K);
+  if (!(is_fin(rootFK) && rootFK > 0.0) || !(__dmul_rn(lo, 0x1p500) >= rootFK)) bad = true;
   const bool call = flag > 0.0;
   const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
   const double U = call ? F : K;
   const double tv = __dsub_rn(B, iota);
-  p.beta = __ddiv_rn(tv, rootFK);
   int st = 0;
   if (bad) st = 3;
   else if (B < iota) st = 1;
   else if (B >= U) st = 2;
-  else if (p.beta < 2.2250738585072014e-308) st = 4;
+  else if (__dmul_rn(tv, 0x1p1022) < rootFK) st = 4;
   p.status = st;
-  p.qrel = __ddiv_rn(__dsub_rn(hi, lo), lo);
-  p.bbar = __ddiv_rn(__dsub_rn(U, B), rootFK);
+  p.F = F;
+  p.B = B;
+  p.rootFK = rootFK;
   p.scale = BSM ? D * rootFK : rootFK;
+  p.call = call;
   return p;
+}
+
+// Normalised solver inputs of a row that reached the solver (A.5 stage 2); correctly rounded quotients.
+struct Norm {
+  double qrel;    // (hi - lo)/lo, hi = max(F,K), lo = min(F,K):  x = -log1p(qrel)
+  double beta;    // time value / sqrt(FK)
+  double bbar;    // (U - B)/sqrt(FK) = b_max - beta, formed without cancellation
+  double bmax;    // lo / sqrt(FK) = e^{x/2}
+};
+
+__device__ __forceinline__ Norm lbr_normalise(double F, double K, double B, double rootFK, bool call) {
+  Norm n;
+  const double lo = fmin(F, K), hi = fmax(F, K);
+  const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
+  const double U = call ? F : K;
+  n.bmax = __ddiv_rn(lo, rootFK);
+  n.beta = __ddiv_rn(__dsub_rn(B, iota), rootFK);
+  n.qrel = __ddiv_rn(__dsub_rn(hi, lo), lo);
+  n.bbar = __ddiv_rn(__dsub_rn(U, B), rootFK);
+  return n;
 }
 
 struct RowOut {
@@ -534,7 +558,8 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
   o.status = (uint8_t)p.status;
   if (p.status == 0) {
     int zone;
-    const NormSolve ns = lbr_solve<NITER>(p.qrel, p.beta, p.bmax, p.bbar, zone);
+    const Norm nm = lbr_normalise(p.F, K, p.B, p.rootFK, p.call);
+    const NormSolve ns = lbr_solve<NITER>(nm.qrel, nm.beta, nm.bmax, nm.bbar, zone);
     const double rinv = rsqrt(tau);
     o.sigma = ns.s * rinv;
     o.vega = p.scale * ns.vfin * (tau * rinv);

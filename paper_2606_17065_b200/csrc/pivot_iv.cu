@@ -64,11 +64,11 @@ constexpr int kTileRows = kTileThreads * kTileRowsPerThread;  // 2048 rows, 104 
 struct TileSmem {
   double sig[kTileRows];      // phase A: tau (queued rows) or final sigma;  phase B2: final sigma
   double veg[kTileRows];      // phase A: D sqrt(FK) (queued rows) or 0;      phase B2: final vega
-  double q0[kTileRows];       // compact queue.  after A: qrel, beta, bbar, bmax;  after B1: x, s0, p1, p2 (lbr_seed)
+  double q0[kTileRows];       // compact queue.  after A: F, K, B, sqrt(FK);  after B1: x, s0, p1, p2 (lbr_seed)
   double q1[kTileRows];
   double q2[kTileRows];
   double q3[kTileRows];
-  uint16_t pos[kTileRows];    // tile position of the queued row
+  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call
   uint16_t perm[kTileRows];   // queue indices grouped by objective: LOWER from the front, LINEAR from the back
   uint16_t permU[kTileRows];  // ... and UPPER
   uint8_t status[kTileRows];
@@ -96,12 +96,13 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     const bool live = p < rows;
     bool queued = false;
     Prelude pr;
-    double tau = 0.0;
+    double tau = 0.0, Kk = 0.0;
     if (live) {
       const int64_t i = base + p;
       const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
       tau = __ldcs(in.tau + i);
-      pr = lbr_prelude<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), tau, r, q, __ldcs(in.P + i), __ldcs(in.flag + i));
+      Kk = __ldcs(in.K + i);
+      pr = lbr_prelude<BSM>(__ldcs(in.S_or_F + i), Kk, tau, r, q, __ldcs(in.P + i), __ldcs(in.flag + i));
       queued = pr.status == 0;
       sm.status[p] = (uint8_t)pr.status;
       sm.sig[p] = queued ? tau : (pr.status == 4 ? 0.0 : canonical_nan());
@@ -114,11 +115,11 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       if (lane == 0) slot = atomicAdd(&sm.count, __popc(m));
       slot = __shfl_sync(0xffffffffu, slot, 0) + __popc(m & ((1u << lane) - 1u));
       if (queued) {
-        sm.q0[slot] = pr.qrel;
-        sm.q1[slot] = pr.beta;
-        sm.q2[slot] = pr.bbar;
-        sm.q3[slot] = pr.bmax;
-        sm.pos[slot] = (uint16_t)p;
+        sm.q0[slot] = pr.F;
+        sm.q1[slot] = Kk;
+        sm.q2[slot] = pr.B;
+        sm.q3[slot] = pr.rootFK;
+        sm.pos[slot] = (uint16_t)(p | (pr.call ? 0x8000 : 0));
       }
     }
   }
@@ -131,10 +132,11 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     const bool act = j < cnt;
     int kind = -1;
     if (act) {
-      const Seed sd = lbr_seed(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+      const Norm nm = lbr_normalise(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], (sm.pos[j] & 0x8000) != 0);
+      const Seed sd = lbr_seed(nm.qrel, nm.beta, nm.bbar, nm.bmax);
       sm.q0[j] = sd.x; sm.q1[j] = sd.s; sm.q2[j] = sd.p1; sm.q3[j] = sd.p2;
       kind = sd.kind;
-      if (ZONES) zone[base + sm.pos[j]] = (int8_t)sd.zone;
+      if (ZONES) zone[base + (sm.pos[j] & 0x7fff)] = (int8_t)sd.zone;
     }
     const unsigned mL = __ballot_sync(0xffffffffu, kind == KIND_LOWER);
     const unsigned mN = __ballot_sync(0xffffffffu, kind == KIND_LINEAR);
@@ -163,7 +165,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     else if (k < nL + nN) { j = sm.perm[kTileRows - 1 - (k - nL)]; kind = KIND_LINEAR; }
     else { j = sm.permU[k - nL - nN]; kind = KIND_UPPER; }
     const NormSolve ns = lbr_refine<kHouseholderSteps>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], kind);
-    const int p = sm.pos[j];
+    const int p = sm.pos[j] & 0x7fff;
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
     sm.sig[p] = ns.s * rinv;
