@@ -45,6 +45,8 @@ __constant__ double kSeriesC[5] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 3
 enum : int { KIND_LOWER = 0, KIND_LINEAR = 1, KIND_UPPER = 2 };
 
 __device__ __forceinline__ bool is_fin(double v) { return fabs(v) < __longlong_as_double(0x7ff0000000000000LL); }
+// 0 < v < inf (false for NaN): two fp64 compares
+__device__ __forceinline__ bool pos_fin(double v) { return v > 0.0 && v < __longlong_as_double(0x7ff0000000000000LL); }
 __device__ __forceinline__ double canonical_nan() { return __longlong_as_double(0x7ff8000000000000LL); }
 
 // 1/x from MUFU.RCP64H (about 20 bits, full fp64 exponent range, no slow path) plus Newton steps.
@@ -488,8 +490,7 @@ template <bool BSM>
 __device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau, double r, double q, double P,
                                                double flag) {
   Prelude p;
-  bool bad = !(is_fin(SorF) && SorF > 0.0) || !(is_fin(K) && K > 0.0) || !(is_fin(tau) && tau > 0.0) || !is_fin(P) ||
-             !(flag == 1.0 || flag == -1.0);
+  bool bad = !pos_fin(SorF) || !pos_fin(K) || !pos_fin(tau) || !is_fin(P) || !(flag == 1.0 || flag == -1.0);
   double F = SorF, D = 1.0, B = P;
   if (BSM) {
     if (!is_fin(r) || !is_fin(q)) bad = true;
@@ -497,12 +498,12 @@ __device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau
       F = __dmul_rn(SorF, exp(__dmul_rn(__dsub_rn(r, q), tau)));
       D = exp(__dmul_rn(-r, tau));
       B = __ddiv_rn(P, D);
-      if (!(is_fin(F) && F > 0.0) || !(is_fin(D) && D > 0.0) || !is_fin(B)) bad = true;
+      if (!pos_fin(F) || !pos_fin(D) || !is_fin(B)) bad = true;
     }
   }
   const double rootFK = __dsqrt_rn(__dmul_rn(F, K));
   const double lo = fmin(F, K);
-  if (!(is_fin(rootFK) && rootFK > 0.0) || !(__dmul_rn(lo, 0x1p500) >= rootFK)) bad = true;
+  if (!pos_fin(rootFK) || !(__dmul_rn(lo, 0x1p500) >= rootFK)) bad = true;
   const bool call = flag > 0.0;
   const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
   const double U = call ? F : K;
@@ -521,7 +522,9 @@ __device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau
   return p;
 }
 
-// Normalised solver inputs of a row that reached the solver (A.5 stage 2); correctly rounded quotients.
+// Normalised solver inputs of a row that reached the solver (A.5 stage 2).  Quotients by Newton
+// reciprocal + one residual correction (~1 ulp, no slow path): sqrt(FK) lies in [2^-537, 2^512] and b_max in
+// [2^-500, 1], so the MUFU reciprocal seeds never leave the normal range; lo itself is never inverted.
 struct Norm {
   double qrel;    // (hi - lo)/lo, hi = max(F,K), lo = min(F,K):  x = -log1p(qrel)
   double beta;    // time value / sqrt(FK)
@@ -534,10 +537,17 @@ __device__ __forceinline__ Norm lbr_normalise(double F, double K, double B, doub
   const double lo = fmin(F, K), hi = fmax(F, K);
   const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
   const double U = call ? F : K;
-  n.bmax = __ddiv_rn(lo, rootFK);
-  n.beta = __ddiv_rn(__dsub_rn(B, iota), rootFK);
-  n.qrel = __ddiv_rn(__dsub_rn(hi, lo), lo);
-  n.bbar = __ddiv_rn(__dsub_rn(U, B), rootFK);
+  const double tv = __dsub_rn(B, iota), ub = __dsub_rn(U, B), d = __dsub_rn(hi, lo);
+  const double r = rcp_nr2(rootFK);
+  double q = lo * r;
+  n.bmax = fma(fma(-rootFK, q, lo), r, q);
+  q = tv * r;
+  n.beta = fma(fma(-rootFK, q, tv), r, q);
+  q = ub * r;
+  n.bbar = fma(fma(-rootFK, q, ub), r, q);
+  const double rl = r * rcp_nr2(n.bmax);  // ~ 1/lo, formed without inverting lo
+  q = d * rl;
+  n.qrel = fma(fma(-lo, q, d), rl, q);
   return n;
 }
 

@@ -89,37 +89,66 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   if (tid < 4) (&sm.count)[tid] = 0;  // count, nkind[0..2]
   __syncthreads();
 
-  // ---- phase A
-#pragma unroll 2
+  // ---- phase A: all rows of the tile; every load of the thread's rows is issued before the first use
+  const double* __restrict__ gF = in.S_or_F + base;
+  const double* __restrict__ gK = in.K + base;
+  const double* __restrict__ gT = in.tau + base;
+  const double* __restrict__ gP = in.P + base;
+  const double* __restrict__ gf = in.flag + base;
+  const double* __restrict__ gr = BSM ? in.r + base : nullptr;
+  const double* __restrict__ gq = BSM ? in.q + base : nullptr;
+  double vF[kTileRowsPerThread], vK[kTileRowsPerThread], vT[kTileRowsPerThread], vP[kTileRowsPerThread],
+      vf[kTileRowsPerThread], vr[kTileRowsPerThread], vq[kTileRowsPerThread];
+#pragma unroll
   for (int k = 0; k < kTileRowsPerThread; ++k) {
     const int p = k * kTileThreads + tid;
     const bool live = p < rows;
-    bool queued = false;
-    Prelude pr;
-    double tau = 0.0, Kk = 0.0;
-    if (live) {
-      const int64_t i = base + p;
-      const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
-      tau = __ldcs(in.tau + i);
-      Kk = __ldcs(in.K + i);
-      pr = lbr_prelude<BSM>(__ldcs(in.S_or_F + i), Kk, tau, r, q, __ldcs(in.P + i), __ldcs(in.flag + i));
-      queued = pr.status == 0;
+    // dead rows read as flag = 0 -> BAD_INPUT, never stored
+    vF[k] = live ? __ldcs(gF + p) : 0.0;
+    vK[k] = live ? __ldcs(gK + p) : 0.0;
+    vT[k] = live ? __ldcs(gT + p) : 0.0;
+    vP[k] = live ? __ldcs(gP + p) : 0.0;
+    vf[k] = live ? __ldcs(gf + p) : 0.0;
+    vr[k] = (BSM && live) ? __ldcs(gr + p) : 0.0;
+    vq[k] = (BSM && live) ? __ldcs(gq + p) : 0.0;
+  }
+  unsigned qmask = 0, cmask = 0;  // bit k: row k of this thread is queued / is a call
+#pragma unroll
+  for (int k = 0; k < kTileRowsPerThread; ++k) {
+    const int p = k * kTileThreads + tid;
+    const Prelude pr = lbr_prelude<BSM>(vF[k], vK[k], vT[k], vr[k], vq[k], vP[k], vf[k]);
+    const bool queued = pr.status == 0;
+    if (p < rows) {
       sm.status[p] = (uint8_t)pr.status;
-      sm.sig[p] = queued ? tau : (pr.status == 4 ? 0.0 : canonical_nan());
+      sm.sig[p] = queued ? vT[k] : (pr.status == 4 ? 0.0 : canonical_nan());
       sm.veg[p] = queued ? pr.scale : 0.0;
-      if (ZONES && !queued) zone[i] = -1;
+      if (ZONES && !queued) zone[base + p] = -1;
     }
-    const unsigned m = __ballot_sync(0xffffffffu, queued);
-    if (m) {
-      int slot = 0;
-      if (lane == 0) slot = atomicAdd(&sm.count, __popc(m));
-      slot = __shfl_sync(0xffffffffu, slot, 0) + __popc(m & ((1u << lane) - 1u));
-      if (queued) {
-        sm.q0[slot] = pr.F;
-        sm.q1[slot] = Kk;
-        sm.q2[slot] = pr.B;
-        sm.q3[slot] = pr.rootFK;
-        sm.pos[slot] = (uint16_t)(p | (pr.call ? 0x8000 : 0));
+    qmask |= queued ? (1u << k) : 0u;
+    cmask |= pr.call ? (1u << k) : 0u;
+    vF[k] = pr.F; vP[k] = pr.B; vT[k] = pr.rootFK;  // what the solver pass needs: F, K, B, sqrt(FK)
+  }
+  {
+    // one warp scan and one shared atomic per warp for the whole tile
+    const int c = __popc(qmask);
+    int incl = c;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int v = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl += v;
+    }
+    int wbase = 0;
+    if (lane == 31 && incl > 0) wbase = atomicAdd(&sm.count, incl);
+    int slot = __shfl_sync(0xffffffffu, wbase, 31) + incl - c;
+#pragma unroll
+    for (int k = 0; k < kTileRowsPerThread; ++k) {
+      if (qmask & (1u << k)) {
+        sm.q0[slot] = vF[k];
+        sm.q1[slot] = vK[k];
+        sm.q2[slot] = vP[k];
+        sm.q3[slot] = vT[k];
+        sm.pos[slot] = (uint16_t)((k * kTileThreads + tid) | ((cmask >> k) & 1u ? 0x8000 : 0));
+        ++slot;
       }
     }
   }
