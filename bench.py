@@ -37,6 +37,9 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # algorithmic bytes per row: forward Black-76 5x8 in + 8+8+1 out; backward 8+8+1 in + 8 out
 FWD_BYTES_PER_ROW = 57
 BWD_BYTES_PER_ROW = 25
+# DRAM traffic per row of the forward kernel measured by ncu (profiles/r1b_forward_tile_ncu_full.md): reads are exactly
+# the 40 algorithmic bytes; part of the 17 written bytes is still dirty in L2 when the kernel ends
+FWD_TRAFFIC_BYTES_PER_ROW = 56.5
 # per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
 # CUDA 12.9 builtins); "/" and sqrt count 1 flop each
 CALL_FLOPS = {"exp": 31, "log": 47, "log1p": 109, "erfc": 113, "erfcx": 165, "ninv": 315, "cbrt": 16}
@@ -149,7 +152,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--rows", type=int, default=1 << 26, help="rows per GPU")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
@@ -281,12 +284,28 @@ def main():
         tot = float(sum(mix))
         flops_all = sum(f * k for f, k in zip(FALLBACK_FLOPS_PER_CLASS, mix)) / tot
 
+    # --- fp64-pipe probe (8 independent DFMA chains per thread, full occupancy), timed live with CUDA events
+    probe_tflops = None
+    try:
+        pv.pivot_iv_probe_dfma(2000, stream=stream)
+        p0 = torch.cuda.Event(enable_timing=True); p1 = torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        nfma = pv.pivot_iv_probe_dfma(40000, stream=stream)
+        p1.record(stream); torch.cuda.synchronize()
+        probe_tflops = 2.0 * nfma / (p0.elapsed_time(p1) * 1e-3) / 1e12
+    except Exception:
+        pass
+
     peaks, peak_src = _peaks()
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     fwd_tflops = flops_all * n / (fwd_ms * 1e-3) / 1e12
-    roofline = {"kernel": "forward_kernel_vec2<false,false>", "bound": "alu", "achieved": fwd_tflops,
-                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": fwd_tflops / FP64_PEAK_TFLOPS, "traffic": None,
-                "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md s7); DFMA probe measures ~35.7",
+    roofline = {"kernel": "forward_kernel_tile<false,false>", "bound": "alu", "achieved": fwd_tflops,
+                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": fwd_tflops / FP64_PEAK_TFLOPS,
+                "traffic": FWD_TRAFFIC_BYTES_PER_ROW * n,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per row of one ncu --set full capture "
+                                  "(profiles/), scaled to this launch's rows",
+                "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md s7)",
+                "dfma_probe_tflops": probe_tflops,
                 "flops_per_row": flops_all, "flops_per_row_excl_transcendental_internals": flops_plain,
                 "avg_launch_ms": fwd_ms,
                 "hbm": {"achieved": FWD_BYTES_PER_ROW * n / (fwd_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
