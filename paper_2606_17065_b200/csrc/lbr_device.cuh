@@ -292,112 +292,135 @@ __device__ __forceinline__ double rc_control(int side, double H, double rH, doub
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Pass 1 of the solve (A.5 stage 4): boundary point, zone, rational seed.
-// In:  qrel = (hi-lo)/lo, beta, bbar = b_max - beta (formed without cancellation), bmax.
-// Out: x = -ln(1+qrel) <= 0, the seed s0, the objective kind and its two parameters
+// Pass 1 of the solve (A.5 stage 4): boundary point, zone, rational seed.  Split in two so that the
+// kernel can regroup rows by zone in between:
+//   lbr_seed_head : x, boundary point s_c, node (s_l or s_u), zone.  The two middle zones (1, 2: s(beta) interpolated
+//                   between the node and the inflection point) are finished here; the tails only hand over their node.
+//   lbr_seed_tail0 / lbr_seed_tail3 : the lower / upper tail maps f_low, f_up, their rational-cubic interpolant in beta
+//                   and its inversion.
+// Result of the pass: x = -ln(1+qrel) <= 0, the seed s0, the objective kind and its two parameters
 //        KIND_LOWER : p1 = ln beta,          p2 = b_max      g = 1/ln b - 1/ln beta
 //        KIND_LINEAR: p1 = beta,             p2 = bbar       g = b - beta
 //        KIND_UPPER : p1 = ln(b_max - beta), p2 = b_max      g = ln((b_max - beta)/(b_max - b))
 // Everything here only has to deliver a seed good to ~1e-3 (Householder(3) is fourth order), so reciprocals and
 // square roots carry ~1e-12 and the tail maps use fp32-grade exp / log / erfcx / Phi^-1 on MUFU.
 // ---------------------------------------------------------------------------------------------------------------
-struct Seed {
-  double x, s, p1, p2;
-  int kind, zone;
+struct SeedHead {
+  int zone;        // 0, 3: tail pending (v = x, s_n, b_n, beta, b_max | bbar);  1, 2: finished (v = x, s0, beta, bbar)
+  double v0, v1, v2, v3, v4;
 };
 
-__device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, double bmax) {
-  Seed o;
+__device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, double bbar, double bmax) {
+  SeedHead o;
   const double x = -log1p_fast(qrel);
   const double a = -x;
-  o.x = x;
+  o.v0 = x;
   const double sc = sqrt_nr1(2.0 * a);        // inflection point of b(x, .)
   const double vc = kPhi0 * bmax;             // b'(x, s_c) = phi0 e^{-|x|/2}
-  const double rvc = kSqrt2Pi * rcp_nr1(bmax);
   // at s_c: |h| = t, so z1 = 0, z2 = sqrt(|x|):  W_c = c (1 - erfcx(sqrt|x|))
   const double Wc = (a > 0.0) ? kSqrtPiOver2 * (1.0 - erfcx_one(sc * kInvSqrt2)) : 0.0;
   const double bc = vc * Wc;
   const double sl = sc - Wc;                  // tangent at the inflection point hits 0 ...
   const double su = sc + (kSqrt2Pi - Wc);     // ... and b_max
   const bool lower = beta < bc;
-  int zone;
-  double s;
+  o.v2 = beta; o.v3 = bbar; o.v4 = 0.0;
   if (lower && !(sl > 0.0)) {  // rounding guard, |x| below ~1e-30: linear seed
-    s = sc * beta * rcp_nr1(bc);
-    zone = 1;
-  } else {
-    const double sn = lower ? sl : su;
-    const WEval w = eval_W(x, sn);
-    const double vn = kPhi0 * exp_fast(-w.E);  // b'(s_n)
-    const double inv_vn = rcp_nr1(vn);
-    const double bn = w.have_W ? w.Wd * vn : fma(-w.Wd, vn, bmax);
-    double xl, xr, yl, yr, dl, dr, dd;
-    int side;
-    if (lower) {
-      if (beta < bn) {
-        zone = 0;  // f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l]
-        const double z = -w.h * kInvSqrt3;
-        const double Y = kSqrtPiOver2 * (double)erfcx_seed(__double2float_rn(z * kInvSqrt2));  // Phi(-z)/phi(z)
-        const double Yp = Y * kPhi0;
-        const double A = exp_seed(-0.5 * z * z), B = exp_seed(0.125 * sn * sn);
-        const double Phz = Yp * A;
-        const double sn2 = sn * sn;
-        const double rA = rcp_nr1(A);
-        xl = 0.0; xr = bn; yl = 0.0; dl = 1.0;
-        yr = kTwoPiOver3Sqrt3 * a * Phz * Phz * Phz;
-        dr = kTwoPi * z * z * Yp * Yp * B;
-        dd = kPiOver6 * (z * z * w.rs * w.rs * w.rs) * Yp *
-             fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, kEightSqrt3 * sn * a) * (B * B) * (rA * rA * rA);
-        side = 1;
-      } else {
-        zone = 1;  // s(beta) on [b_l, b_c], s'' = 0 at b_c
-        xl = bn; xr = bc; yl = sl; yr = sc; dl = inv_vn; dr = rvc; dd = 0.0; side = 1;
-      }
-    } else {
-      if (beta <= bn) {
-        zone = 2;  // s(beta) on [b_c, b_u], s'' = 0 at b_c
-        xl = bc; xr = bn; yl = sc; yr = su; dl = rvc; dr = inv_vn; dd = 0.0; side = 0;
-      } else {
-        zone = 3;  // f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max]
-        const double hu2 = w.h * w.h;
-        const double tn = 0.5 * sn;
-        const double A = exp_seed(0.5 * hu2), B = exp_seed(0.125 * sn * sn);
-        xl = bn; xr = bmax;
-        yl = 0.5 * (double)erfcx_seed(__double2float_rn(tn * kInvSqrt2)) * rcp_nr1(B);  // Phi(-t)
-        yr = 0.0;
-        dl = -0.5 * A; dr = -0.5;
-        dd = kSqrtPiOver2 * (A * A) * B * hu2 * w.rs;
-        side = 0;
-      }
-    }
-    const double H = xr - xl;
-    const double rH = rcp_nr1(H);
-    const double r = rc_control(side, H, rH, yl, yr, dl, dr, dd);
-    const double u = (beta - xl) * rH;
-    const double omu = ((zone == 3) ? bbar : (xr - beta)) * rH;
-    double y = rc_eval(u, omu, H, yl, yr, dl, dr, r);
-    if (zone == 0) {
-      if (!(y > 0.0)) y = fma(yr, u, xr * omu) * u;
-      // Phi(-z) = (f/c)^{1/3}  ->  ln p = ln(f/c)/3
-      const double lnp = fmin(log_seed(y * rcp_nr1(kTwoPiOver3Sqrt3 * a)) * (1.0 / 3.0), -1.0651);
-      s = a * kInvSqrt3 * rcp_nr1(ninv_tail_seed(lnp));
-    } else if (zone == 3) {
-      if (!(y > 0.0)) y = fma(yl, omu, 0.5 * H * u) * omu;
-      s = 2.0 * ninv_tail_seed(fmin(log_seed(y), -1.0651));
-    } else {
-      s = y;
-    }
-    if (!(s > 0.0) || !is_fin(s)) s = sn;
+    o.zone = 1;
+    o.v1 = sc * beta * rcp_nr1(bc);
+    return o;
   }
-  o.s = s;
-  o.zone = zone;
-  if (zone == 0) {
-    o.kind = KIND_LOWER; o.p1 = log_fast(beta); o.p2 = bmax;
-  } else if (zone == 3 && beta > 0.5 * bmax) {
+  const double sn = lower ? sl : su;
+  const WEval w = eval_W(x, sn);
+  const double vn = kPhi0 * exp_fast(-w.E);  // b'(s_n)
+  const double bn = w.have_W ? w.Wd * vn : fma(-w.Wd, vn, bmax);
+  if (lower ? (beta < bn) : (beta > bn)) {   // a tail: hand the node over
+    o.zone = lower ? 0 : 3;
+    o.v1 = sn; o.v2 = bn; o.v3 = beta; o.v4 = lower ? bmax : bbar;
+    return o;
+  }
+  // zones 1 and 2: s(beta) between the node and the inflection point, s'' = 0 at the inflection point
+  o.zone = lower ? 1 : 2;
+  const double inv_vn = rcp_nr1(vn), rvc = kSqrt2Pi * rcp_nr1(bmax);
+  const double xl = lower ? bn : bc, xr = lower ? bc : bn;
+  const double yl = lower ? sn : sc, yr = lower ? sc : sn;
+  const double dl = lower ? inv_vn : rvc, dr = lower ? rvc : inv_vn;
+  const double H = xr - xl, rH = rcp_nr1(H);
+  const double r = rc_control(lower ? 1 : 0, H, rH, yl, yr, dl, dr, 0.0);
+  const double s = rc_eval((beta - xl) * rH, (xr - beta) * rH, H, yl, yr, dl, dr, r);
+  o.v1 = (s > 0.0 && is_fin(s)) ? s : sn;
+  return o;
+}
+
+struct Seed {
+  double x, s, p1, p2;
+  int kind, zone;
+};
+
+// zone 0: f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l]
+__device__ __forceinline__ Seed lbr_seed_tail0(double x, double sn, double bn, double beta, double bmax) {
+  const double a = -x;
+  const double rs = rcp_nr1(sn);
+  const double z = a * rs * kInvSqrt3;
+  const double Y = kSqrtPiOver2 * (double)erfcx_seed(__double2float_rn(z * kInvSqrt2));  // Phi(-z)/phi(z)
+  const double Yp = Y * kPhi0;
+  const double A = exp_seed(-0.5 * z * z), B = exp_seed(0.125 * sn * sn);
+  const double Phz = Yp * A;
+  const double sn2 = sn * sn;
+  const double rA = rcp_nr1(A);
+  const double yr = kTwoPiOver3Sqrt3 * a * Phz * Phz * Phz;
+  const double dr = kTwoPi * z * z * Yp * Yp * B;
+  const double dd = kPiOver6 * (z * z * rs * rs * rs) * Yp *
+                    fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, kEightSqrt3 * sn * a) * (B * B) * (rA * rA * rA);
+  const double H = bn, rH = rcp_nr1(bn);
+  const double r = rc_control(1, H, rH, 0.0, yr, 1.0, dr, dd);
+  const double u = beta * rH, omu = (bn - beta) * rH;
+  double y = rc_eval(u, omu, H, 0.0, yr, 1.0, dr, r);
+  if (!(y > 0.0)) y = fma(yr, u, bn * omu) * u;
+  // Phi(-z) = (f/c)^{1/3}  ->  ln p = ln(f/c)/3
+  const double lnp = fmin(log_seed(y * rcp_nr1(kTwoPiOver3Sqrt3 * a)) * (1.0 / 3.0), -1.0651);
+  double s = a * kInvSqrt3 * rcp_nr1(ninv_tail_seed(lnp));
+  if (!(s > 0.0) || !is_fin(s)) s = sn;
+  Seed o;
+  o.x = x; o.s = s; o.zone = 0;
+  o.kind = KIND_LOWER; o.p1 = log_fast(beta); o.p2 = bmax;
+  return o;
+}
+
+// zone 3: f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max]
+__device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bn, double beta, double bbar) {
+  const double bmax = beta + bbar;
+  const double rs = rcp_nr1(sn);
+  const double h = x * rs;
+  const double hu2 = h * h;
+  const double tn = 0.5 * sn;
+  const double A = exp_seed(0.5 * hu2), B = exp_seed(0.125 * sn * sn);
+  const double yl = 0.5 * (double)erfcx_seed(__double2float_rn(tn * kInvSqrt2)) * rcp_nr1(B);  // Phi(-t)
+  const double dl = -0.5 * A;
+  const double dd = kSqrtPiOver2 * (A * A) * B * hu2 * rs;
+  const double H = bmax - bn, rH = rcp_nr1(H);
+  const double r = rc_control(0, H, rH, yl, 0.0, dl, -0.5, dd);
+  const double u = (beta - bn) * rH, omu = bbar * rH;
+  double y = rc_eval(u, omu, H, yl, 0.0, dl, -0.5, r);
+  if (!(y > 0.0)) y = fma(yl, omu, 0.5 * H * u) * omu;
+  double s = 2.0 * ninv_tail_seed(fmin(log_seed(y), -1.0651));
+  if (!(s > 0.0) || !is_fin(s)) s = sn;
+  Seed o;
+  o.x = x; o.s = s; o.zone = 3;
+  if (bbar < 0.5 * bmax) {
     o.kind = KIND_UPPER; o.p1 = log_fast(bbar); o.p2 = bmax;
   } else {
     o.kind = KIND_LINEAR; o.p1 = beta; o.p2 = bbar;
   }
+  return o;
+}
+
+// one-call form (row-per-thread kernel)
+__device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, double bmax) {
+  const SeedHead hd = lbr_seed_head(qrel, beta, bbar, bmax);
+  if (hd.zone == 0) return lbr_seed_tail0(hd.v0, hd.v1, hd.v2, hd.v3, hd.v4);
+  if (hd.zone == 3) return lbr_seed_tail3(hd.v0, hd.v1, hd.v2, hd.v3, hd.v4);
+  Seed o;
+  o.x = hd.v0; o.s = hd.v1; o.p1 = hd.v2; o.p2 = hd.v3; o.kind = KIND_LINEAR; o.zone = hd.zone;
   return o;
 }
 

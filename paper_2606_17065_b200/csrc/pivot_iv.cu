@@ -68,12 +68,13 @@ struct TileSmem {
   double q1[kTileRows];
   double q2[kTileRows];
   double q3[kTileRows];
-  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call
-  uint16_t perm[kTileRows];   // queue indices grouped by objective: LOWER from the front, LINEAR from the back
-  uint16_t permU[kTileRows];  // ... and UPPER
+  double q4[kTileRows];       // fifth word of a pending tail row between B1a and B1b
+  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call, bit 14 = zone 3 row with UPPER objective
+  uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, finished middle-zone rows from the back
+  uint16_t permU[kTileRows];  // ... and zone 3 rows
   uint8_t status[kTileRows];
   int count;                  // queued rows
-  int nkind[3];               // rows per objective kind
+  int nkind[3];               // rows per class: zone 0, zones 1-2, zone 3
 };
 
 template <bool BSM, bool ZONES>
@@ -154,47 +155,64 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   }
   __syncthreads();
 
-  // ---- phase B1: boundary point, zone, seed; rows regrouped by objective kind
+  // ---- phase B1a: x, boundary point, node, zone; middle zones (1, 2) finished; rows regrouped by zone class
+  //      lists: zone 0 (-> LOWER) from the front of perm, finished LINEAR rows from the back, zone 3 in permU
   const int cnt = sm.count;
   for (int j0 = 0; j0 < cnt; j0 += kTileThreads) {   // j0 is CTA-uniform: every lane reaches the ballots
     const int j = j0 + tid;
-    const bool act = j < cnt;
-    int kind = -1;
-    if (act) {
+    int cls = -1;  // 0: zone 0, 1: finished (zones 1, 2), 2: zone 3
+    if (j < cnt) {
       const Norm nm = lbr_normalise(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], (sm.pos[j] & 0x8000) != 0);
-      const Seed sd = lbr_seed(nm.qrel, nm.beta, nm.bbar, nm.bmax);
-      sm.q0[j] = sd.x; sm.q1[j] = sd.s; sm.q2[j] = sd.p1; sm.q3[j] = sd.p2;
-      kind = sd.kind;
-      if (ZONES) zone[base + (sm.pos[j] & 0x7fff)] = (int8_t)sd.zone;
+      const SeedHead hd = lbr_seed_head(nm.qrel, nm.beta, nm.bbar, nm.bmax);
+      sm.q0[j] = hd.v0; sm.q1[j] = hd.v1; sm.q2[j] = hd.v2; sm.q3[j] = hd.v3; sm.q4[j] = hd.v4;
+      cls = (hd.zone == 0) ? 0 : ((hd.zone == 3) ? 2 : 1);
+      if (ZONES) zone[base + (sm.pos[j] & 0x3fff)] = (int8_t)hd.zone;
     }
-    const unsigned mL = __ballot_sync(0xffffffffu, kind == KIND_LOWER);
-    const unsigned mN = __ballot_sync(0xffffffffu, kind == KIND_LINEAR);
-    const unsigned mU = __ballot_sync(0xffffffffu, kind == KIND_UPPER);
-    int bL = 0, bN = 0, bU = 0;
+    const unsigned m0 = __ballot_sync(0xffffffffu, cls == 0);
+    const unsigned m1 = __ballot_sync(0xffffffffu, cls == 1);
+    const unsigned m2 = __ballot_sync(0xffffffffu, cls == 2);
+    int b0 = 0, b1 = 0, b2 = 0;
     if (lane == 0) {
-      if (mL) bL = atomicAdd(&sm.nkind[KIND_LOWER], __popc(mL));
-      if (mN) bN = atomicAdd(&sm.nkind[KIND_LINEAR], __popc(mN));
-      if (mU) bU = atomicAdd(&sm.nkind[KIND_UPPER], __popc(mU));
+      if (m0) b0 = atomicAdd(&sm.nkind[0], __popc(m0));
+      if (m1) b1 = atomicAdd(&sm.nkind[1], __popc(m1));
+      if (m2) b2 = atomicAdd(&sm.nkind[2], __popc(m2));
     }
-    bL = __shfl_sync(0xffffffffu, bL, 0);
-    bN = __shfl_sync(0xffffffffu, bN, 0);
-    bU = __shfl_sync(0xffffffffu, bU, 0);
+    b0 = __shfl_sync(0xffffffffu, b0, 0);
+    b1 = __shfl_sync(0xffffffffu, b1, 0);
+    b2 = __shfl_sync(0xffffffffu, b2, 0);
     const unsigned lt = (1u << lane) - 1u;
-    if (kind == KIND_LOWER) sm.perm[bL + __popc(mL & lt)] = (uint16_t)j;
-    else if (kind == KIND_LINEAR) sm.perm[kTileRows - 1 - (bN + __popc(mN & lt))] = (uint16_t)j;
-    else if (kind == KIND_UPPER) sm.permU[bU + __popc(mU & lt)] = (uint16_t)j;
+    if (cls == 0) sm.perm[b0 + __popc(m0 & lt)] = (uint16_t)j;
+    else if (cls == 1) sm.perm[kTileRows - 1 - (b1 + __popc(m1 & lt))] = (uint16_t)j;
+    else if (cls == 2) sm.permU[b2 + __popc(m2 & lt)] = (uint16_t)j;
   }
   __syncthreads();
 
-  // ---- phase B2: Householder steps; a warp sees one objective kind (except at the two group boundaries)
-  const int nL = sm.nkind[KIND_LOWER], nN = sm.nkind[KIND_LINEAR];
+  // ---- phase B1b: the tail seeds, zone 0 rows then zone 3 rows, dense (one mixed warp at the boundary)
+  const int n0 = sm.nkind[0], n1 = sm.nkind[1], n3 = sm.nkind[2];
+  for (int k = tid; k < n0 + n3; k += kTileThreads) {
+    Seed sd;
+    int j;
+    if (k < n0) {
+      j = sm.perm[k];
+      sd = lbr_seed_tail0(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], sm.q4[j]);
+    } else {
+      j = sm.permU[k - n0];
+      sd = lbr_seed_tail3(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], sm.q4[j]);
+      if (sd.kind == KIND_UPPER) sm.pos[j] |= 0x4000;
+    }
+    sm.q1[j] = sd.s; sm.q2[j] = sd.p1; sm.q3[j] = sd.p2;
+  }
+  __syncthreads();
+
+  // ---- phase B2: Householder steps; zone 0 rows (LOWER), then finished middle rows (LINEAR), then zone 3 rows
+  //      (UPPER or LINEAR by their flag): a warp sees one objective kind except at the group boundaries
   for (int k = tid; k < cnt; k += kTileThreads) {
     int j, kind;
-    if (k < nL) { j = sm.perm[k]; kind = KIND_LOWER; }
-    else if (k < nL + nN) { j = sm.perm[kTileRows - 1 - (k - nL)]; kind = KIND_LINEAR; }
-    else { j = sm.permU[k - nL - nN]; kind = KIND_UPPER; }
+    if (k < n0) { j = sm.perm[k]; kind = KIND_LOWER; }
+    else if (k < n0 + n1) { j = sm.perm[kTileRows - 1 - (k - n0)]; kind = KIND_LINEAR; }
+    else { j = sm.permU[k - n0 - n1]; kind = (sm.pos[j] & 0x4000) ? KIND_UPPER : KIND_LINEAR; }
     const NormSolve ns = lbr_refine<kHouseholderSteps>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], kind);
-    const int p = sm.pos[j] & 0x7fff;
+    const int p = sm.pos[j] & 0x3fff;
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
     sm.sig[p] = ns.s * rinv;
