@@ -222,3 +222,34 @@ def test_streams_and_preallocated_outputs():
     s.synchronize()
     assert np.array_equal(out[0].cpu().numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
     assert torch.equal(out[2], ref[2])
+
+
+def test_degenerate_tile_compositions():
+    """Tiles of the compaction kernel with an empty queue, a single queued row, only upper-tail rows, only near-ATM rows:
+    the shared-memory lists (zone 0 / middle / zone 3) must work when any of them is empty or holds the whole tile."""
+    rng = np.random.default_rng(77)
+    n = 3 * 1024 + 17
+    F = np.full(n, 100.0)
+    T = np.full(n, 0.5)
+    flag = np.ones(n)
+    cases = {}
+    K = F * np.exp(rng.uniform(0.1, 0.5, n))
+    cases["all_below_intrinsic_or_zero"] = (K, np.where(np.arange(n) % 2 == 0, 0.0, -1.0))            # status 4 / 1
+    P = np.zeros(n); P[1500] = 2.5
+    cases["one_queued_row"] = (K, P)
+    cases["upper_tail_only"] = (K, F * (1.0 - 10.0 ** rng.uniform(-12, -2, n)))                        # beta -> b_max
+    K2 = F * (1.0 + rng.uniform(-1e-9, 1e-9, n))
+    cases["near_atm_tiny_prices"] = (K2, 10.0 ** rng.uniform(-250, -1, n))                             # lower tail, |x| ~ 1e-9
+    cases["near_atm_mid_prices"] = (K2, rng.uniform(0.5, 60.0, n))
+    for name, (Kk, Pp) in cases.items():
+        cols = [F, np.ascontiguousarray(Kk), T, np.ascontiguousarray(Pp), flag]
+        o = po.forward(*cols)
+        g = tuple(t.cpu().numpy() for t in pv.pivot_iv_forward(*[torch.from_numpy(x).cuda() for x in cols]))
+        c = dict(zip(KEYS, cols)); c["r"] = None; c["q"] = None
+        st = compare_forward(g, o, c)
+        if name == "all_below_intrinsic_or_zero":
+            assert st["ok"] == 0
+        if name == "one_queued_row":
+            assert st["ok"] == 1
+        if name in ("upper_tail_only", "near_atm_mid_prices"):
+            assert st["ok"] == n, name
