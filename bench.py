@@ -119,6 +119,38 @@ def _flops_per_row_from_counts(counts, rows):
     return tot_plain / n, (tot_plain + tot_calls) / n
 
 
+def run_sweep(pv, wl, hbm_peak, flops_mixed):
+    """Config 4 (BASELINE.json configs[4]): forward IV/s for n = 2^10 .. 2^28, inputs as config 1 ("all") and its
+    rejection-sampled 1-solve variant; per size the median and best of 20 launches timed one by one with CUDA events."""
+    stream = torch.cuda.current_stream()
+    res = []
+    for e in range(10, 29, 2):
+        n = 1 << e
+        row = {"n": n}
+        for name, so in (("all", False), ("solve", True)):
+            cfg = wl.config4(n, seed=40 + e, device="cuda", solve_only=so)
+            a = [cfg[k] for k in KEYS]
+            out = (torch.empty(n, dtype=torch.float64, device="cuda"), torch.empty(n, dtype=torch.float64, device="cuda"),
+                   torch.empty(n, dtype=torch.uint8, device="cuda"))
+            for _ in range(3):
+                pv.pivot_iv_forward(*a, out=out, stream=stream)
+            ts = []
+            for _ in range(20):
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                pv.pivot_iv_forward(*a, out=out, stream=stream)
+                e1.record(stream); e1.synchronize()
+                ts.append(e0.elapsed_time(e1))
+            med, best = float(np.median(ts)), float(np.min(ts))
+            row[name] = {"ms_median": med, "ms_best": best, "iv_per_s": n / (med * 1e-3),
+                         "hbm_frac": FWD_BYTES_PER_ROW * n / (med * 1e-3) / 1e9 / hbm_peak}
+            if not so:
+                row[name]["fp64_frac"] = flops_mixed * n / (med * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+            del cfg, a, out
+        res.append(row)
+    return res
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -158,6 +190,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="config 4: forward-only size sweep n = 2^10 .. 2^28 (all rows and the 1-solve variant); adds a "
+                         "'sweep' list to the JSON line")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -315,6 +350,12 @@ def main():
                     "unit": "GB/s", "frac": bwd_gbs / hbm_peak, "traffic": None, "avg_launch_ms": bwd_ms,
                     "peak_source": peak_src}
 
+    sweep = None
+    if args.sweep and rank == 0 and world == 1:
+        del cfg, a, out, gP, gsig
+        torch.cuda.empty_cache()
+        sweep = run_sweep(pv, wl, hbm_peak, flops_all)
+
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": "rows/s", "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -329,6 +370,8 @@ def main():
                 "clocks": clocks, "e2e": e2e, "gpu_launches": K * (pv.load_library().pivot_iv_launches_per_forward() + pv.load_library().pivot_iv_launches_per_backward()),
                 "roofline": roofline, "roofline_backward": roofline_bwd, "cpu_baseline": cpu}
         line.update(err)
+        if sweep is not None:
+            line["sweep"] = sweep
         line["paper_context"] = {"h100_triton_fused_iv_per_s": 1.79e9, "h100_max_rel_err": 9.3e-14,
                                  "h100_label_pipeline_per_s": 48.9e6, "source": "PAPER.md:156,175 (1e5 rows; not the target)"}
         print(json.dumps(line), flush=True)

@@ -58,10 +58,12 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __re
 // config 1/4 rows leave at the validity check; here the solver's warps are full.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
-constexpr int kTileRowsPerThread = 4;
-constexpr int kTileRows = kTileThreads * kTileRowsPerThread;  // 2048 rows, 104 KB of shared memory, 2 CTAs per SM
+// RPT rows per thread: 4 (1024-row tiles, 63.5 KB of shared memory, 3 CTAs per SM) for large n; 1 (256-row tiles) for
+// small n, so that a launch of 65,536 rows still spreads over every SM.
 
+template <int RPT>
 struct TileSmem {
+  static constexpr int kTileRows = kTileThreads * RPT;
   double sig[kTileRows];      // phase A: tau (queued rows) or final sigma;  phase B2: final sigma
   double veg[kTileRows];      // phase A: D sqrt(FK) (queued rows) or 0;      phase B2: final vega
   double q0[kTileRows];       // compact queue.  after A: F, K, B, sqrt(FK);  after B1: x, s0, p1, p2 (lbr_seed)
@@ -77,12 +79,13 @@ struct TileSmem {
   int nkind[3];               // rows per class: zone 0, zones 1-2, zone 3
 };
 
-template <bool BSM, bool ZONES>
+template <bool BSM, bool ZONES, int RPT>
 __global__ void __launch_bounds__(kTileThreads, 3)
 forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                     uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  TileSmem& sm = *reinterpret_cast<TileSmem*>(smem_raw);
+  constexpr int kTileRows = kTileThreads * RPT;
+  TileSmem<RPT>& sm = *reinterpret_cast<TileSmem<RPT>*>(smem_raw);
   const int tid = threadIdx.x;
   const int lane = tid & 31;
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
@@ -98,10 +101,10 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const double* __restrict__ gf = in.flag + base;
   const double* __restrict__ gr = BSM ? in.r + base : nullptr;
   const double* __restrict__ gq = BSM ? in.q + base : nullptr;
-  double vF[kTileRowsPerThread], vK[kTileRowsPerThread], vT[kTileRowsPerThread], vP[kTileRowsPerThread],
-      vf[kTileRowsPerThread], vr[kTileRowsPerThread], vq[kTileRowsPerThread];
+  double vF[RPT], vK[RPT], vT[RPT], vP[RPT],
+      vf[RPT], vr[RPT], vq[RPT];
 #pragma unroll
-  for (int k = 0; k < kTileRowsPerThread; ++k) {
+  for (int k = 0; k < RPT; ++k) {
     const int p = k * kTileThreads + tid;
     const bool live = p < rows;
     // dead rows read as flag = 0 -> BAD_INPUT, never stored
@@ -115,7 +118,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   }
   unsigned qmask = 0, cmask = 0;  // bit k: row k of this thread is queued / is a call
 #pragma unroll
-  for (int k = 0; k < kTileRowsPerThread; ++k) {
+  for (int k = 0; k < RPT; ++k) {
     const int p = k * kTileThreads + tid;
     const Prelude pr = lbr_prelude<BSM>(vF[k], vK[k], vT[k], vr[k], vq[k], vP[k], vf[k]);
     const bool queued = pr.status == 0;
@@ -142,7 +145,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     if (lane == 31 && incl > 0) wbase = atomicAdd(&sm.count, incl);
     int slot = __shfl_sync(0xffffffffu, wbase, 31) + incl - c;
 #pragma unroll
-    for (int k = 0; k < kTileRowsPerThread; ++k) {
+    for (int k = 0; k < RPT; ++k) {
       if (qmask & (1u << k)) {
         sm.q0[slot] = vF[k];
         sm.q1[slot] = vK[k];
@@ -222,7 +225,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
 
   // ---- phase C
 #pragma unroll 4
-  for (int k = 0; k < kTileRowsPerThread; ++k) {
+  for (int k = 0; k < RPT; ++k) {
     const int p = k * kTileThreads + tid;
     if (p < rows) {
       __stcs(sigma + base + p, sm.sig[p]);
@@ -324,11 +327,20 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
     const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
     forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, 0, n, sigma, vega, status, zone);
   } else {
-    static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES>,
-                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem));
-    if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
-    const int64_t blocks = (n + kTileRows - 1) / kTileRows;
-    forward_kernel_tile<BSM, ZONES><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem), st>>>(in, n, sigma, vega, status, zone);
+    // small launches use 256-row tiles so that the grid still covers the chip (n <= 2^19: at most 2048 CTAs)
+    if (n <= ((int64_t)1 << 19)) {
+      static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES, 1>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<1>));
+      if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
+      const int64_t blocks = (n + kTileThreads - 1) / kTileThreads;
+      forward_kernel_tile<BSM, ZONES, 1><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<1>), st>>>(in, n, sigma, vega, status, zone);
+    } else {
+      static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES, 4>,
+                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<4>));
+      if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
+      const int64_t blocks = (n + 4 * kTileThreads - 1) / (4 * kTileThreads);
+      forward_kernel_tile<BSM, ZONES, 4><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<4>), st>>>(in, n, sigma, vega, status, zone);
+    }
   }
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
