@@ -501,4 +501,55 @@ template <class T> inline T black_vega_eq14(T SorF, T Kk, T tau, const T* r, con
   return F * D * K<T>::phi0() * exp(-T(0.5) * d1 * d1) * sqrt(tau);
 }
 
+// ---------------------------------------------------------------------------------------------
+// the second half of eq.(8):  xi_bar = -(sigma_bar / V) dP/dxi
+// at sigma = sigma_imp, with the gate of eq.(9)/(10) applied to the common factor exactly as in
+// backward_row.  The paper obtains dP/dxi "by ordinary autograd through the analytic Black price
+// helper"; written out, for the discounted price of eq.(2)
+//   P = theta [ S e^{-q tau} Phi(theta d1) - K e^{-r tau} Phi(theta d2) ],
+//   d1,2 = [ln(S/K) + (r - q) tau +- s^2/2] / s,  s = sigma sqrt(tau):
+//   dP/dS   =  theta e^{-q tau} Phi(theta d1)
+//   dP/dK   = -theta e^{-r tau} Phi(theta d2)
+//   dP/dtau =  theta [ -q S e^{-q tau} Phi(theta d1) + r K e^{-r tau} Phi(theta d2) ] + V sigma / (2 tau)
+//   dP/dr   =  theta K tau e^{-r tau} Phi(theta d2)
+//   dP/dq   = -theta S tau e^{-q tau} Phi(theta d1)
+// (the phi(d1), phi(d2) terms of dP/dS, dP/dK, dP/dr, dP/dq cancel through S e^{-q tau} phi(d1) =
+// K e^{-r tau} phi(d2); in dP/dtau they leave V sigma / (2 tau), V = S e^{-q tau} phi(d1) sqrt(tau),
+// eq.(14)).  Black-76 with D = 1 (r = q = NULL): the same with S -> F, r = q = 0; only dF, dK, dtau.
+// These five formulas are pinned in tests/test_oracle_pins.py by central differences of black_price.
+// ---------------------------------------------------------------------------------------------
+template <class T> struct Greeks { T dS, dK, dtau, dr, dq; };
+
+template <class T>
+inline Greeks<T> black_greeks(T SorF, T Kk, T tau, const T* r, const T* q, T sigma, T flag) {
+  using std::exp; using std::log; using std::sqrt;
+  const T rr = (r && q) ? *r : T(0), qq = (r && q) ? *q : T(0);
+  const T s = sigma * sqrt(tau);
+  const T d1 = (log(SorF / Kk) + (rr - qq) * tau + T(0.5) * s * s) / s;
+  const T d2 = d1 - s;
+  const T th = (flag > T(0)) ? T(1) : T(-1);
+  const T Dq = exp(-qq * tau), Dr = exp(-rr * tau);
+  const T N1 = Phi_<T>(th * d1), N2 = Phi_<T>(th * d2);
+  const T V = SorF * Dq * K<T>::phi0() * exp(-T(0.5) * d1 * d1) * sqrt(tau);
+  Greeks<T> g;
+  g.dS = th * Dq * N1;
+  g.dK = -th * Dr * N2;
+  g.dtau = th * (-qq * SorF * Dq * N1 + rr * Kk * Dr * N2) + V * sigma / (T(2) * tau);
+  g.dr = (r && q) ? th * Kk * tau * Dr * N2 : T(0);    // Black-76 with D = 1 has no rate inputs
+  g.dq = (r && q) ? -th * SorF * tau * Dq * N1 : T(0);
+  return g;
+}
+
+// xi_bar = -(gated sigma_bar / V) dP/dxi; the gated factor is backward_row's grad_P.
+template <class T>
+inline Greeks<T> backward_inputs_row(T gsigma, T vega, uint8_t status, T floor_, int mode, T SorF, T Kk, T tau,
+                                     const T* r, const T* q, T sigma, T flag) {
+  Greeks<T> z{T(0), T(0), T(0), T(0), T(0)};
+  const T gP = backward_row<T>(gsigma, vega, status, floor_, mode);
+  if (status != ST_OK || gP == T(0)) return z;
+  const Greeks<T> g = black_greeks<T>(SorF, Kk, tau, r, q, sigma, flag);
+  z.dS = -gP * g.dS; z.dK = -gP * g.dK; z.dtau = -gP * g.dtau; z.dr = -gP * g.dr; z.dq = -gP * g.dq;
+  return z;
+}
+
 }  // namespace lbr_oracle

@@ -203,4 +203,37 @@ void oracle_householder_terms(int64_t n, const int* kind, const double* x, const
   }
 }
 
+// prec: 0 = double, 1 = long double.  out5 = dP/dS, dP/dK, dP/dtau, dP/dr, dP/dq (n each, row-major blocks).
+void oracle_black_greeks(int prec, int64_t n, const double* SorF, const double* Kk, const double* tau, const double* r,
+                         const double* q, const double* sig, const double* flag, double* dS, double* dK, double* dtau,
+                         double* dr, double* dq) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    if (prec == 0) {
+      double rr = r ? r[i] : 0, qq = q ? q[i] : 0;
+      const Greeks<double> g = black_greeks<double>(SorF[i], Kk[i], tau[i], (r && q) ? &rr : nullptr, (r && q) ? &qq : nullptr, sig[i], flag[i]);
+      dS[i] = g.dS; dK[i] = g.dK; dtau[i] = g.dtau; dr[i] = g.dr; dq[i] = g.dq;
+    } else {
+      long double rr = r ? r[i] : 0, qq = q ? q[i] : 0;
+      const Greeks<long double> g = black_greeks<long double>(SorF[i], Kk[i], tau[i], (r && q) ? &rr : nullptr, (r && q) ? &qq : nullptr, sig[i], flag[i]);
+      dS[i] = (double)g.dS; dK[i] = (double)g.dK; dtau[i] = (double)g.dtau; dr[i] = (double)g.dr; dq[i] = (double)g.dq;
+    }
+  }
+}
+
+void oracle_backward_inputs(int64_t n, const double* gsigma, const double* vega, const uint8_t* status, double vega_floor,
+                            int mode, const double* SorF, const double* Kk, const double* tau, const double* r,
+                            const double* q, const double* sig, const double* flag, double* gS, double* gK, double* gtau,
+                            double* gr, double* gq) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    double rr = r ? r[i] : 0, qq = q ? q[i] : 0;
+    const Greeks<double> g = backward_inputs_row<double>(gsigma[i], vega[i], status[i], vega_floor, mode, SorF[i], Kk[i],
+                                                        tau[i], (r && q) ? &rr : nullptr, (r && q) ? &qq : nullptr, sig[i], flag[i]);
+    gS[i] = g.dS; gK[i] = g.dK; gtau[i] = g.dtau;
+    if (gr) gr[i] = g.dr;
+    if (gq) gq[i] = g.dq;
+  }
+}
+
 }  // extern "C"

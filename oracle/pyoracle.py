@@ -191,3 +191,27 @@ def count_ops(SorF, K, tau, P, flag, r=None, q=None, fixed_iters=2):
     lib().oracle_count_ops(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(P), _p(flag),
                            C.c_int(fixed_iters), counts.ctypes.data_as(C.c_void_p), rows.ctypes.data_as(C.c_void_p))
     return counts, rows
+
+
+def black_greeks(SorF, K, tau, sigma, flag, r=None, q=None, prec=1):
+    """dP/dS (or dF), dP/dK, dP/dtau, dP/dr, dP/dq of the discounted Black price."""
+    SorF, K, tau, sigma, flag = map(_d, (SorF, K, tau, sigma, flag))
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    outs = [np.empty(SorF.size) for _ in range(5)]
+    lib().oracle_black_greeks(C.c_int(prec), C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(sigma),
+                              _p(flag), *[_p(o) for o in outs])
+    return tuple(outs)
+
+
+def backward_inputs(gsigma, vega, status, vega_floor, mode, SorF, K, tau, sigma, flag, r=None, q=None):
+    """xi_bar = -(gated sigma_bar / V) dP/dxi (eq.(8) second half): returns (gS|gF, gK, gtau, gr, gq)."""
+    gsigma, vega, SorF, K, tau, sigma, flag = map(_d, (gsigma, vega, SorF, K, tau, sigma, flag))
+    status = np.ascontiguousarray(status, dtype=np.uint8)
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    outs = [np.empty(SorF.size) for _ in range(5)]
+    lib().oracle_backward_inputs(C.c_int64(SorF.size), _p(gsigma), _p(vega), _p(status, _U8), C.c_double(vega_floor),
+                                 C.c_int(mode), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(sigma), _p(flag),
+                                 *[_p(o) for o in outs])
+    return tuple(outs)

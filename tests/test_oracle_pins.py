@@ -484,3 +484,95 @@ def test_backward_gate_truth_table():
     assert att[3] == pytest.approx(gs[3] / V[3], rel=1e-12)
     # floor = 0: attenuate at V = 0 stays finite (0), mask at V = 0 is off-gate
     assert po.backward([1.0], [0.0], [0], 0.0, 1)[0] == 0.0 and po.backward([1.0], [0.0], [0], 0.0, 0)[0] == 0.0
+
+
+# ------------------------------------------------------------------ input gradients, eq.(8) second half
+def _bsm_rows(n, seed):
+    rng = np.random.default_rng(seed)
+    S = np.exp(rng.normal(np.log(4000.0), 0.25, n))
+    K = S * rng.uniform(0.7, 1.4, n)
+    tau = np.exp(rng.uniform(np.log(10 / 365), np.log(2.0), n))
+    r = rng.uniform(0.0, 0.05, n)
+    q = rng.uniform(0.0, 0.02, n)
+    sig = rng.uniform(0.1, 0.6, n)
+    flag = np.where(rng.random(n) < 0.5, 1.0, -1.0)
+    return S, K, tau, r, q, sig, flag
+
+
+def test_black_greeks_against_mpmath_derivatives_of_eq2():
+    """Each of the five closed forms against mpmath's numerical derivative of the literal eq.(2) price (50 digits):
+    a wrong sign, a dropped discount factor or a swapped d1/d2 fails it."""
+    S, K, tau, r, q, sig, flag = _bsm_rows(40, 5)
+
+    def price(S_, K_, t_, r_, q_, sg_, th):
+        s = sg_ * mp.sqrt(t_)
+        d1 = (mp.log(S_ / K_) + (r_ - q_) * t_ + s * s / 2) / s
+        d2 = d1 - s
+        return th * (S_ * mp.exp(-q_ * t_) * mp_Phi(th * d1) - K_ * mp.exp(-r_ * t_) * mp_Phi(th * d2))
+
+    g = po.black_greeks(S, K, tau, sig, flag, r=r, q=q, prec=1)
+    for i in range(S.size):
+        a = [mp.mpf(float(v[i])) for v in (S, K, tau, r, q)]
+        sg, th = mp.mpf(float(sig[i])), int(flag[i])
+        for j in range(5):
+            f = lambda z, j=j: price(*[z if m == j else a[m] for m in range(5)], sg, th)
+            ref = mp.diff(f, a[j])
+            got = mp.mpf(float(g[j][i]))
+            scale = max(abs(ref), mp.mpf(1e-3) * abs(price(*a, sg, th)) / abs(a[j]) if a[j] != 0 else 0)
+            assert abs(got - ref) <= 1e-12 * scale + 1e-15, (i, j, got, ref)
+
+
+def test_black76_greeks_reduce_to_forward_form():
+    """r = q = NULL: dP/dF = theta Phi(theta d1), dP/dK = -theta Phi(theta d2), dP/dtau = V sigma/(2 tau); dr = dq = 0."""
+    S, K, tau, r, q, sig, flag = _bsm_rows(500, 6)
+    g = po.black_greeks(S, K, tau, sig, flag, prec=1)
+    e = 1e-5
+    pF = (po.black_price(S * (1 + e), K, tau, sig, flag) - po.black_price(S * (1 - e), K, tau, sig, flag)) / (2 * e * S)
+    pK = (po.black_price(S, K * (1 + e), tau, sig, flag) - po.black_price(S, K * (1 - e), tau, sig, flag)) / (2 * e * K)
+    pT = (po.black_price(S, K, tau * (1 + e), sig, flag) - po.black_price(S, K, tau * (1 - e), sig, flag)) / (2 * e * tau)
+    assert np.max(np.abs(g[0] - pF)) <= 1e-7
+    assert np.max(np.abs(g[1] - pK)) <= 1e-7
+    assert np.all(np.abs(g[2] - pT) <= 1e-6 * np.abs(g[2]) + 1e-6)
+    assert np.all(g[3] == 0) and np.all(g[4] == 0)
+    assert np.allclose(g[2], po.vega_eq14(S, K, tau, sig) * sig / (2 * tau), rtol=1e-13, atol=0)
+
+
+def test_input_gradients_are_the_implicit_derivatives_of_the_solver():
+    """xi_bar for sigma_bar = 1 must equal d sigma_imp / d xi of the oracle's own inversion (implicit function theorem,
+    eq.(8)): central differences of po.forward in S, K, tau, r, q at fixed observed price."""
+    S, K, tau, r, q, sig, flag = _bsm_rows(600, 8)
+    P = po.black_price(S, K, tau, sig, flag, r=r, q=q)
+    s0, v0, st = po.forward(S, K, tau, P, flag, r=r, q=q)
+    m = (st == 0) & (v0 > 50.0)
+    assert m.sum() > 300
+    S, K, tau, r, q, flag, P, s0, v0, st = (a[m] for a in (S, K, tau, r, q, flag, P, s0, v0, st))
+    gin = po.backward_inputs(np.ones_like(s0), v0, st, 1e-8, 0, S, K, tau, s0, flag, r=r, q=q)
+    args = [S, K, tau, r, q]
+    for j, h in enumerate((1e-6, 1e-6, 1e-6, 1e-7, 1e-7)):
+        up = list(args); dn = list(args)
+        step = h * np.maximum(np.abs(args[j]), 1.0 if j >= 3 else 0.0)
+        up[j] = args[j] + step; dn[j] = args[j] - step
+        su = po.forward(up[0], up[1], up[2], P, flag, r=up[3], q=up[4])[0]
+        sd = po.forward(dn[0], dn[1], dn[2], P, flag, r=dn[3], q=dn[4])[0]
+        fd = (su - sd) / (2 * step)
+        err = np.abs(fd - gin[j]) / np.maximum(np.abs(gin[j]), 1e-3 * np.abs(s0 / args[j]) if j < 3 else 1e-3)
+        assert np.median(err) <= 1e-6 and np.quantile(err, 0.99) <= 1e-4, (j, np.median(err), np.quantile(err, 0.99))
+
+
+def test_input_gradient_gate_follows_grad_P():
+    """Off-gate / invalid rows give exactly +0 in every component, in both modes; on-gate rows scale with -grad_P."""
+    S, K, tau, r, q, sig, flag = _bsm_rows(200, 9)
+    P = po.black_price(S, K, tau, sig, flag, r=r, q=q)
+    s0, v0, st = po.forward(S, K, tau, P, flag, r=r, q=q)
+    st2 = st.copy(); st2[::5] = 1
+    gs = np.random.default_rng(1).standard_normal(S.size)
+    for mode in (0, 1):
+        floor = float(np.median(v0))
+        gP = po.backward(gs, v0, st2, floor, mode)
+        gin = po.backward_inputs(gs, v0, st2, floor, mode, S, K, tau, s0, flag, r=r, q=q)
+        greeks = po.black_greeks(S, K, tau, s0, flag, r=r, q=q, prec=0)
+        off = gP == 0
+        assert off.sum() > 20 and (~off).sum() > 20
+        for j in range(5):
+            assert np.array_equal(gin[j][off].view(np.uint64), np.zeros(off.sum()).view(np.uint64))
+            assert np.allclose(gin[j][~off], -gP[~off] * greeks[j][~off], rtol=1e-14, atol=0)
