@@ -94,6 +94,32 @@ int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, 
 int pivot_iv_backward(const double* grad_sigma, const double* vega, const uint8_t* status, double vega_floor,
                       int mode, int64_t n, double* grad_P, pivot_iv_stream stream);
 
+/* ---- next rows of the path ---- */
+/* The smooth Black price node P_BSM(xi, sigma; theta) and its vega (eq.(2)/(3); :322 eq.(14)): what the
+ * price loss eq.(11) and the round trip of eq.(12) evaluate.  Evaluated as
+ * D (intrinsic + sqrt(FK) b(x, sigma sqrt(tau))) so that deep in-the-money rows keep their time value.
+ *   in      device pointers; in->P is not read and may be NULL; r = q = NULL selects Black-76 with D = 1
+ *   sigma   [in, device, n doubles] volatility; 0 gives the discounted intrinsic value; negative / NaN / bad inputs give NaN
+ *   price   [out, device, n doubles]; vega [out, device, n doubles] may be NULL.
+ * Returns PIVOT_ERR_NULL / _BAD_N / _MIXED_RQ / _CUDA. */
+int pivot_iv_black_price(const pivot_iv_inputs* in, const double* sigma, int64_t n, double* price, double* vega,
+                      pivot_iv_stream stream);
+
+/* Full vector-Jacobian product of eq.(8), one fused elementwise kernel:
+ *   grad_P = gate * grad_sigma / vega            (exactly pivot_iv_backward's value, same gate and modes)
+ *   xi_bar = -grad_P * dP/dxi at sigma = sigma_imp, xi = (S, K, tau, r, q) in BSM mode, (F, K, tau) in Black-76 mode,
+ * with the analytic derivatives of the discounted price eq.(2) (the paper differentiates a price helper by autograd):
+ *   dP/dS = theta e^{-q tau} Phi(theta d1), dP/dK = -theta e^{-r tau} Phi(theta d2), dP/dr = theta K tau e^{-r tau} Phi(theta d2),
+ *   dP/dq = -theta S tau e^{-q tau} Phi(theta d1), dP/dtau = theta[-q S e^{-q tau} Phi(theta d1) + r K e^{-r tau} Phi(theta d2)] + V sigma/(2 tau).
+ * Rows that are not OK or off-gate get exactly +0.0 in every output.
+ *   in, sigma, vega, status  the forward's inputs and outputs (device); in->P is not read
+ *   grad_sigma [in, n]; grad_P, grad_S_or_F, grad_K, grad_tau [out, n]; grad_r, grad_q [out, n] required iff BSM mode.
+ * Returns PIVOT_ERR_NULL / _BAD_N / _BAD_MODE / _BAD_FLOOR / _MIXED_RQ / _CUDA. */
+int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, const double* vega, const uint8_t* status,
+                             const double* grad_sigma, double vega_floor, int mode, int64_t n, double* grad_P,
+                             double* grad_S_or_F, double* grad_K, double* grad_tau, double* grad_r, double* grad_q,
+                             pivot_iv_stream stream);
+
 /* ---- host-buffer pipeline (the streaming label-generation setting: batches of rows, H2D included) ----
  * A pipeline owns `n_slots` device staging slots of `chunk_rows` rows each, one CUDA stream per slot and pinned
  * bounce buffers are NOT used: host arrays are copied directly (pin them for full PCIe speed).  The *_host calls split

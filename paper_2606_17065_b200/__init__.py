@@ -11,7 +11,9 @@ from .binding import (  # noqa: F401
     Pipeline,
     library_path,
     load_library,
+    pivot_iv_black_price,
     pivot_iv_backward,
+    pivot_iv_backward_inputs,
     pivot_iv_forward,
     pivot_iv_forward_zones,
     pivot_iv_probe_dfma,
@@ -21,7 +23,8 @@ from .binding import (  # noqa: F401
 )
 
 __all__ = [
-    "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "Pipeline", "pivot_iv_probe_dfma",
+    "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_backward_inputs", "pivot_iv_black_price",
+    "Pipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
     "GATE_ATTENUATE", "EXPORTS",
 ]

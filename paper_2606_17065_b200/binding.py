@@ -18,6 +18,7 @@ EXPORTS = (
     "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_pipeline_create",
     "pivot_iv_pipeline_destroy", "pivot_iv_forward_host", "pivot_iv_forward_backward_host", "pivot_iv_probe_dfma",
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
+    "pivot_iv_black_price", "pivot_iv_backward_inputs",
 )
 
 
@@ -54,6 +55,8 @@ def load_library():
     lib.pivot_iv_forward_host.argtypes = [vp, C.POINTER(_Inputs), i64, vp, vp, vp]
     lib.pivot_iv_forward_backward_host.argtypes = [vp, C.POINTER(_Inputs), vp, dbl, cint, i64, vp, vp, vp, vp]
     lib.pivot_iv_probe_dfma.argtypes = [i64, vp, C.POINTER(dbl), vp]
+    lib.pivot_iv_black_price.argtypes = [C.POINTER(_Inputs), vp, i64, vp, vp, vp]
+    lib.pivot_iv_backward_inputs.argtypes = [C.POINTER(_Inputs), vp, vp, vp, vp, dbl, cint, i64, vp, vp, vp, vp, vp, vp, vp]
     lib.pivot_iv_strerror.argtypes = [cint]
     lib.pivot_iv_strerror.restype = C.c_char_p
     for name in EXPORTS:
@@ -147,6 +150,40 @@ def pivot_iv_backward(grad_sigma, vega, status, vega_floor: float, mode: int, ou
                                      _dev(status, "status", torch.uint8), float(vega_floor), int(mode), n,
                                      _dev(gP, "grad_P"), _stream_ptr(stream)))
     return gP
+
+
+def pivot_iv_black_price(S_or_F, K, tau, sigma, flag, r=None, q=None, with_vega=True, stream=None):
+    """(price, vega) of the Black-76 / BSM price eq.(2)/(3) at `sigma` (CUDA fp64 tensors); vega is None if not asked."""
+    _require_cuda()
+    lib = load_library()
+    n = S_or_F.numel()
+    inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), None,
+                  _dev(flag, "flag"))
+    price = torch.empty(n, dtype=torch.float64, device=S_or_F.device)
+    vega = torch.empty(n, dtype=torch.float64, device=S_or_F.device) if with_vega else None
+    with torch.cuda.device(S_or_F.device):
+        _check(lib.pivot_iv_black_price(C.byref(inp), _dev(sigma, "sigma"), n, _dev(price, "price"), _dev(vega, "vega"),
+                                     _stream_ptr(stream)))
+    return price, vega
+
+
+def pivot_iv_backward_inputs(S_or_F, K, tau, flag, sigma, vega, status, grad_sigma, vega_floor: float, mode: int,
+                             r=None, q=None, stream=None):
+    """Full VJP of eq.(8): returns (grad_P, grad_S_or_F, grad_K, grad_tau, grad_r, grad_q); the last two are None in
+    Black-76 mode (r = q = None)."""
+    _require_cuda()
+    lib = load_library()
+    n = S_or_F.numel()
+    inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), None,
+                  _dev(flag, "flag"))
+    outs = [torch.empty(n, dtype=torch.float64, device=S_or_F.device) for _ in range(4)]
+    outs += [torch.empty(n, dtype=torch.float64, device=S_or_F.device) if r is not None else None for _ in range(2)]
+    with torch.cuda.device(S_or_F.device):
+        _check(lib.pivot_iv_backward_inputs(C.byref(inp), _dev(sigma, "sigma"), _dev(vega, "vega"),
+                                            _dev(status, "status", torch.uint8), _dev(grad_sigma, "grad_sigma"),
+                                            float(vega_floor), int(mode), n, *[_dev(o, "grad") for o in outs],
+                                            _stream_ptr(stream)))
+    return tuple(outs)
 
 
 def pivot_iv_probe_dfma(iters: int, stream=None) -> float:

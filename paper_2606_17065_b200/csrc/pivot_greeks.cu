@@ -1,0 +1,189 @@
+// pivot_greeks.cu -- the "next" rows of the hot path, sm_100a:
+//   pivot_iv_black_price        the smooth Black price node P_BSM(xi, sigma; theta) and its vega (eq.(2)/(3),
+//                            :322 eq.(14)) -- what L_price eq.(11) and the round trip of eq.(12) evaluate;
+//   pivot_iv_backward_inputs the full VJP of eq.(8): grad_P and xi_bar = -(sigma_bar/V) dP/dxi with
+//                            analytic Greeks instead of autograd through a price helper, same gate as pivot_iv_backward.
+// Both are streaming elementwise kernels (one thread per row, coalesced 8-byte accesses, every element touched once).
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "../../include/pivot_iv.h"
+#include "lbr_device.cuh"
+
+namespace pivot {
+
+constexpr int kEwThreads = 256;
+
+// Black price through the OTM-normalised form: P = D (intrinsic + sqrt(FK) b(x, s)), b from the same W / Wbar ratios as
+// the solver (no cancellation for deep in-the-money rows).  sigma == 0 gives the discounted intrinsic value; NaN / negative
+// sigma or bad inputs give NaN.
+template <bool BSM>
+__device__ __forceinline__ void black_row(double SorF, double K, double tau, double r, double q, double sigma, double flag,
+                                          double& price, double& vega) {
+  price = canonical_nan();
+  vega = canonical_nan();
+  bool bad = !pos_fin(SorF) || !pos_fin(K) || !pos_fin(tau) || !(sigma >= 0.0) || !is_fin(sigma) ||
+             !(flag == 1.0 || flag == -1.0);
+  double F = SorF, D = 1.0;
+  if (BSM) {
+    if (!is_fin(r) || !is_fin(q)) bad = true;
+    if (!bad) {
+      F = SorF * exp((r - q) * tau);
+      D = exp(-r * tau);
+      if (!pos_fin(F) || !pos_fin(D)) bad = true;
+    }
+  }
+  const double rootFK = sqrt(F * K);
+  const double lo = fmin(F, K), hi = fmax(F, K);
+  if (!pos_fin(rootFK) || !(lo * 0x1p500 >= rootFK)) bad = true;
+  if (bad) return;
+  const bool call = flag > 0.0;
+  const double iota = fmax(call ? F - K : K - F, 0.0);
+  const double rt = sqrt(tau);
+  const double s = sigma * rt;
+  double b = 0.0, v = 0.0;
+  if (s > 0.0) {
+    const double x = -log1p_fast((hi - lo) / lo);
+    const WEval w = eval_W(x, s);
+    v = kPhi0 * exp_fast(-w.E);
+    b = w.have_W ? w.Wd * v : fma(-w.Wd, v, lo / rootFK);
+  }
+  price = D * fma(rootFK, b, iota);
+  vega = D * rootFK * v * rt;
+}
+
+template <bool BSM>
+__global__ void __launch_bounds__(kEwThreads)
+black_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, int64_t n, double* __restrict__ price,
+                   double* __restrict__ vega) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+    double p, v;
+    black_row<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(sigma + i),
+                   __ldcs(in.flag + i), p, v);
+    __stcs(price + i, p);
+    if (vega) __stcs(vega + i, v);
+  }
+}
+
+// Phi(z1), Phi(z2) from one erfcx pair and two exps: Phi(-|z|) = erfcx(|z|/sqrt2) exp(-z^2/2) / 2.
+__device__ __forceinline__ void Phi_pair(double z1, double z2, double& P1, double& P2) {
+  double e1, e2;
+  erfcx_pair(fabs(z1) * kInvSqrt2, fabs(z2) * kInvSqrt2, e1, e2);
+  const double t1 = 0.5 * e1 * exp_fast(-0.5 * z1 * z1), t2 = 0.5 * e2 * exp_fast(-0.5 * z2 * z2);
+  P1 = (z1 < 0.0) ? t1 : 1.0 - t1;
+  P2 = (z2 < 0.0) ? t2 : 1.0 - t2;
+}
+
+template <bool BSM, int MODE>
+__global__ void __launch_bounds__(kEwThreads)
+backward_inputs_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, const double* __restrict__ vega,
+                       const uint8_t* __restrict__ status, const double* __restrict__ gs, double floor_, int64_t n,
+                       double* __restrict__ gP, double* __restrict__ gS, double* __restrict__ gK, double* __restrict__ gT,
+                       double* __restrict__ gR, double* __restrict__ gQ) {
+  const double floor2 = __dmul_rn(floor_, floor_);
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double V = __ldcs(vega + i), g = __ldcs(gs + i);
+    const uint8_t st = status[i];
+    // the gated common factor: exactly pivot_iv_backward's grad_P
+    double c;
+    if (MODE == PIVOT_GATE_MASK) {
+      c = ((st == PIVOT_ST_OK) && (fabs(V) > floor_)) ? __ddiv_rn(g, V) : 0.0;
+    } else {
+      const double den = __dadd_rn(__dmul_rn(V, V), floor2);
+      c = ((st == PIVOT_ST_OK) && (den > 0.0)) ? __ddiv_rn(__dmul_rn(g, V), den) : 0.0;
+    }
+    double dS = 0.0, dK = 0.0, dT = 0.0, dR = 0.0, dQ = 0.0;
+    if (st == PIVOT_ST_OK && c != 0.0) {
+      const double S = __ldcs(in.S_or_F + i), K = __ldcs(in.K + i), tau = __ldcs(in.tau + i), sg = __ldcs(sigma + i);
+      const double th = (__ldcs(in.flag + i) > 0.0) ? 1.0 : -1.0;
+      const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+      const double s = sg * sqrt(tau);
+      const double d1 = (log_fast(S / K) + (r - q) * tau + 0.5 * s * s) / s;
+      const double d2 = d1 - s;
+      double N1, N2;
+      Phi_pair(th * d1, th * d2, N1, N2);
+      const double Dq = BSM ? exp_fast(-q * tau) : 1.0, Dr = BSM ? exp_fast(-r * tau) : 1.0;
+      const double a1 = th * Dq * N1, a2 = th * Dr * N2;   // dP/dS, -dP/dK
+      dS = -c * a1;
+      dK = c * a2;
+      dT = -c * (fma(-q * S, a1, r * K * a2) + V * sg / (2.0 * tau));
+      dR = -c * (K * tau * a2);
+      dQ = c * (S * tau * a1);
+    }
+    __stcs(gP + i, c);
+    __stcs(gS + i, dS);
+    __stcs(gK + i, dK);
+    __stcs(gT + i, dT);
+    if (BSM) {
+      __stcs(gR + i, dR);
+      __stcs(gQ + i, dQ);
+    }
+  }
+}
+
+inline int ew_blocks(int64_t n) {
+  static const int sms = [] {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0)
+      v = 148;
+    return v;
+  }();
+  int64_t blocks = (n + kEwThreads - 1) / kEwThreads;
+  const int64_t cap = (int64_t)sms * 8 * 4;  // 8 resident CTAs of 256 threads per SM, 4 waves' worth; grid-stride beyond
+  return (int)(blocks < cap ? blocks : cap);
+}
+
+}  // namespace pivot
+
+using namespace pivot;
+
+extern "C" {
+
+int pivot_iv_black_price(const pivot_iv_inputs* in, const double* sigma, int64_t n, double* price, double* vega,
+                      pivot_iv_stream stream) {
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (n == 0) return PIVOT_OK;
+  if (!in->S_or_F || !in->K || !in->tau || !in->flag || !sigma || !price) return PIVOT_ERR_NULL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (in->r)
+    black_price_kernel<true><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma, n, price, vega);
+  else
+    black_price_kernel<false><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma, n, price, vega);
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, const double* vega, const uint8_t* status,
+                             const double* grad_sigma, double vega_floor, int mode, int64_t n, double* grad_P,
+                             double* grad_S_or_F, double* grad_K, double* grad_tau, double* grad_r, double* grad_q,
+                             pivot_iv_stream stream) {
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE) return PIVOT_ERR_BAD_MODE;
+  if (!(vega_floor >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (n == 0) return PIVOT_OK;
+  const bool bsm = in->r != nullptr;
+  if (!in->S_or_F || !in->K || !in->tau || !in->flag || !sigma || !vega || !status || !grad_sigma || !grad_P ||
+      !grad_S_or_F || !grad_K || !grad_tau || (bsm && (!grad_r || !grad_q)))
+    return PIVOT_ERR_NULL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const int blocks = ew_blocks(n);
+#define PIVOT_LAUNCH_BI(B, M)                                                                                         \
+  backward_inputs_kernel<B, M><<<blocks, kEwThreads, 0, st>>>(*in, sigma, vega, status, grad_sigma, vega_floor, n,    \
+                                                              grad_P, grad_S_or_F, grad_K, grad_tau, grad_r, grad_q)
+  if (bsm) {
+    if (mode == PIVOT_GATE_MASK) PIVOT_LAUNCH_BI(true, PIVOT_GATE_MASK); else PIVOT_LAUNCH_BI(true, PIVOT_GATE_ATTENUATE);
+  } else {
+    if (mode == PIVOT_GATE_MASK) PIVOT_LAUNCH_BI(false, PIVOT_GATE_MASK); else PIVOT_LAUNCH_BI(false, PIVOT_GATE_ATTENUATE);
+  }
+#undef PIVOT_LAUNCH_BI
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+}  // extern "C"
