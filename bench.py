@@ -350,6 +350,31 @@ def main():
                     "unit": "GB/s", "frac": bwd_gbs / hbm_peak, "traffic": None, "avg_launch_ms": bwd_ms,
                     "peak_source": peak_src}
 
+    # --- the "next" rows, timed separately from the step: Black price node and full-VJP backward
+    next_rows = None
+    if rank == 0 and world == 1:
+        def _time(fn, reps=10):
+            for _ in range(3):
+                fn()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(reps):
+                fn()
+            e1.record(stream); torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / reps
+        sig_in = torch.where(out[2] == 0, out[0], torch.full_like(out[0], 0.2))
+        ms_p = _time(lambda: pv.pivot_iv_black_price(a[0], a[1], a[2], sig_in, a[4], stream=stream))
+        ms_b = _time(lambda: pv.pivot_iv_backward_inputs(a[0], a[1], a[2], a[4], out[0], out[1], out[2], gsig, VEGA_FLOOR,
+                                                         pv.GATE_MASK, stream=stream))
+        on_frac = float(((out[2] == 0) & (out[1] > VEGA_FLOOR)).double().mean().item())
+        bp, bb = 56.0, 17.0 + 32.0 + 40.0 * on_frac   # algorithmic bytes/row (Black-76): see DESIGN.md section 11
+        next_rows = {"black_price": {"ms": ms_p, "rows_per_s": n / (ms_p * 1e-3), "bytes_per_row": bp,
+                                     "hbm_frac": bp * n / (ms_p * 1e-3) / 1e9 / hbm_peak},
+                     "backward_inputs": {"ms": ms_b, "rows_per_s": n / (ms_b * 1e-3), "bytes_per_row": bb,
+                                         "gate_on_fraction": on_frac,
+                                         "hbm_frac": bb * n / (ms_b * 1e-3) / 1e9 / hbm_peak}}
+        del sig_in
+
     sweep = None
     if args.sweep and rank == 0 and world == 1:
         del cfg, a, out, gP, gsig
@@ -372,6 +397,8 @@ def main():
         line.update(err)
         if sweep is not None:
             line["sweep"] = sweep
+        if next_rows is not None:
+            line["next_rows"] = next_rows
         line["paper_context"] = {"h100_triton_fused_iv_per_s": 1.79e9, "h100_max_rel_err": 9.3e-14,
                                  "h100_label_pipeline_per_s": 48.9e6, "source": "PAPER.md:156,175 (1e5 rows; not the target)"}
         print(json.dumps(line), flush=True)
