@@ -470,8 +470,15 @@ inline RowResult<T> lbr_row(T SorF, T Kk, T tau, const T* r, const T* q, T P, T 
 }
 
 // O9: backward rule.  mode 0 = MASK 1{|V| > floor}, mode 1 = ATTENUATE V^2/(V^2+floor^2).
+// mode 2 = STRICT ("Rows outside G_tau return a zero cotangent when the upstream gradient is
+// already zero, and return NaN when a loss explicitly asks for an ill-conditioned gradient"; :418 uses it with the floor
+// 1e-14): on G_tau = {OK and |V| > floor} the exact sigma_bar / V, elsewhere +0 if sigma_bar == 0 else NaN.
 template <class T> inline T backward_row(T gsigma, T vega, uint8_t status, T floor_, int mode) {
   using std::fabs;
+  if (mode == 2) {
+    if (status == ST_OK && fabs(vega) > floor_) return gsigma / vega;
+    return (gsigma == T(0)) ? T(0) : std::numeric_limits<T>::quiet_NaN();
+  }
   if (status != ST_OK) return T(0);
   if (mode == 0) return (fabs(vega) > floor_) ? gsigma / vega : T(0);
   const T den = vega * vega + floor_ * floor_;
@@ -546,6 +553,12 @@ inline Greeks<T> backward_inputs_row(T gsigma, T vega, uint8_t status, T floor_,
                                      const T* r, const T* q, T sigma, T flag) {
   Greeks<T> z{T(0), T(0), T(0), T(0), T(0)};
   const T gP = backward_row<T>(gsigma, vega, status, floor_, mode);
+  using std::fabs;
+  if (mode == 2 && !(status == ST_OK && fabs(vega) > floor_)) {  // STRICT, off the gate: every component is 0 or NaN with grad_P
+    z.dS = z.dK = z.dtau = z.dr = z.dq = gP;
+    if (!(r && q)) z.dr = z.dq = T(0);
+    return z;
+  }
   if (status != ST_OK || gP == T(0)) return z;
   const Greeks<T> g = black_greeks<T>(SorF, Kk, tau, r, q, sigma, flag);
   z.dS = -gP * g.dS; z.dK = -gP * g.dK; z.dtau = -gP * g.dtau; z.dr = -gP * g.dr; z.dq = -gP * g.dq;

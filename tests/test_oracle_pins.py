@@ -482,6 +482,18 @@ def test_backward_gate_truth_table():
     w = V ** 2 / (V ** 2 + floor ** 2)
     assert np.allclose(att, w * gs / V, rtol=1e-15)
     assert att[3] == pytest.approx(gs[3] / V[3], rel=1e-12)
+    # STRICT: exact gradient on the gate, +0 off the gate iff the upstream cotangent is 0, else NaN
+    for status in (0, 1, 2, 3, 4):
+        for V in vegas:
+            for gs in (0.0, -0.0, -2.5, 1e300, float("nan"), float("inf")):
+                out = po.backward([gs], [V], [status], floor, 2)[0]
+                if status == 0 and abs(V) > floor:
+                    exp = gs / V
+                    assert (np.isnan(exp) and np.isnan(out)) or out == exp
+                elif gs == 0.0:
+                    assert out == 0.0 and not np.signbit(out)
+                else:
+                    assert np.isnan(out)
     # floor = 0: attenuate at V = 0 stays finite (0), mask at V = 0 is off-gate
     assert po.backward([1.0], [0.0], [0], 0.0, 1)[0] == 0.0 and po.backward([1.0], [0.0], [0], 0.0, 0)[0] == 0.0
 
