@@ -32,7 +32,7 @@ extern "C" {
 #define PIVOT_OK 0
 #define PIVOT_ERR_NULL (-1)      /* a required pointer is NULL */
 #define PIVOT_ERR_BAD_N (-2)     /* n < 0 */
-#define PIVOT_ERR_BAD_MODE (-3)  /* mode not PIVOT_GATE_MASK / PIVOT_GATE_ATTENUATE */
+#define PIVOT_ERR_BAD_MODE (-3)  /* mode not PIVOT_GATE_MASK / PIVOT_GATE_ATTENUATE / PIVOT_GATE_STRICT */
 #define PIVOT_ERR_BAD_FLOOR (-4) /* vega_floor is NaN or negative */
 #define PIVOT_ERR_MIXED_RQ (-5)  /* exactly one of r, q is NULL */
 #define PIVOT_ERR_CUDA (-6)      /* CUDA runtime error (launch, copy, allocation inside a pipeline) */
@@ -49,6 +49,8 @@ extern "C" {
 /* gate modes of the backward pass (eq.(9), :148-150 eq.(10)) */
 #define PIVOT_GATE_MASK 0      /* hard mask 1{|V| > vega_floor} */
 #define PIVOT_GATE_ATTENUATE 1 /* smooth gate w(V) = V^2 / (V^2 + vega_floor^2) */
+#define PIVOT_GATE_STRICT 2    /* exact gradient on {OK, |V| > vega_floor}; elsewhere +0 if the upstream
+                                  cotangent is 0, NaN otherwise (an ill-conditioned gradient was explicitly asked for) */
 
 /* Row tuple as parallel arrays (PAPER.md:123 "every input is treated as a tensor"; :51 xi = (S,K,tau,r,q), theta).
  * For the device entry points these are DEVICE pointers; for the *_host entry points HOST pointers. */
@@ -89,6 +91,7 @@ int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, 
  *   MASK:      grad_P = grad_sigma / vega                              if status == OK and |vega| > vega_floor (strict)
  *   ATTENUATE: grad_P = grad_sigma * vega / (vega^2 + vega_floor^2)    if status == OK   (= w(V) grad_sigma / V)
  *   otherwise  grad_P = +0.0 exactly (by select, so 0*NaN never leaks).
+ *   STRICT:    grad_P = grad_sigma / vega if status == OK and |vega| > vega_floor; else +0.0 if grad_sigma == 0, else NaN.
  *   grad_sigma, vega [in, device, n doubles]; status [in, device, n bytes]; grad_P [out, device, n doubles], may
  *   alias grad_sigma.  Returns PIVOT_ERR_NULL / _BAD_N / _BAD_MODE / _BAD_FLOOR / _CUDA. */
 int pivot_iv_backward(const double* grad_sigma, const double* vega, const uint8_t* status, double vega_floor,

@@ -7,6 +7,7 @@ There is no CPU fallback: calling any entry point without the built library or w
 from .binding import (  # noqa: F401
     GATE_ATTENUATE,
     GATE_MASK,
+    GATE_STRICT,
     PivotError,
     Pipeline,
     library_path,
@@ -26,5 +27,5 @@ __all__ = [
     "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_backward_inputs", "pivot_iv_black_price",
     "Pipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
-    "GATE_ATTENUATE", "EXPORTS",
+    "GATE_ATTENUATE", "GATE_STRICT", "EXPORTS",
 ]

@@ -12,6 +12,7 @@ _SO = os.path.join(HERE, "libpivot_iv.so")
 
 GATE_MASK = 0
 GATE_ATTENUATE = 1
+GATE_STRICT = 2
 
 # every symbol include/pivot_iv.h declares
 EXPORTS = (

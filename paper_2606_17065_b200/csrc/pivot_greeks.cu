@@ -90,14 +90,22 @@ backward_inputs_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, con
     const uint8_t st = status[i];
     // the gated common factor: exactly pivot_iv_backward's grad_P
     double c;
+    bool strict_off = false;
     if (MODE == PIVOT_GATE_MASK) {
       c = ((st == PIVOT_ST_OK) && (fabs(V) > floor_)) ? __ddiv_rn(g, V) : 0.0;
+    } else if (MODE == PIVOT_GATE_STRICT) {
+      const bool on = (st == PIVOT_ST_OK) && (fabs(V) > floor_);
+      c = on ? __ddiv_rn(g, V) : ((g == 0.0) ? 0.0 : canonical_nan());
+      strict_off = !on;
     } else {
       const double den = __dadd_rn(__dmul_rn(V, V), floor2);
       c = ((st == PIVOT_ST_OK) && (den > 0.0)) ? __ddiv_rn(__dmul_rn(g, V), den) : 0.0;
     }
     double dS = 0.0, dK = 0.0, dT = 0.0, dR = 0.0, dQ = 0.0;
-    if (st == PIVOT_ST_OK && c != 0.0) {
+    if (strict_off) {
+      dS = dK = dT = c;                 // 0 or NaN with grad_P
+      dR = dQ = c;
+    } else if (st == PIVOT_ST_OK && c != 0.0) {
       const double S = __ldcs(in.S_or_F + i), K = __ldcs(in.K + i), tau = __ldcs(in.tau + i), sg = __ldcs(sigma + i);
       const double th = (__ldcs(in.flag + i) > 0.0) ? 1.0 : -1.0;
       const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
@@ -164,7 +172,7 @@ int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, con
                              pivot_iv_stream stream) {
   if (!in) return PIVOT_ERR_NULL;
   if (n < 0) return PIVOT_ERR_BAD_N;
-  if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE) return PIVOT_ERR_BAD_MODE;
+  if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE && mode != PIVOT_GATE_STRICT) return PIVOT_ERR_BAD_MODE;
   if (!(vega_floor >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
   if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
   if (n == 0) return PIVOT_OK;
@@ -178,9 +186,13 @@ int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, con
   backward_inputs_kernel<B, M><<<blocks, kEwThreads, 0, st>>>(*in, sigma, vega, status, grad_sigma, vega_floor, n,    \
                                                               grad_P, grad_S_or_F, grad_K, grad_tau, grad_r, grad_q)
   if (bsm) {
-    if (mode == PIVOT_GATE_MASK) PIVOT_LAUNCH_BI(true, PIVOT_GATE_MASK); else PIVOT_LAUNCH_BI(true, PIVOT_GATE_ATTENUATE);
+    if (mode == PIVOT_GATE_MASK) PIVOT_LAUNCH_BI(true, PIVOT_GATE_MASK);
+    else if (mode == PIVOT_GATE_STRICT) PIVOT_LAUNCH_BI(true, PIVOT_GATE_STRICT);
+    else PIVOT_LAUNCH_BI(true, PIVOT_GATE_ATTENUATE);
   } else {
-    if (mode == PIVOT_GATE_MASK) PIVOT_LAUNCH_BI(false, PIVOT_GATE_MASK); else PIVOT_LAUNCH_BI(false, PIVOT_GATE_ATTENUATE);
+    if (mode == PIVOT_GATE_MASK) PIVOT_LAUNCH_BI(false, PIVOT_GATE_MASK);
+    else if (mode == PIVOT_GATE_STRICT) PIVOT_LAUNCH_BI(false, PIVOT_GATE_STRICT);
+    else PIVOT_LAUNCH_BI(false, PIVOT_GATE_ATTENUATE);
   }
 #undef PIVOT_LAUNCH_BI
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;

@@ -247,6 +247,9 @@ __device__ __forceinline__ double backward_row(double gs, double V, uint8_t st, 
   if (MODE == PIVOT_GATE_MASK) {
     const bool on = (st == PIVOT_ST_OK) && (fabs(V) > floor_);
     return on ? __ddiv_rn(gs, V) : 0.0;
+  } else if (MODE == PIVOT_GATE_STRICT) {
+    const bool on = (st == PIVOT_ST_OK) && (fabs(V) > floor_);
+    return on ? __ddiv_rn(gs, V) : ((gs == 0.0) ? 0.0 : canonical_nan());
   } else {
     const double den = __dadd_rn(__dmul_rn(V, V), floor2);
     const bool on = (st == PIVOT_ST_OK) && (den > 0.0);
@@ -396,13 +399,14 @@ int launch_backward_t(const double* gs, const double* vega, const uint8_t* statu
 int backward_impl(const double* gs, const double* vega, const uint8_t* status, double floor_, int mode, int64_t n,
                   double* gP, cudaStream_t st) {
   if (n < 0) return PIVOT_ERR_BAD_N;
-  if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE) return PIVOT_ERR_BAD_MODE;
+  if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE && mode != PIVOT_GATE_STRICT) return PIVOT_ERR_BAD_MODE;
   if (!(floor_ >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
   if (n == 0) return PIVOT_OK;
   if (!gs || !vega || !status || !gP) return PIVOT_ERR_NULL;
   if (n > ((int64_t)1 << 38)) return PIVOT_ERR_BAD_N;
-  return mode == PIVOT_GATE_MASK ? launch_backward_t<PIVOT_GATE_MASK>(gs, vega, status, floor_, n, gP, st)
-                                 : launch_backward_t<PIVOT_GATE_ATTENUATE>(gs, vega, status, floor_, n, gP, st);
+  if (mode == PIVOT_GATE_MASK) return launch_backward_t<PIVOT_GATE_MASK>(gs, vega, status, floor_, n, gP, st);
+  if (mode == PIVOT_GATE_STRICT) return launch_backward_t<PIVOT_GATE_STRICT>(gs, vega, status, floor_, n, gP, st);
+  return launch_backward_t<PIVOT_GATE_ATTENUATE>(gs, vega, status, floor_, n, gP, st);
 }
 
 }  // namespace
@@ -441,7 +445,7 @@ const char* pivot_iv_strerror(int code) {
     case PIVOT_OK: return "ok";
     case PIVOT_ERR_NULL: return "a required pointer is NULL";
     case PIVOT_ERR_BAD_N: return "n is negative or too large";
-    case PIVOT_ERR_BAD_MODE: return "mode must be PIVOT_GATE_MASK (0) or PIVOT_GATE_ATTENUATE (1)";
+    case PIVOT_ERR_BAD_MODE: return "mode must be PIVOT_GATE_MASK (0), PIVOT_GATE_ATTENUATE (1) or PIVOT_GATE_STRICT (2)";
     case PIVOT_ERR_BAD_FLOOR: return "vega_floor must be a non-negative number";
     case PIVOT_ERR_MIXED_RQ: return "r and q must both be NULL (Black-76) or both non-NULL (BSM)";
     case PIVOT_ERR_CUDA: return "CUDA runtime error";
@@ -483,7 +487,7 @@ int pipeline_run(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* 
   if (n < 0) return PIVOT_ERR_BAD_N;
   if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
   if (bwd) {
-    if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE) return PIVOT_ERR_BAD_MODE;
+    if (mode != PIVOT_GATE_MASK && mode != PIVOT_GATE_ATTENUATE && mode != PIVOT_GATE_STRICT) return PIVOT_ERR_BAD_MODE;
     if (!(floor_ >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
   }
   if (n == 0) return PIVOT_OK;

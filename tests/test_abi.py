@@ -50,7 +50,12 @@ def test_argument_validation_without_gpu(lib):
     assert lib.pivot_iv_forward(ctypes.byref(inp), i64(-1), 8, 8, 8, None) == -2     # n < 0
     assert lib.pivot_iv_forward(ctypes.byref(inp), i64(0), None, None, None, None) == 0   # n == 0 no-op
     assert lib.pivot_iv_forward(ctypes.byref(inp), i64(4), None, 8, 8, None) == -1
-    assert lib.pivot_iv_backward(8, 8, 8, ctypes.c_double(1e-8), 2, i64(4), 8, None) == -3
+    assert lib.pivot_iv_backward(8, 8, 8, ctypes.c_double(1e-8), 3, i64(4), 8, None) == -3    # modes are 0, 1, 2
+    assert lib.pivot_iv_backward(8, 8, 8, ctypes.c_double(1e-8), -1, i64(4), 8, None) == -3
+    assert lib.pivot_iv_backward_inputs(ctypes.byref(inp), 8, 8, 8, 8, ctypes.c_double(1e-8), 7, i64(4), 8, 8, 8, 8, None, None, None) == -3
+    assert lib.pivot_iv_backward_inputs(ctypes.byref(inp), 8, 8, 8, 8, ctypes.c_double(1e-8), 0, i64(4), 8, None, 8, 8, None, None, None) == -1
+    assert lib.pivot_iv_black_price(ctypes.byref(inp), None, i64(4), 8, None, None) == -1
+    assert lib.pivot_iv_black_price(ctypes.byref(inp), 8, i64(0), 8, None, None) == 0
     assert lib.pivot_iv_backward(8, 8, 8, ctypes.c_double(-1.0), 0, i64(4), 8, None) == -4
     assert lib.pivot_iv_backward(8, 8, 8, ctypes.c_double(float("nan")), 0, i64(4), 8, None) == -4
     assert lib.pivot_iv_backward(None, 8, 8, ctypes.c_double(0.0), 0, i64(4), 8, None) == -1

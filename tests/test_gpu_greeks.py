@@ -111,3 +111,31 @@ def test_backward_inputs_matches_oracle(mode, bsm):
         bound = tolrow[on] * np.maximum(np.abs(want[on]), np.abs(gPh[on]) * scales[j][on])
         assert np.all(err <= bound + 1e-300), (j, float(np.max(err / (bound + 1e-300))))
     assert (~off).sum() > 0.5 * n
+
+
+def test_strict_gate_mode_matches_oracle():
+    """on the gate the exact gradient, off the gate +0 iff the upstream cotangent is
+    0 else NaN -- in pivot_iv_backward and in every component of pivot_iv_backward_inputs, bit for bit vs the oracle."""
+    cfg = wl.config3(1 << 18, seed=41)
+    d, c = to_device(cfg), to_numpy(cfg)
+    n = c["K"].size
+    sig, vega, st = pv.pivot_iv_forward(*[d[k] for k in KEYS])
+    gs = torch.randn(n, dtype=torch.float64, device="cuda", generator=torch.Generator(device="cuda").manual_seed(6))
+    gs[::3] = 0.0
+    gs[1::97] = float("nan")
+    floor = 1e-14
+    gP = pv.pivot_iv_backward(gs, vega, st, floor, pv.GATE_STRICT).cpu().numpy()
+    vega_h, st_h, gs_h = vega.cpu().numpy(), st.cpu().numpy(), gs.cpu().numpy()
+    ref = po.backward(gs_h, vega_h, st_h, floor, 2)
+    assert np.array_equal(np.isnan(gP), np.isnan(ref))
+    fin = ~np.isnan(ref)
+    assert np.array_equal(gP[fin].view(np.uint64), ref[fin].view(np.uint64))
+    off = ~((st_h == 0) & (np.abs(vega_h) > floor))
+    assert off.sum() > 1000 and np.isnan(gP[off & (gs_h != 0)]).all() and np.all(gP[off & (gs_h == 0)] == 0)
+    outs = pv.pivot_iv_backward_inputs(d["SorF"], d["K"], d["tau"], d["flag"], sig, vega, st, gs, floor, pv.GATE_STRICT)
+    assert np.array_equal(outs[0].cpu().numpy().view(np.uint64)[fin], ref.view(np.uint64)[fin])
+    for j in (1, 2, 3):
+        g = outs[j].cpu().numpy()
+        assert np.isnan(g[off & (gs_h != 0)]).all() and np.all(g[off & (gs_h == 0)] == 0)
+        on = ~off & np.isfinite(gs_h)
+        assert np.isfinite(g[on]).all()

@@ -159,7 +159,7 @@ def test_bsm_bad_rates_and_mixed_rq_error():
     with pytest.raises(pv.PivotError):
         pv.pivot_iv_backward(s, v, st, -1.0, 0)
     with pytest.raises(pv.PivotError):
-        pv.pivot_iv_backward(s, v, st, 1e-8, 2)
+        pv.pivot_iv_backward(s, v, st, 1e-8, 3)
 
 
 def test_full_size_headline_sampled():
