@@ -368,8 +368,14 @@ inline void householder_terms(int kind, T x, T s, T beta, T bbar_beta, T* nu_, T
     h3 = B3 + gp * (T(2) * gp + T(3) * B2);
   } else {
     const T v = exp(ln_v<T>(h, t));
-    const T b = (t + h > T(10)) ? norm_black<T>(x, s) : v * W_ratio<T>(h, t);
-    nu = (beta - b) / v;
+    if (bbar_beta < beta) {
+      // beta > b_max/2: beta - b = (b_max - b) - (b_max - beta), both terms in their complementary form (O4, O2);
+      // b - beta itself would lose eps * b_max / (b_max - beta) as beta approaches b_max
+      nu = Wbar_ratio<T>(h, t) - bbar_beta / v;
+    } else {
+      const T b = (t + h > T(10)) ? norm_black<T>(x, s) : v * W_ratio<T>(h, t);
+      nu = (beta - b) / v;
+    }
     h2 = B2;
     h3 = B3;
   }
@@ -447,12 +453,19 @@ inline RowResult<T> lbr_row(T SorF, T Kk, T tau, const T* r, const T* q, T P, T 
   const T U = (flag > T(0)) ? F : Kk;
   if (B < iota) { out.status = ST_BELOW_INTRINSIC; return out; }
   if (B >= U) { out.status = ST_ABOVE_MAX; return out; }
-  const T tv = B - iota;
+  // Time value (reading 18).  Out of the money (iota == 0) it is B itself.  In the money:
+  //   max(F,K) <= 2 min(F,K): iota = F - K is exact (Sterbenz) and so is B - iota: the textbook form;
+  //   max(F,K) >  2 min(F,K): iota carries half an ulp of max(F,K), which is eps e^{|x|/2} / beta relative to the time
+  //     value (1e-11 at |x| = 12); but U - iota = min(F,K) holds exactly and U - B is exact (B >= iota > U/2, Sterbenz),
+  //     so tv = min(F,K) - (U - B) has a single rounding at the scale of min(F,K), and beta + (b_max - beta) = b_max
+  //     holds to rounding.  Pinned against the __float128 bisection by
+  //     test_lbr_in_the_money_large_moneyness_against_truth.  A tv that comes out <= 0 is AT_INTRINSIC.
+  const T lo = (F < Kk) ? F : Kk, hi = (F < Kk) ? Kk : F;
+  const T tv = (iota > T(0) && hi > T(2) * lo) ? lo - (U - B) : B - iota;
   const T beta = tv / rootFK;
   out.beta = beta;
   if (beta < T(DBL_MIN)) { out.status = ST_AT_INTRINSIC; out.sigma = T(0); return out; }
   // O3: OTM call, x = -|ln(F/K)| (log1p of the exact difference keeps |x| accurate near the money)
-  const T lo = (F < Kk) ? F : Kk, hi = (F < Kk) ? Kk : F;
   const T x = -log1p((hi - lo) / lo);
   const T bmax = lo / rootFK;              // e^{x/2}
   const T bbar_beta = (U - B) / rootFK;    // b_max - beta

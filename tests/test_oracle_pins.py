@@ -588,3 +588,25 @@ def test_input_gradient_gate_follows_grad_P():
         for j in range(5):
             assert np.array_equal(gin[j][off].view(np.uint64), np.zeros(off.sum()).view(np.uint64))
             assert np.allclose(gin[j][~off], -gP[~off] * greeks[j][~off], rtol=1e-14, atol=0)
+
+
+def test_lbr_in_the_money_large_moneyness_against_truth():
+    """In-the-money rows at |x| up to 12: the time value must not inherit the rounding of F - K (reading 18).
+    With tv = B - fl(F - K) the oracle sat 1e-11 away from the __float128 bisection of the literal price here."""
+    rng = np.random.default_rng(321)
+    n = 600
+    x = rng.choice([-1.0, 1.0], n) * rng.uniform(3.0, 12.0, n)
+    F = np.exp(rng.uniform(np.log(0.5), np.log(5e3), n)); K = F * np.exp(-x)
+    T = np.exp(rng.uniform(np.log(0.05), np.log(20), n))
+    s = rng.uniform(0.5, 1.6, n) * np.sqrt(2 * np.abs(x))
+    flag = np.where(K >= F, -1.0, 1.0)   # in the money
+    P = po.black_price(F, K, T, s / np.sqrt(T), flag, prec=1)
+    sg, vega, st = po.forward(F, K, T, P, flag)
+    ok = st == 0
+    assert ok.sum() > 500
+    tr = po.truth_iv(F[ok], K[ok], T[ok], P[ok], flag[ok])
+    # what is left is the rounding of the quoted price itself: eps * P / (time value) relative to the time value,
+    # times the elasticity of sigma to the time value (<= ~1 here)
+    tvq = P[ok] - np.maximum(np.where(flag[ok] > 0, F[ok] - K[ok], K[ok] - F[ok]), 0)
+    rel = np.abs(sg[ok] / tr - 1)
+    assert np.all(rel <= 2e-13 + 4 * EPS * np.minimum(F, K)[ok] / tvq), float(rel.max())
