@@ -317,11 +317,33 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   o.v0 = x;
   const double sc = sqrt_nr1(2.0 * a);        // inflection point of b(x, .)
   const double vc = kPhi0 * bmax;             // b'(x, s_c) = phi0 e^{-|x|/2}
-  // at s_c: |h| = t, so z1 = 0, z2 = sqrt(|x|):  W_c = c (1 - erfcx(sqrt|x|))
-  const double Wc = (a > 0.0) ? kSqrtPiOver2 * (1.0 - erfcx_one(sc * kInvSqrt2)) : 0.0;
+  // at s_c: |h| = t = s_c/2, so z1 = 0, z2 = sqrt(|x|):  W_c = c (1 - erfcx(sqrt|x|)), and the tangent at the inflection
+  // point hits 0 at s_l = s_c - W_c.  For small s_c that difference cancels (s_l ~ 0.63 s_c^2), so there s_l comes from
+  // the small-t series of W itself:  W_c = s_c (w1 + t^2 w3/6 + t^4 w5/120 + ...), w1 = 1 - t w0  =>
+  //   s_l = s_c (t w0 - t^2 w3/6 - t^4 w5/120 - t^6 w7/5040),  w(.) at h = -t, w0 = c erfcx(t/sqrt2)
+  const double tc = 0.5 * sc;
+  const bool small_c = tc < kSmallT;
+  const double ec = erfcx_one(small_c ? tc * kInvSqrt2 : sc * kInvSqrt2);
+  double Wc, sl;
+  if (small_c) {
+    const double w0 = kSqrtPiOver2 * ec;
+    const double w1 = fma(-tc, w0, 1.0);
+    const double w2 = fma(-tc, w1, w0);
+    const double w3 = fma(-tc, w2, 2.0 * w1);
+    const double w4 = fma(-tc, w3, 3.0 * w2);
+    const double w5 = fma(-tc, w4, 4.0 * w3);
+    const double w6 = fma(-tc, w5, 5.0 * w4);
+    const double w7 = fma(-tc, w6, 6.0 * w5);
+    const double t2 = tc * tc;
+    const double tail = t2 * fma(t2, fma(t2, w7 * kSeriesC[2], w5 * kSeriesC[1]), w3 * kSeriesC[0]);
+    sl = sc * fma(tc, w0, -tail);
+    Wc = sc - sl;
+  } else {
+    Wc = kSqrtPiOver2 * (1.0 - ec);
+    sl = sc - Wc;
+  }
   const double bc = vc * Wc;
-  const double sl = sc - Wc;                  // tangent at the inflection point hits 0 ...
-  const double su = sc + (kSqrt2Pi - Wc);     // ... and b_max
+  const double su = sc + (kSqrt2Pi - Wc);     // ... and the tangent hits b_max at s_u
   const bool lower = beta < bc;
   o.v2 = beta; o.v3 = bbar; o.v4 = 0.0;
   if (lower && !(sl > 0.0)) {  // rounding guard, |x| below ~1e-30: linear seed
@@ -347,7 +369,7 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   const double H = xr - xl, rH = rcp_nr1(H);
   const double r = rc_control(lower ? 1 : 0, H, rH, yl, yr, dl, dr, 0.0);
   const double s = rc_eval((beta - xl) * rH, (xr - beta) * rH, H, yl, yr, dl, dr, r);
-  o.v1 = (s > 0.0 && is_fin(s)) ? s : sn;
+  o.v1 = (s > 0.0 && is_fin(s)) ? s : sc;   // a failed interpolant falls back to the inflection point
   return o;
 }
 
@@ -530,7 +552,10 @@ __device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau
   const bool call = flag > 0.0;
   const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
   const double U = call ? F : K;
-  const double tv = __dsub_rn(B, iota);
+  const double hi = fmax(F, K);
+  // time value (reading 18): B - iota where iota = F - K is exact (hi <= 2 lo, or out of the money), else
+  // lo - (U - B), which does not inherit the half-ulp-of-hi rounding of iota (U - iota = lo exactly, U - B exact)
+  const double tv = (iota > 0.0 && hi > __dmul_rn(2.0, lo)) ? __dsub_rn(lo, __dsub_rn(U, B)) : __dsub_rn(B, iota);
   int st = 0;
   if (bad) st = 3;
   else if (B < iota) st = 1;
@@ -560,7 +585,8 @@ __device__ __forceinline__ Norm lbr_normalise(double F, double K, double B, doub
   const double lo = fmin(F, K), hi = fmax(F, K);
   const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
   const double U = call ? F : K;
-  const double tv = __dsub_rn(B, iota), ub = __dsub_rn(U, B), d = __dsub_rn(hi, lo);
+  const double ub = __dsub_rn(U, B), d = __dsub_rn(hi, lo);
+  const double tv = (iota > 0.0 && hi > __dmul_rn(2.0, lo)) ? __dsub_rn(lo, ub) : __dsub_rn(B, iota);  // as in lbr_prelude
   const double r = rcp_nr2(rootFK);
   double q = lo * r;
   n.bmax = fma(fma(-rootFK, q, lo), r, q);
