@@ -253,3 +253,32 @@ def test_degenerate_tile_compositions():
             assert st["ok"] == 1
         if name in ("upper_tail_only", "near_atm_mid_prices"):
             assert st["ok"] == n, name
+
+
+@pytest.mark.parametrize("case", ["wide", "nearatm", "hugevol", "tinyvol"])
+def test_wide_domain_fuzz(case):
+    """Beyond the configs' ranges: |x| up to 12 with F over nine decades, |x| down to one ulp, total vol up to 40 and
+    |h| up to 37.  (A first version of the seed-grade arithmetic lost s_l to cancellation at |x| ~ 1e-16, and the
+    textbook in-the-money time value B - (F - K) sat 1e-11 off the __float128 bisection at |x| = 12: DESIGN.md reading 18.)"""
+    rng = np.random.default_rng({"wide": 1, "nearatm": 2, "hugevol": 3, "tinyvol": 4}[case])
+    n = 1 << 19
+
+    def lu(lo, hi):
+        return np.exp(rng.uniform(np.log(lo), np.log(hi), n))
+    if case == "wide":
+        F = lu(1e-3, 1e6); x = rng.uniform(-12, 12, n); T = lu(1e-5, 50); s = lu(1e-5, 12)
+    elif case == "nearatm":
+        F = lu(1, 1e4); x = rng.choice([-1, 1], n) * lu(1e-16, 1e-2); T = lu(1e-4, 5); s = lu(1e-9, 3)
+    elif case == "hugevol":
+        F = lu(1, 1e4); x = rng.uniform(-3, 3, n); T = lu(0.01, 30); s = lu(2, 40)
+    else:
+        F = lu(1, 1e4); x = rng.uniform(-0.5, 0.5, n); T = lu(1e-4, 2); s = np.abs(x) / rng.uniform(0.5, 37.5, n) + 1e-12
+    K = F * np.exp(-x)
+    flag = np.where(rng.random(n) < 0.5, 1.0, -1.0)
+    P = po.black_price(F, K, T, s / np.sqrt(T), flag, prec=1) * (1 + 1e-9 * rng.standard_normal(n))
+    cols = [np.ascontiguousarray(a) for a in (F, K, T, P, flag)]
+    o = po.forward(*cols)
+    g = tuple(t.cpu().numpy() for t in pv.pivot_iv_forward(*[torch.from_numpy(a).cuda() for a in cols]))
+    c = dict(zip(KEYS, cols)); c["r"] = None; c["q"] = None
+    st = compare_forward(g, o, c)
+    assert st["ok"] > 0.3 * n
