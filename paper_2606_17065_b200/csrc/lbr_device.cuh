@@ -519,7 +519,7 @@ __device__ __forceinline__ NormSolve lbr_solve(double qrel, double beta, double 
 //   beta = RN(tv / rootFK) < DBL_MIN   <=>   tv * 2^1022 < rootFK     (exact: the scaling is exact, and for doubles
 //   bmax = RN(lo / rootFK) >= 2^-500   <=>   lo * 2^500 >= rootFK      a < b implies a <= b - ulp(b) < b (1 - 2^-53))
 // so the status byte equals the one obtained from the correctly rounded quotients, bit for bit, and rows that leave
-// here (64.6 % of config 1/4) cost no division (a zero numerator would even take the divide's slow path).
+// here (57.8 % of config 1/4) cost no division (a zero numerator would even take the divide's slow path).
 // The status decision uses only correctly rounded IEEE operations issued through intrinsics, so it cannot be
 // contracted into FMAs and is bit-reproducible against any IEEE-754 implementation of the same sequence.
 struct Prelude {
