@@ -324,6 +324,11 @@ def main():
         dt = time.perf_counter() - t0
         cpu = {"value": m / dt, "unit": "rows/s", "cores": po.max_threads(), "kind": "oracle",
                "sample": f"first {m} rows of the same workload, forward + MASK backward, one pass"}
+        # single-thread figure, to sit beside the paper's 1.60e5 IV/s scalar Python-loop baseline
+        m1 = min(m, 1 << 20)
+        t1 = time.perf_counter()
+        po.forward(c["SorF"][:m1], c["K"][:m1], c["tau"][:m1], c["P"][:m1], c["flag"][:m1], nthreads=1)
+        cpu["single_thread_forward_iv_per_s"] = m1 / (time.perf_counter() - t1)
         gs_, gv_, gst_ = (t_[:m].cpu().numpy() for t_ in out)
         ok = (ost == 0) & (gst_ == 0)
         err["status_mismatches"] = int((ost != gst_).sum())
