@@ -299,15 +299,16 @@ __device__ __forceinline__ double rc_control(int side, double H, double rH, doub
 //   lbr_seed_tail0 / lbr_seed_tail3 : the lower / upper tail maps f_low, f_up, their rational-cubic interpolant in beta
 //                   and its inversion.
 // Result of the pass: x = -ln(1+qrel) <= 0, the seed s0, the objective kind and its two parameters
-//        KIND_LOWER : p1 = ln beta,          p2 = b_max      g = 1/ln b - 1/ln beta
+//        KIND_LOWER : p1 = ln beta,          p2 unused       g = 1/ln b - 1/ln beta
 //        KIND_LINEAR: p1 = beta,             p2 = bbar       g = b - beta
-//        KIND_UPPER : p1 = ln(b_max - beta), p2 = b_max      g = ln((b_max - beta)/(b_max - b))
+//        KIND_UPPER : p1 = ln(b_max - beta), p2 unused       g = ln((b_max - beta)/(b_max - b))
 // Everything here only has to deliver a seed good to ~1e-3 (Householder(3) is fourth order), so reciprocals and
 // square roots carry ~1e-12 and the tail maps use fp32-grade exp / log / erfcx / Phi^-1 on MUFU.
 // ---------------------------------------------------------------------------------------------------------------
 struct SeedHead {
-  int zone;        // 0, 3: tail pending (v = x, s_n, b_n, beta, b_max | bbar);  1, 2: finished (v = x, s0, beta, bbar)
-  double v0, v1, v2, v3, v4;
+  int zone;        // 0: tail pending, v = (x, s_n, b_n, beta);  3: tail pending, v = (x, s_n, b_n, bbar);
+                   // 1, 2: finished, v = (x, s0, beta, bbar)
+  double v0, v1, v2, v3;
 };
 
 __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, double bbar, double bmax) {
@@ -345,7 +346,7 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   const double bc = vc * Wc;
   const double su = sc + (kSqrt2Pi - Wc);     // ... and the tangent hits b_max at s_u
   const bool lower = beta < bc;
-  o.v2 = beta; o.v3 = bbar; o.v4 = 0.0;
+  o.v2 = beta; o.v3 = bbar;
   if (lower && !(sl > 0.0)) {  // rounding guard, |x| below ~1e-30: linear seed
     o.zone = 1;
     o.v1 = sc * beta * rcp_nr1(bc);
@@ -357,7 +358,7 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   const double bn = w.have_W ? w.Wd * vn : fma(-w.Wd, vn, bmax);
   if (lower ? (beta < bn) : (beta > bn)) {   // a tail: hand the node over
     o.zone = lower ? 0 : 3;
-    o.v1 = sn; o.v2 = bn; o.v3 = beta; o.v4 = lower ? bmax : bbar;
+    o.v1 = sn; o.v2 = bn; o.v3 = lower ? beta : bbar;
     return o;
   }
   // zones 1 and 2: s(beta) between the node and the inflection point, s'' = 0 at the inflection point
@@ -379,7 +380,7 @@ struct Seed {
 };
 
 // zone 0: f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l]
-__device__ __forceinline__ Seed lbr_seed_tail0(double x, double sn, double bn, double beta, double bmax) {
+__device__ __forceinline__ Seed lbr_seed_tail0(double x, double sn, double bn, double beta) {
   const double a = -x;
   const double rs = rcp_nr1(sn);
   const double z = a * rs * kInvSqrt3;
@@ -404,13 +405,14 @@ __device__ __forceinline__ Seed lbr_seed_tail0(double x, double sn, double bn, d
   if (!(s > 0.0) || !is_fin(s)) s = sn;
   Seed o;
   o.x = x; o.s = s; o.zone = 0;
-  o.kind = KIND_LOWER; o.p1 = log_fast(beta); o.p2 = bmax;
+  o.kind = KIND_LOWER; o.p1 = log_fast(beta); o.p2 = 0.0;   // b_max = e^{x/2} is rebuilt by lbr_refine if ever needed
   return o;
 }
 
 // zone 3: f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max]
-__device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bn, double beta, double bbar) {
-  const double bmax = beta + bbar;
+__device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bn, double bbar) {
+  const double bmax = exp_fast(0.5 * x);   // e^{x/2} (the handover carries four words: beta = b_max - bbar)
+  const double beta = bmax - bbar;
   const double rs = rcp_nr1(sn);
   const double h = x * rs;
   const double hu2 = h * h;
@@ -429,7 +431,7 @@ __device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bn, d
   Seed o;
   o.x = x; o.s = s; o.zone = 3;
   if (bbar < 0.5 * bmax) {
-    o.kind = KIND_UPPER; o.p1 = log_fast(bbar); o.p2 = bmax;
+    o.kind = KIND_UPPER; o.p1 = log_fast(bbar); o.p2 = 0.0;
   } else {
     o.kind = KIND_LINEAR; o.p1 = beta; o.p2 = bbar;
   }
@@ -439,8 +441,8 @@ __device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bn, d
 // one-call form (row-per-thread kernel)
 __device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, double bmax) {
   const SeedHead hd = lbr_seed_head(qrel, beta, bbar, bmax);
-  if (hd.zone == 0) return lbr_seed_tail0(hd.v0, hd.v1, hd.v2, hd.v3, hd.v4);
-  if (hd.zone == 3) return lbr_seed_tail3(hd.v0, hd.v1, hd.v2, hd.v3, hd.v4);
+  if (hd.zone == 0) return lbr_seed_tail0(hd.v0, hd.v1, hd.v2, hd.v3);
+  if (hd.zone == 3) return lbr_seed_tail3(hd.v0, hd.v1, hd.v2, hd.v3);
   Seed o;
   o.x = hd.v0; o.s = hd.v1; o.p1 = hd.v2; o.p2 = hd.v3; o.kind = KIND_LINEAR; o.zone = hd.zone;
   return o;
@@ -476,8 +478,8 @@ __device__ __forceinline__ NormSolve lbr_refine(double x, double s, double p1, d
       h3 = B3;
     } else {
       const bool want_W = kind == KIND_LOWER;
-      double R = w.Wd;  // the ratio the objective wants: W (lower tail) or Wbar (upper tail); p2 = b_max
-      if (want_W != w.have_W) R = fma(p2 * kSqrt2Pi, exp_fast(w.E), -w.Wd);
+      double R = w.Wd;  // the ratio the objective wants: W (lower tail) or Wbar (upper tail)
+      if (want_W != w.have_W) R = fma(exp_fast(0.5 * x) * kSqrt2Pi, exp_fast(w.E), -w.Wd);   // rare: b_max = e^{x/2} rebuilt here
       const double L = kLnPhi0 - w.E + log_fast(R);  // ln b (lower) or ln(b_max - b) (upper)
       if (want_W) {
         // g = 1/ln b - 1/ln beta  (p1 = ln beta)

@@ -58,7 +58,7 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __re
 // config 1/4 rows leave at the validity check; here the solver's warps are full.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
-// RPT rows per thread: 4 (1024-row tiles, 63.5 KB of shared memory, 3 CTAs per SM) for large n; 1 (256-row tiles) for
+// RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers) for large n; 1 (256-row tiles) for
 // small n, so that a launch of 65,536 rows still spreads over every SM.
 
 template <int RPT>
@@ -70,7 +70,6 @@ struct TileSmem {
   double q1[kTileRows];
   double q2[kTileRows];
   double q3[kTileRows];
-  double q4[kTileRows];       // fifth word of a pending tail row between B1a and B1b
   uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call, bit 14 = zone 3 row with UPPER objective
   uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, finished middle-zone rows from the back
   uint16_t permU[kTileRows];  // ... and zone 3 rows
@@ -80,7 +79,7 @@ struct TileSmem {
 };
 
 template <bool BSM, bool ZONES, int RPT>
-__global__ void __launch_bounds__(kTileThreads, 3)
+__global__ void __launch_bounds__(kTileThreads, BSM ? 3 : 4)
 forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                     uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -167,7 +166,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     if (j < cnt) {
       const Norm nm = lbr_normalise(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], (sm.pos[j] & 0x8000) != 0);
       const SeedHead hd = lbr_seed_head(nm.qrel, nm.beta, nm.bbar, nm.bmax);
-      sm.q0[j] = hd.v0; sm.q1[j] = hd.v1; sm.q2[j] = hd.v2; sm.q3[j] = hd.v3; sm.q4[j] = hd.v4;
+      sm.q0[j] = hd.v0; sm.q1[j] = hd.v1; sm.q2[j] = hd.v2; sm.q3[j] = hd.v3;
       cls = (hd.zone == 0) ? 0 : ((hd.zone == 3) ? 2 : 1);
       if (ZONES) zone[base + (sm.pos[j] & 0x3fff)] = (int8_t)hd.zone;
     }
@@ -197,10 +196,10 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     int j;
     if (k < n0) {
       j = sm.perm[k];
-      sd = lbr_seed_tail0(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], sm.q4[j]);
+      sd = lbr_seed_tail0(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
     } else {
       j = sm.permU[k - n0];
-      sd = lbr_seed_tail3(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], sm.q4[j]);
+      sd = lbr_seed_tail3(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
       if (sd.kind == KIND_UPPER) sm.pos[j] |= 0x4000;
     }
     sm.q1[j] = sd.s; sm.q2[j] = sd.p1; sm.q3[j] = sd.p2;
