@@ -215,3 +215,25 @@ def backward_inputs(gsigma, vega, status, vega_floor, mode, SorF, K, tau, sigma,
                                  C.c_int(mode), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(sigma), _p(flag),
                                  *[_p(o) for o in outs])
     return tuple(outs)
+
+
+def loss_price(SorF, K, tau, Pstar, flag, sigma_hat, r=None, q=None):
+    """eq.(11) as raw sums: (sum (P_model - P*)^2, sum |P*|, rows used)."""
+    SorF, K, tau, Pstar, flag, sigma_hat = map(_d, (SorF, K, tau, Pstar, flag, sigma_hat))
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    out = np.empty(3)
+    lib().oracle_loss_price(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(Pstar), _p(flag),
+                            _p(sigma_hat), _p(out))
+    return out
+
+
+def loss_roundtrip(SorF, K, tau, Pstar, flag, sigma_hat, sigma_star, vega_floor, r=None, q=None):
+    """eq.(12) as raw sums: (sum w (IV(P~) - sigma*)^2, sum w, rows used)."""
+    SorF, K, tau, Pstar, flag, sigma_hat, sigma_star = map(_d, (SorF, K, tau, Pstar, flag, sigma_hat, sigma_star))
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    out = np.empty(3)
+    lib().oracle_loss_roundtrip(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(Pstar), _p(flag),
+                                _p(sigma_hat), _p(sigma_star), C.c_double(vega_floor), _p(out))
+    return out

@@ -610,3 +610,43 @@ def test_lbr_in_the_money_large_moneyness_against_truth():
     tvq = P[ok] - np.maximum(np.where(flag[ok] > 0, F[ok] - K[ok], K[ok] - F[ok]), 0)
     rel = np.abs(sg[ok] / tr - 1)
     assert np.all(rel <= 2e-13 + 4 * EPS * np.minimum(F, K)[ok] / tvq), float(rel.max())
+
+
+# ------------------------------------------------------------------ the two objectives, eq.(11) / eq.(12)
+def test_loss_price_closed_forms():
+    """eq.(11): with P* = P_model + delta the sums are sum delta^2 and sum |P*| (numpy, independent of the oracle's loop);
+    sigma_hat = sigma_true gives exactly 0."""
+    S, K, tau, r, q, sig, flag = _bsm_rows(5000, 12)
+    pm = po.black_price(S, K, tau, sig, flag, r=r, q=q, prec=1)
+    z = po.loss_price(S, K, tau, pm, flag, sig, r=r, q=q)
+    assert z[0] <= 1e-20 * np.sum(pm ** 2) and z[2] == S.size
+    delta = np.random.default_rng(2).standard_normal(S.size) * 0.01 * pm
+    out = po.loss_price(S, K, tau, pm + delta, flag, sig, r=r, q=q)
+    assert out[0] == pytest.approx(np.sum(delta ** 2), rel=1e-9)
+    assert out[1] == pytest.approx(np.sum(np.abs(pm + delta)), rel=1e-14)
+    L = (out[0] / out[2]) / (out[1] / out[2]) ** 2
+    assert L == pytest.approx(np.mean((delta / np.mean(np.abs(pm + delta))) ** 2), rel=1e-9)
+
+
+def test_loss_roundtrip_against_direct_formula():
+    """eq.(12): on gate-on rows IV(P_model(sigma_hat)) = sigma_hat, so the sum must equal sum w(V_hat)(sigma_hat - sigma*)^2
+    computed without any inversion; gate-off rows use the sentinel P*, whose IV is sigma* itself, and contribute 0."""
+    S, K, tau, r, q, sig_star, flag = _bsm_rows(4000, 13)
+    Pstar = po.black_price(S, K, tau, sig_star, flag, r=r, q=q, prec=1)
+    sstar, _, st0 = po.forward(S, K, tau, Pstar, flag, r=r, q=q)
+    keep = (st0 == 0) & (np.abs(sstar / sig_star - 1) < 1e-6)        # rows whose market IV is recoverable
+    assert keep.sum() > 3500
+    S, K, tau, r, q, sig_star, flag, Pstar, sstar = (a[keep] for a in (S, K, tau, r, q, sig_star, flag, Pstar, sstar))
+    sig_hat = sig_star * (1 + 0.05 * np.random.default_rng(3).standard_normal(S.size))
+    vh = po.vega_eq14(S, K, tau, sig_hat, r=r, q=q)
+    floor = float(np.quantile(vh, 0.3))                 # 30 % of the rows fall off the gate
+    out = po.loss_roundtrip(S, K, tau, Pstar, flag, sig_hat, sstar, floor, r=r, q=q)
+    w = vh ** 2 / (vh ** 2 + floor ** 2)
+    on = vh > floor
+    direct = np.sum(w[on] * (sig_hat[on] - sstar[on]) ** 2)
+    assert out[2] == S.size
+    assert out[0] == pytest.approx(direct, rel=1e-9)
+    assert out[1] == pytest.approx(np.sum(w), rel=1e-13)
+    # sigma_hat = sigma*: zero
+    z = po.loss_roundtrip(S, K, tau, Pstar, flag, sstar, sstar, floor, r=r, q=q)
+    assert z[0] <= 1e-24 * S.size
