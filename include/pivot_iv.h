@@ -123,6 +123,22 @@ int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, con
                              double* grad_S_or_F, double* grad_K, double* grad_tau, double* grad_r, double* grad_q,
                              pivot_iv_stream stream);
 
+/* The two PIVOT objectives as sums, so that the caller normalises by the rows used:
+ *   eq.(11)  L_price = (out3[0]/out3[2]) / (out3[1]/out3[2])^2,  out3 += { sum (P_BS(xi, sigma_hat) - P*)^2, sum |P*|, rows used }
+ *   eq.(12)  L_rt    =  out3[0]/out3[2],                         out3 += { sum w (JaeckelIV(P~) - sigma*)^2, sum w, rows used },
+ *            w = V_hat^2/(V_hat^2 + vega_floor^2) (eq.(10)), V_hat = vega at sigma_hat, P~ = model price where |V_hat| > vega_floor,
+ *            else the sentinel market price P* (in->P); the inversion is the same fused forward kernel as pivot_iv_forward.
+ * Rows with a non-finite model price or P* are skipped by (11); rows whose inversion is not OK or whose sigma* is not finite by (12).
+ * out3 [device, 3 doubles] is ACCUMULATED into (zero it first).  sigma_hat, sigma_star [in, device, n doubles].
+ * workspace [device, pivot_iv_loss_roundtrip_workspace_bytes(n) bytes, 8-byte aligned] is scratch of the round trip
+ * (P~, V_hat, the inversion's sigma / vega / status).  Launches: 1 kernel (price loss), 3 kernels (round trip).
+ * Returns PIVOT_ERR_NULL / _BAD_N / _BAD_FLOOR / _MIXED_RQ / _BAD_ARG / _CUDA. */
+int pivot_iv_loss_price(const pivot_iv_inputs* in, const double* sigma_hat, int64_t n, double* out3,
+                        pivot_iv_stream stream);
+int64_t pivot_iv_loss_roundtrip_workspace_bytes(int64_t n);
+int pivot_iv_loss_roundtrip(const pivot_iv_inputs* in, const double* sigma_hat, const double* sigma_star, double vega_floor,
+                            int64_t n, void* workspace, double* out3, pivot_iv_stream stream);
+
 /* ---- host-buffer pipeline (the streaming label-generation setting: batches of rows, H2D included) ----
  * A pipeline owns `n_slots` device staging slots of `chunk_rows` rows each, one CUDA stream per slot and pinned
  * bounce buffers are NOT used: host arrays are copied directly (pin them for full PCIe speed).  The *_host calls split

@@ -241,7 +241,7 @@ void oracle_backward_inputs(int64_t n, const double* gsigma, const double* vega,
 //   eq.(12)  L_rt    = (1/|B|) sum_i w_tau(V_hat_i) (JaeckelIV(P~_i) - sigma*_i)^2,   w_tau(V) = V^2/(V^2 + tau^2) (eq.(10)),
 //            P~_i = model price where |V_hat_i| > tau, else the sentinel market price P*_i
 // Returned as raw sums so that the caller normalises: price: out = {sum (P_model - P*)^2, sum |P*|, rows used};
-// round trip: out = {sum w (sigma_rt - sigma*)^2, sum w, rows used}.  Rows whose model price is not finite (bad inputs)
+// round trip: out = {sum w (sigma_rt - sigma*)^2, sum w, rows used}.  Rows whose sigma_hat or model price is not finite
 // are skipped in both; rows whose round-trip inversion is not OK or whose sigma* is not finite are skipped in (12).
 void oracle_loss_price(int64_t n, const double* SorF, const double* Kk, const double* tau, const double* r, const double* q,
                        const double* Pstar, const double* flag, const double* sig_hat, double* out3) {
@@ -250,7 +250,7 @@ void oracle_loss_price(int64_t n, const double* SorF, const double* Kk, const do
     long double rr = r ? r[i] : 0, qq = q ? q[i] : 0;
     const long double pm = black_price<long double>(SorF[i], Kk[i], tau[i], (r && q) ? &rr : nullptr, (r && q) ? &qq : nullptr,
                                                     sig_hat[i], flag[i]);
-    if (!std::isfinite((double)pm) || !std::isfinite(Pstar[i])) continue;
+    if (!std::isfinite(sig_hat[i]) || !std::isfinite((double)pm) || !std::isfinite(Pstar[i])) continue;
     const long double d = pm - (long double)Pstar[i];
     s2 += d * d; s1 += fabsl((long double)Pstar[i]); cnt += 1;
   }
@@ -266,7 +266,7 @@ void oracle_loss_roundtrip(int64_t n, const double* SorF, const double* Kk, cons
     const double* pr = (r && q) ? &rr : nullptr; const double* pq = (r && q) ? &qq : nullptr;
     const double pm = black_price<double>(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i], flag[i]);
     const double vh = black_vega_eq14<double>(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i]);
-    if (!std::isfinite(pm) || !std::isfinite(vh) || !std::isfinite(sig_star[i])) continue;
+    if (!std::isfinite(sig_hat[i]) || !std::isfinite(pm) || !std::isfinite(vh) || !std::isfinite(sig_star[i])) continue;
     const double pt = (std::fabs(vh) > vega_floor) ? pm : Pstar[i];
     const RowResult<double> o = lbr_row<double>(SorF[i], Kk[i], tau[i], pr, pq, pt, flag[i]);
     if (o.status != ST_OK) continue;

@@ -17,6 +17,8 @@ from .binding import (  # noqa: F401
     pivot_iv_backward_inputs,
     pivot_iv_forward,
     pivot_iv_forward_zones,
+    pivot_iv_loss_price,
+    pivot_iv_loss_roundtrip,
     pivot_iv_probe_dfma,
     pivot_iv_strerror,
     pivot_iv_version,
@@ -25,6 +27,7 @@ from .binding import (  # noqa: F401
 
 __all__ = [
     "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_backward_inputs", "pivot_iv_black_price",
+    "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "Pipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
     "GATE_ATTENUATE", "GATE_STRICT", "EXPORTS",

@@ -133,6 +133,91 @@ backward_inputs_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, con
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The two PIVOT objectives as sums (eq.(11), eq.(12)).
+// ---------------------------------------------------------------------------------------------------------------
+// adds (a, b, c) over the CTA into out[0..2]: warp shuffles, one shared-memory hop, three fp64 atomics per CTA
+__device__ __forceinline__ void block_add3(double a, double b, double c, double* __restrict__ out) {
+  __shared__ double red[3][kEwThreads / 32];
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    a += __shfl_down_sync(0xffffffffu, a, d);
+    b += __shfl_down_sync(0xffffffffu, b, d);
+    c += __shfl_down_sync(0xffffffffu, c, d);
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) { red[0][warp] = a; red[1][warp] = b; red[2][warp] = c; }
+  __syncthreads();
+  if (warp == 0) {
+    a = (lane < kEwThreads / 32) ? red[0][lane] : 0.0;
+    b = (lane < kEwThreads / 32) ? red[1][lane] : 0.0;
+    c = (lane < kEwThreads / 32) ? red[2][lane] : 0.0;
+#pragma unroll
+    for (int d = 4; d > 0; d >>= 1) {
+      a += __shfl_down_sync(0xffffffffu, a, d);
+      b += __shfl_down_sync(0xffffffffu, b, d);
+      c += __shfl_down_sync(0xffffffffu, c, d);
+    }
+    if (lane == 0) { atomicAdd(out + 0, a); atomicAdd(out + 1, b); atomicAdd(out + 2, c); }
+  }
+}
+
+// eq.(11): out += { sum (P_model - P*)^2, sum |P*|, rows used }
+template <bool BSM>
+__global__ void __launch_bounds__(kEwThreads)
+loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int64_t n, double* __restrict__ out) {
+  double s2 = 0.0, s1 = 0.0, cnt = 0.0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+    double pm, v;
+    black_row<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(sigma_hat + i),
+                   __ldcs(in.flag + i), pm, v);
+    const double ps = __ldcs(in.P + i);
+    if (is_fin(pm) && is_fin(ps)) {
+      const double d = pm - ps;
+      s2 = fma(d, d, s2); s1 += fabs(ps); cnt += 1.0;
+    }
+  }
+  block_add3(s2, s1, cnt, out);
+}
+
+// eq.(12), step 1: model price, V_hat, and the price handed to the inversion: P~ = model price on the gate, the
+// sentinel market price P* off it
+template <bool BSM>
+__global__ void __launch_bounds__(kEwThreads)
+rt_prepare_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, double floor_, int64_t n,
+                  double* __restrict__ Ptilde, double* __restrict__ Vhat) {
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+    double pm, v;
+    black_row<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(sigma_hat + i),
+                   __ldcs(in.flag + i), pm, v);
+    Ptilde[i] = !is_fin(pm) ? canonical_nan() : ((fabs(v) > floor_) ? pm : __ldcs(in.P + i));
+    Vhat[i] = v;
+  }
+}
+
+// eq.(12), step 3: out += { sum w (sigma_rt - sigma*)^2, sum w, rows used },  w = V_hat^2 / (V_hat^2 + floor^2) (eq.(10))
+__global__ void __launch_bounds__(kEwThreads)
+rt_reduce_kernel(const double* __restrict__ sigma_rt, const uint8_t* __restrict__ status, const double* __restrict__ Vhat,
+                 const double* __restrict__ sigma_star, double floor_, int64_t n, double* __restrict__ out) {
+  double acc = 0.0, wsum = 0.0, cnt = 0.0;
+  const double f2 = floor_ * floor_;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double v = __ldcs(Vhat + i), ss = __ldcs(sigma_star + i);
+    if (status[i] == PIVOT_ST_OK && is_fin(v) && is_fin(ss)) {
+      const double v2 = v * v;
+      const double w = v2 / (v2 + f2);
+      const double d = __ldcs(sigma_rt + i) - ss;
+      acc = fma(w * d, d, acc); wsum += w; cnt += 1.0;
+    }
+  }
+  block_add3(acc, wsum, cnt, out);
+}
+
 inline int ew_blocks(int64_t n) {
   static const int sms = [] {
     int dev = 0, v = 0;
@@ -195,6 +280,47 @@ int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, con
     else PIVOT_LAUNCH_BI(false, PIVOT_GATE_ATTENUATE);
   }
 #undef PIVOT_LAUNCH_BI
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int pivot_iv_loss_price(const pivot_iv_inputs* in, const double* sigma_hat, int64_t n, double* out3,
+                        pivot_iv_stream stream) {
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (n == 0) return PIVOT_OK;
+  if (!in->S_or_F || !in->K || !in->tau || !in->flag || !in->P || !sigma_hat || !out3) return PIVOT_ERR_NULL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (in->r) loss_price_kernel<true><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma_hat, n, out3);
+  else loss_price_kernel<false><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma_hat, n, out3);
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int64_t pivot_iv_loss_roundtrip_workspace_bytes(int64_t n) { return n < 0 ? 0 : ((33 * n + 15) / 16) * 16; }
+
+int pivot_iv_loss_roundtrip(const pivot_iv_inputs* in, const double* sigma_hat, const double* sigma_star, double vega_floor,
+                            int64_t n, void* workspace, double* out3, pivot_iv_stream stream) {
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if (!(vega_floor >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (n == 0) return PIVOT_OK;
+  if (!in->S_or_F || !in->K || !in->tau || !in->flag || !in->P || !sigma_hat || !sigma_star || !workspace || !out3)
+    return PIVOT_ERR_NULL;
+  if ((reinterpret_cast<uintptr_t>(workspace) & 7u) != 0) return PIVOT_ERR_BAD_ARG;
+  double* w = static_cast<double*>(workspace);
+  double *Ptilde = w, *Vhat = w + n, *sig_rt = w + 2 * n, *vega_rt = w + 3 * n;
+  uint8_t* status = reinterpret_cast<uint8_t*>(w + 4 * n);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const int blocks = ew_blocks(n);
+  if (in->r) rt_prepare_kernel<true><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, vega_floor, n, Ptilde, Vhat);
+  else rt_prepare_kernel<false><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, vega_floor, n, Ptilde, Vhat);
+  if (cudaGetLastError() != cudaSuccess) return PIVOT_ERR_CUDA;
+  pivot_iv_inputs in2 = *in;
+  in2.P = Ptilde;
+  const int rc = pivot_iv_forward(&in2, n, sig_rt, vega_rt, status, stream);   // the same fused inversion kernel
+  if (rc != PIVOT_OK) return rc;
+  rt_reduce_kernel<<<blocks, kEwThreads, 0, st>>>(sig_rt, status, Vhat, sigma_star, vega_floor, n, out3);
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 

@@ -139,3 +139,35 @@ def test_strict_gate_mode_matches_oracle():
         assert np.isnan(g[off & (gs_h != 0)]).all() and np.all(g[off & (gs_h == 0)] == 0)
         on = ~off & np.isfinite(gs_h)
         assert np.isfinite(g[on]).all()
+
+
+@pytest.mark.parametrize("bsm", [False, True])
+def test_losses_match_oracle(bsm):
+    """the sums of eq.(11) and eq.(12) against the oracle's plain loops (different summation order:
+    tolerance 1e-11 relative), including gate-off rows (sentinel price) and rows that are skipped."""
+    cfg = wl.config2(days=6, seed=51) if bsm else wl.config0(200_000, seed=52)
+    d, c = to_device(cfg), to_numpy(cfg)
+    n = c["K"].size
+    rq = dict(r=d.get("r"), q=d.get("q"))
+    rqh = dict(r=c.get("r"), q=c.get("q"))
+    sstar, vstar, st = pv.pivot_iv_forward(*[d[k] for k in KEYS], **rq)
+    sstar_h = sstar.cpu().numpy()
+    rng = np.random.default_rng(7)
+    base = np.where(np.isfinite(sstar_h) & (sstar_h > 0), sstar_h, 0.3)
+    sig_hat = base * (1 + 0.05 * rng.standard_normal(n))
+    sig_hat[::997] = np.nan                                   # skipped rows
+    sh = torch.from_numpy(sig_hat).cuda()
+    vh = pv.pivot_iv_black_price(d["SorF"], d["K"], d["tau"], torch.nan_to_num(sh, nan=0.3), d["flag"], **rq)[1]
+    floor = float(torch.quantile(vh[torch.isfinite(vh)][:1_000_000], 0.3).item())
+    got_p = pv.pivot_iv_loss_price(d["SorF"], d["K"], d["tau"], d["P"], d["flag"], sh, **rq).cpu().numpy()
+    ref_p = po.loss_price(c["SorF"], c["K"], c["tau"], c["P"], c["flag"], sig_hat, **rqh)
+    assert got_p[2] == ref_p[2] and 0 < ref_p[2] < n
+    assert got_p[0] == pytest.approx(ref_p[0], rel=1e-11) and got_p[1] == pytest.approx(ref_p[1], rel=1e-12)
+    got_r = pv.pivot_iv_loss_roundtrip(d["SorF"], d["K"], d["tau"], d["P"], d["flag"], sh, sstar, floor, **rq).cpu().numpy()
+    ref_r = po.loss_roundtrip(c["SorF"], c["K"], c["tau"], c["P"], c["flag"], sig_hat, sstar_h, floor, **rqh)
+    assert abs(got_r[2] - ref_r[2]) <= 2 and ref_r[2] > 0.5 * n      # a row at a status boundary may differ
+    assert got_r[1] == pytest.approx(ref_r[1], rel=1e-9)
+    assert got_r[0] == pytest.approx(ref_r[0], rel=1e-9)
+    # sigma_hat = sigma*: the round-trip loss vanishes (every row inverts back to sigma* or uses the sentinel)
+    zero = pv.pivot_iv_loss_roundtrip(d["SorF"], d["K"], d["tau"], d["P"], d["flag"], sstar, sstar, floor, **rq).cpu().numpy()
+    assert zero[0] <= 1e-22 * max(zero[2], 1.0)
