@@ -222,6 +222,9 @@ struct WEval {
   bool have_W;
 };
 
+// SEED = true: the erfcx pair in fp32 on the FMA pipe (2e-7): enough for the node of the seed interpolant, where
+// z1 = O(1) by construction (no cancellation in e1 - e2) and |h| ~ 0.8 whenever the small-t series is taken.
+template <bool SEED = false>
 __device__ __forceinline__ WEval eval_W(double x, double s) {
   WEval w;
   w.rs = rcp_nr2(s);
@@ -233,7 +236,12 @@ __device__ __forceinline__ WEval eval_W(double x, double s) {
   const double z1 = (ah - t) * kInvSqrt2;
   const bool neg = z1 < 0.0;
   double e1, e2;
-  erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
+  if (SEED) {
+    e1 = (double)erfcx_seed(__double2float_rn(small ? ah * kInvSqrt2 : fabs(z1)));
+    e2 = (double)erfcx_seed(__double2float_rn((ah + t) * kInvSqrt2));
+  } else {
+    erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
+  }
   w.have_W = small || !neg;
   if (small) {
     const double h = w.h;
@@ -353,8 +361,8 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
     return o;
   }
   const double sn = lower ? sl : su;
-  const WEval w = eval_W(x, sn);
-  const double vn = kPhi0 * exp_fast(-w.E);  // b'(s_n)
+  const WEval w = eval_W<true>(x, sn);
+  const double vn = kPhi0 * exp_seed(-w.E);  // b'(s_n), seed grade
   const double bn = w.have_W ? w.Wd * vn : fma(-w.Wd, vn, bmax);
   if (lower ? (beta < bn) : (beta > bn)) {   // a tail: hand the node over
     o.zone = lower ? 0 : 3;
