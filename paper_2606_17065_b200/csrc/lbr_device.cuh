@@ -251,17 +251,20 @@ __device__ __forceinline__ WEval eval_W(double x, double s) {
     const double w3 = fma(h, w2, 2.0 * w1);
     const double w4 = fma(h, w3, 3.0 * w2);
     const double w5 = fma(h, w4, 4.0 * w3);
-    const double w6 = fma(h, w5, 5.0 * w4);
-    const double w7 = fma(h, w6, 6.0 * w5);
-    const double w8 = fma(h, w7, 7.0 * w6);
-    const double w9 = fma(h, w8, 8.0 * w7);
-    const double w10 = fma(h, w9, 9.0 * w8);
-    const double w11 = fma(h, w10, 10.0 * w9);
     const double t2 = t * t;
-    double acc = w11 * kSeriesC[4];
-    acc = fma(acc, t2, w9 * kSeriesC[3]);
-    acc = fma(acc, t2, w7 * kSeriesC[2]);
-    acc = fma(acc, t2, w5 * kSeriesC[1]);
+    double acc = w5 * kSeriesC[1];
+    if (!SEED) {   // seed grade stops at the t^5 term (t < 0.1: the next one is below 1e-8)
+      const double w6 = fma(h, w5, 5.0 * w4);
+      const double w7 = fma(h, w6, 6.0 * w5);
+      const double w8 = fma(h, w7, 7.0 * w6);
+      const double w9 = fma(h, w8, 8.0 * w7);
+      const double w10 = fma(h, w9, 9.0 * w8);
+      const double w11 = fma(h, w10, 10.0 * w9);
+      acc = w11 * kSeriesC[4];
+      acc = fma(acc, t2, w9 * kSeriesC[3]);
+      acc = fma(acc, t2, w7 * kSeriesC[2]);
+      acc = fma(acc, t2, w5 * kSeriesC[1]);
+    }
     acc = fma(acc, t2, w3 * kSeriesC[0]);
     acc = fma(acc, t2, w1);
     w.Wd = s * acc;  // 2 t acc
@@ -332,7 +335,7 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   //   s_l = s_c (t w0 - t^2 w3/6 - t^4 w5/120 - t^6 w7/5040),  w(.) at h = -t, w0 = c erfcx(t/sqrt2)
   const double tc = 0.5 * sc;
   const bool small_c = tc < kSmallT;
-  const double ec = erfcx_one(small_c ? tc * kInvSqrt2 : sc * kInvSqrt2);
+  const double ec = (double)erfcx_seed(__double2float_rn(small_c ? tc * kInvSqrt2 : sc * kInvSqrt2));   // seed grade (2e-7)
   double Wc, sl;
   if (small_c) {
     const double w0 = kSqrtPiOver2 * ec;
