@@ -46,16 +46,19 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __re
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Forward kernel v4, "tile compaction".  A CTA owns a tile of kTileRows consecutive rows.
-//   Phase A (all rows, coalesced 8-byte loads): prelude -> status.  Rows that need the solver are appended to a
-//            compact queue in shared memory (warp ballot + one shared atomic per warp); the others get their final
-//            sigma / vega straight away.  For queued rows the staged output slots carry tau and D sqrt(FK) meanwhile.
-//   Phase B (queued rows only, DENSE warps): x = -log1p(qrel), the four-stage LBR solve, sigma and vega into the
-//            staged output slots of the row's tile position.
+// Forward kernel, "tile compaction".  A CTA owns a tile of kTileRows consecutive rows.
+//   Phase A  (all rows, coalesced 8-byte loads): prelude -> status, with exact IEEE operations and no division.  Rows
+//            that need the solver are appended to a compact queue in shared memory (one warp prefix scan and one shared
+//            atomic per warp per tile); the others get their final sigma / vega straight away.  For queued rows the
+//            staged output slots carry tau and D sqrt(FK) meanwhile.
+//   Phase B1 (queued rows, DENSE warps): lbr_normalise + lbr_seed_head: x, boundary point, node, zone; the middle zones
+//            get their seed here; rows are regrouped by zone class (warp ballots + three shared counters).
+//   Phase B2 (queued rows, grouped zone 0 / middle / zone 3): the tail seeds (lbr_seed_tail0 / _tail3) fused with the
+//            two Householder(3) steps (lbr_refine); sigma and vega into the staged output slots of the row.
 //   Phase C: the staged sigma, vega and status of the tile are streamed out with coalesced stores.
-// Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); the partition by "needs the solver" costs
-// shared-memory traffic only.  The ncu capture of v3 (profiles/r1a_*) showed 10.45 of 32 lanes active because ~2/3 of
-// config 1/4 rows leave at the validity check; here the solver's warps are full.
+// Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); both partitions cost shared-memory traffic only.
+// The ncu capture of the one-row-per-thread kernel (profiles/r1a_*, r1d_ab_*) shows ~11 of 32 lanes active because more
+// than half of config 1/4's rows leave at the validity check; here the solver's warps are full (26.6 of 32).
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
 // RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers) for large n; 1 (256-row tiles) for
@@ -70,7 +73,7 @@ struct TileSmem {
   double q1[kTileRows];
   double q2[kTileRows];
   double q3[kTileRows];
-  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call, bit 14 = zone 3 row with UPPER objective
+  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call
   uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, finished middle-zone rows from the back
   uint16_t permU[kTileRows];  // ... and zone 3 rows
   uint8_t status[kTileRows];
@@ -189,31 +192,26 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   }
   __syncthreads();
 
-  // ---- phase B1b: the tail seeds, zone 0 rows then zone 3 rows, dense (one mixed warp at the boundary)
-  const int n0 = sm.nkind[0], n1 = sm.nkind[1], n3 = sm.nkind[2];
-  for (int k = tid; k < n0 + n3; k += kTileThreads) {
-    Seed sd;
-    int j;
-    if (k < n0) {
-      j = sm.perm[k];
-      sd = lbr_seed_tail0(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
-    } else {
-      j = sm.permU[k - n0];
-      sd = lbr_seed_tail3(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
-      if (sd.kind == KIND_UPPER) sm.pos[j] |= 0x4000;
-    }
-    sm.q1[j] = sd.s; sm.q2[j] = sd.p1; sm.q3[j] = sd.p2;
-  }
-  __syncthreads();
-
-  // ---- phase B2: Householder steps; zone 0 rows (LOWER), then finished middle rows (LINEAR), then zone 3 rows
-  //      (UPPER or LINEAR by their flag): a warp sees one objective kind except at the group boundaries
+  // ---- phase B2: the tail seeds (zone 0 rows, zone 3 rows) fused with the Householder steps; rows ordered zone 0
+  //      (LOWER), finished middle rows (LINEAR), zone 3 (UPPER or LINEAR): a warp sees one zone and one objective kind
+  //      except at the two group boundaries
+  const int n0 = sm.nkind[0], n1 = sm.nkind[1];
   for (int k = tid; k < cnt; k += kTileThreads) {
     int j, kind;
-    if (k < n0) { j = sm.perm[k]; kind = KIND_LOWER; }
-    else if (k < n0 + n1) { j = sm.perm[kTileRows - 1 - (k - n0)]; kind = KIND_LINEAR; }
-    else { j = sm.permU[k - n0 - n1]; kind = (sm.pos[j] & 0x4000) ? KIND_UPPER : KIND_LINEAR; }
-    const NormSolve ns = lbr_refine<kHouseholderSteps>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], kind);
+    double x, s0, p1, p2;
+    if (k < n0) {
+      j = sm.perm[k];
+      const Seed sd = lbr_seed_tail0(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+      x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = KIND_LOWER;
+    } else if (k < n0 + n1) {
+      j = sm.perm[kTileRows - 1 - (k - n0)];
+      x = sm.q0[j]; s0 = sm.q1[j]; p1 = sm.q2[j]; p2 = sm.q3[j]; kind = KIND_LINEAR;
+    } else {
+      j = sm.permU[k - n0 - n1];
+      const Seed sd = lbr_seed_tail3(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+      x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = sd.kind;
+    }
+    const NormSolve ns = lbr_refine<kHouseholderSteps>(x, s0, p1, p2, kind);
     const int p = sm.pos[j] & 0x3fff;
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
