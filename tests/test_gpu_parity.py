@@ -282,3 +282,37 @@ def test_wide_domain_fuzz(case):
     c = dict(zip(KEYS, cols)); c["r"] = None; c["q"] = None
     st = compare_forward(g, o, c)
     assert st["ok"] > 0.3 * n
+
+
+def test_kernel_variants_agree_bit_for_bit():
+    """The 256-row-tile kernel (n <= 2^19), the 1024-row-tile kernel (n > 2^19) and the one-row-per-thread A/B variant
+    (PIVOT_IV_FWD_KERNEL=rowwise, separate process) run the same per-row arithmetic: identical bits on the same rows."""
+    import os
+    import subprocess
+    import sys
+    n_big = (1 << 19) + 1029
+    cfg = wl.config1(n_big, seed=77)
+    d = to_device(cfg)
+    big = pv.pivot_iv_forward(*[d[k] for k in KEYS])                       # 1024-row tiles
+    m = (1 << 19) - 3
+    small = pv.pivot_iv_forward(*[d[k][:m] for k in KEYS])                 # 256-row tiles
+    for a, b in zip(big, small):
+        assert np.array_equal(a[:m].cpu().numpy().view(np.uint8 if a.dtype == torch.uint8 else np.uint64),
+                              b.cpu().numpy().view(np.uint8 if b.dtype == torch.uint8 else np.uint64))
+    code = ("import torch, numpy as np, sys; sys.path.insert(0, %r);"
+            "import paper_2606_17065_b200 as pv; from paper_2606_17065_b200 import workloads as wl;"
+            "c = wl.config1(%d, seed=77, device='cuda');"
+            "o = pv.pivot_iv_forward(*[c[k] for k in ('SorF','K','tau','P','flag')]);"
+            "np.save(sys.argv[1], np.stack([o[0].cpu().numpy().view(np.uint64), o[1].cpu().numpy().view(np.uint64),"
+            " o[2].cpu().numpy().astype(np.uint64)]))") % (os.path.dirname(os.path.dirname(os.path.abspath(__file__))), n_big)
+    import tempfile
+    with tempfile.TemporaryDirectory() as td:
+        out = os.path.join(td, "rw.npy")
+        env = dict(os.environ, PIVOT_IV_FWD_KERNEL="rowwise")
+        subprocess.run([sys.executable, "-c", code, out], check=True, env=env)
+        rw = np.load(out)
+    cfg_dev = wl.config1(n_big, seed=77, device="cuda")                    # same generator as the subprocess
+    ref = pv.pivot_iv_forward(*[cfg_dev[k] for k in KEYS])
+    assert np.array_equal(rw[0], ref[0].cpu().numpy().view(np.uint64))
+    assert np.array_equal(rw[1], ref[1].cpu().numpy().view(np.uint64))
+    assert np.array_equal(rw[2], ref[2].cpu().numpy().astype(np.uint64))
