@@ -77,8 +77,8 @@ struct TileSmem {
   uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, finished middle-zone rows from the back
   uint16_t permU[kTileRows];  // ... and zone 3 rows
   uint8_t status[kTileRows];
+  unsigned long long nclass;  // rows per class, three 21-bit fields: zone 0 | zones 1-2 << 21 | zone 3 << 42
   int count;                  // queued rows
-  int nkind[3];               // rows per class: zone 0, zones 1-2, zone 3
 };
 
 template <bool BSM, bool ZONES, int RPT>
@@ -92,7 +92,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const int lane = tid & 31;
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
   const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
-  if (tid < 4) (&sm.count)[tid] = 0;  // count, nkind[0..2]
+  if (tid == 0) { sm.count = 0; sm.nclass = 0ull; }
   __syncthreads();
 
   // ---- phase A: all rows of the tile; every load of the thread's rows is issued before the first use
@@ -176,15 +176,13 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     const unsigned m0 = __ballot_sync(0xffffffffu, cls == 0);
     const unsigned m1 = __ballot_sync(0xffffffffu, cls == 1);
     const unsigned m2 = __ballot_sync(0xffffffffu, cls == 2);
-    int b0 = 0, b1 = 0, b2 = 0;
-    if (lane == 0) {
-      if (m0) b0 = atomicAdd(&sm.nkind[0], __popc(m0));
-      if (m1) b1 = atomicAdd(&sm.nkind[1], __popc(m1));
-      if (m2) b2 = atomicAdd(&sm.nkind[2], __popc(m2));
-    }
-    b0 = __shfl_sync(0xffffffffu, b0, 0);
-    b1 = __shfl_sync(0xffffffffu, b1, 0);
-    b2 = __shfl_sync(0xffffffffu, b2, 0);
+    // one 64-bit shared atomic per warp hands out the three list offsets at once
+    unsigned long long base3 = 0ull;
+    if (lane == 0)
+      base3 = atomicAdd(&sm.nclass, (unsigned long long)__popc(m0) | ((unsigned long long)__popc(m1) << 21) |
+                                        ((unsigned long long)__popc(m2) << 42));
+    base3 = __shfl_sync(0xffffffffu, base3, 0);
+    const int b0 = (int)(base3 & 0x1fffffu), b1 = (int)((base3 >> 21) & 0x1fffffu), b2 = (int)(base3 >> 42);
     const unsigned lt = (1u << lane) - 1u;
     if (cls == 0) sm.perm[b0 + __popc(m0 & lt)] = (uint16_t)j;
     else if (cls == 1) sm.perm[kTileRows - 1 - (b1 + __popc(m1 & lt))] = (uint16_t)j;
@@ -195,7 +193,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   // ---- phase B2: the tail seeds (zone 0 rows, zone 3 rows) fused with the Householder steps; rows ordered zone 0
   //      (LOWER), finished middle rows (LINEAR), zone 3 (UPPER or LINEAR): a warp sees one zone and one objective kind
   //      except at the two group boundaries
-  const int n0 = sm.nkind[0], n1 = sm.nkind[1];
+  const int n0 = (int)(sm.nclass & 0x1fffffu), n1 = (int)((sm.nclass >> 21) & 0x1fffffu);
   for (int k = tid; k < cnt; k += kTileThreads) {
     int j, kind;
     double x, s0, p1, p2;
