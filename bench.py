@@ -142,6 +142,13 @@ def run_sweep(pv, wl, hbm_peak, flops_mixed):
                 e1.record(stream); e1.synchronize()
                 ts.append(e0.elapsed_time(e1))
             med, best = float(np.median(ts)), float(np.min(ts))
+            # the same 20 launches enqueued back to back (for small n a lone launch is dominated by the host-side call)
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(20):
+                pv.pivot_iv_forward(*a, out=out, stream=stream)
+            e1.record(stream); e1.synchronize()
+            row.setdefault("ms_back_to_back", {})[name] = e0.elapsed_time(e1) / 20
             row[name] = {"ms_median": med, "ms_best": best, "iv_per_s": n / (med * 1e-3),
                          "hbm_frac": FWD_BYTES_PER_ROW * n / (med * 1e-3) / 1e9 / hbm_peak}
             if not so:
