@@ -472,46 +472,53 @@ struct NormSolve {
   double vfin;  // b'(x, s) at that s
 };
 
+// One Householder(3) step.  SEED = true evaluates W, exp and log at seed grade (fp32 erfcx pair, MUFU exp / log,
+// ~1e-6 relative in the step): enough for every step but the last, because the step is fourth order and the last step
+// then takes an iterate that is good to ~1e-6 to ~1e-24.
+template <bool SEED>
+__device__ __forceinline__ double householder_step(double x, double s, double p1, double p2, int kind) {
+  const WEval w = eval_W<SEED>(x, s);
+  const double hr = w.h * w.rs;
+  const double B2 = fma(w.h, hr, -0.25 * s);                  // second derivative of b over b'
+  const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // third derivative of b over b'
+  double nu, h2, h3;
+  if (kind == KIND_LINEAR) {
+    // g = b - beta:  nu = (beta - b)/b'  (p1 = beta, p2 = bbar)
+    const double inv_v = kSqrt2Pi * (SEED ? exp_seed(w.E) : exp_fast(w.E));
+    nu = w.have_W ? fma(p1, inv_v, -w.Wd) : fma(-p2, inv_v, w.Wd);
+    h2 = B2;
+    h3 = B3;
+  } else {
+    const bool want_W = kind == KIND_LOWER;
+    double R = w.Wd;  // the ratio the objective wants: W (lower tail) or Wbar (upper tail)
+    if (want_W != w.have_W) R = fma(exp_fast(0.5 * x) * kSqrt2Pi, exp_fast(w.E), -w.Wd);   // rare: b_max = e^{x/2} rebuilt here
+    const double L = kLnPhi0 - w.E + (SEED ? log_seed(R) : log_fast(R));  // ln b (lower) or ln(b_max - b) (upper)
+    if (want_W) {
+      // g = 1/ln b - 1/ln beta  (p1 = ln beta)
+      const double rLW = rcp_nr2(L * R);
+      const double lam = rLW * R, ub = rLW * L;  // 1/L, b'/b = 1/W
+      const double k2 = fma(2.0, lam, 1.0);
+      nu = (p1 - L) * (L * rcp_nr2(p1)) * R;
+      h2 = fma(-ub, k2, B2);
+      h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
+    } else {
+      // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar  (p1 = ln(b_max - beta))
+      const double gp = rcp_nr2(R);
+      nu = (L - p1) * R;
+      h2 = B2 + gp;
+      h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
+    }
+  }
+  double ds = nu * fma(0.5 * h2, nu, 1.0) * rcp_nr2(fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0));
+  if (!(ds > -0.5 * s)) ds = -0.5 * s;
+  return s + ds;
+}
+
 template <int NITER>
 __device__ __forceinline__ NormSolve lbr_refine(double x, double s, double p1, double p2, int kind) {
 #pragma unroll 1
-  for (int it = 0; it < NITER; ++it) {
-    const WEval w = eval_W(x, s);
-    const double hr = w.h * w.rs;
-    const double B2 = fma(w.h, hr, -0.25 * s);                  // b''/b'
-    const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // b'''/b'
-    double nu, h2, h3;
-    if (kind == KIND_LINEAR) {
-      // g = b - beta:  nu = (beta - b)/b'  (p1 = beta, p2 = bbar)
-      const double inv_v = kSqrt2Pi * exp_fast(w.E);
-      nu = w.have_W ? fma(p1, inv_v, -w.Wd) : fma(-p2, inv_v, w.Wd);
-      h2 = B2;
-      h3 = B3;
-    } else {
-      const bool want_W = kind == KIND_LOWER;
-      double R = w.Wd;  // the ratio the objective wants: W (lower tail) or Wbar (upper tail)
-      if (want_W != w.have_W) R = fma(exp_fast(0.5 * x) * kSqrt2Pi, exp_fast(w.E), -w.Wd);   // rare: b_max = e^{x/2} rebuilt here
-      const double L = kLnPhi0 - w.E + log_fast(R);  // ln b (lower) or ln(b_max - b) (upper)
-      if (want_W) {
-        // g = 1/ln b - 1/ln beta  (p1 = ln beta)
-        const double rLW = rcp_nr2(L * R);
-        const double lam = rLW * R, ub = rLW * L;  // 1/L, b'/b = 1/W
-        const double k2 = fma(2.0, lam, 1.0);
-        nu = (p1 - L) * (L * rcp_nr2(p1)) * R;
-        h2 = fma(-ub, k2, B2);
-        h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
-      } else {
-        // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar  (p1 = ln(b_max - beta))
-        const double gp = rcp_nr2(R);
-        nu = (L - p1) * R;
-        h2 = B2 + gp;
-        h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
-      }
-    }
-    double ds = nu * fma(0.5 * h2, nu, 1.0) * rcp_nr2(fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0));
-    if (!(ds > -0.5 * s)) ds = -0.5 * s;
-    s += ds;
-  }
+  for (int it = 0; it < NITER - 1; ++it) s = householder_step<true>(x, s, p1, p2, kind);
+  s = householder_step<false>(x, s, p1, p2, kind);
   const double rs = rcp_nr2(s);
   const double h = x * rs, t = 0.5 * s;
   NormSolve o;
