@@ -227,7 +227,7 @@ struct WEval {
 template <bool SEED = false>
 __device__ __forceinline__ WEval eval_W(double x, double s) {
   WEval w;
-  w.rs = rcp_nr2(s);
+  w.rs = SEED ? rcp_nr1(s) : rcp_nr2(s);
   w.h = x * w.rs;  // <= 0
   const double t = 0.5 * s;
   const double ah = -w.h;
@@ -495,21 +495,22 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
     const double L = kLnPhi0 - w.E + (SEED ? log_seed(R) : log_fast(R));  // ln b (lower) or ln(b_max - b) (upper)
     if (want_W) {
       // g = 1/ln b - 1/ln beta  (p1 = ln beta)
-      const double rLW = rcp_nr2(L * R);
+      const double rLW = (SEED ? rcp_nr1(L * R) : rcp_nr2(L * R));
       const double lam = rLW * R, ub = rLW * L;  // 1/L, b'/b = 1/W
       const double k2 = fma(2.0, lam, 1.0);
-      nu = (p1 - L) * (L * rcp_nr2(p1)) * R;
+      nu = (p1 - L) * (L * (SEED ? rcp_nr1(p1) : rcp_nr2(p1))) * R;
       h2 = fma(-ub, k2, B2);
       h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
     } else {
       // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar  (p1 = ln(b_max - beta))
-      const double gp = rcp_nr2(R);
+      const double gp = SEED ? rcp_nr1(R) : rcp_nr2(R);
       nu = (L - p1) * R;
       h2 = B2 + gp;
       h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
     }
   }
-  double ds = nu * fma(0.5 * h2, nu, 1.0) * rcp_nr2(fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0));
+  const double den = fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0);
+  double ds = nu * fma(0.5 * h2, nu, 1.0) * (SEED ? rcp_nr1(den) : rcp_nr2(den));
   if (!(ds > -0.5 * s)) ds = -0.5 * s;
   return s + ds;
 }
