@@ -37,7 +37,7 @@ FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # algorithmic bytes per row: forward Black-76 5x8 in + 8+8+1 out; backward 8+8+1 in + 8 out
 FWD_BYTES_PER_ROW = 57
 BWD_BYTES_PER_ROW = 25
-# DRAM traffic per row of the forward kernel measured by ncu (profiles/r1f_forward_tile_ncu_full.md): reads are exactly
+# DRAM traffic per row of the forward kernel measured by ncu (profiles/r1g_forward_tile_ncu_full.md): reads are exactly
 # the 40 algorithmic bytes; part of the 17 written bytes is still dirty in L2 when the kernel ends
 FWD_TRAFFIC_BYTES_PER_ROW = 56.5  # r1c capture: 40.0 read + 16.5 written
 # per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
