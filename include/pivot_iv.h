@@ -13,7 +13,8 @@
  *     explicit pivot_iv_pipeline object), and the device entry points never synchronise the host:
  *     work is enqueued on `stream` (a cudaStream_t passed as an opaque pointer; NULL = the legacy default stream);
  *   - all arrays are SoA, contiguous, length n, fp64 unless stated; pointers need only their natural alignment
- *     (8 B for double): a 16-B-aligned fast path and a scalar path exist on the GPU, there is no CPU fallback;
+ *     (8 B for double): the forward kernel uses 8-byte accesses throughout, the backward kernel has a 16-B-aligned
+ *     vector path and a scalar path; there is no CPU fallback;
  *   - n == 0 is a successful no-op.
  */
 #ifndef PIVOT_IV_H_
