@@ -274,6 +274,16 @@ __device__ __forceinline__ WEval eval_W(double x, double s) {
   return w;
 }
 
+// sqrt(v), v > 0 normal, ~1 ulp, no slow path: MUFU.RSQ64H + two Newton steps + one residual correction
+__device__ __forceinline__ double sqrt_nr2(double v) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(v));
+  y = y * fma(-0.5 * v, y * y, 1.5);
+  y = y * fma(-0.5 * v, y * y, 1.5);
+  const double s = v * y;
+  return fma(fma(-s, s, v), 0.5 * y, s);
+}
+
 // Rational cubic on [0,1] (Delbourgo-Gregory form), H = interval width, u and omu = 1-u both supplied.
 // Seed-grade arithmetic: reciprocals carry ~1e-12.
 __device__ __forceinline__ double rc_eval(double u, double omu, double H, double yl, double yr, double dl, double dr,

@@ -34,20 +34,27 @@ __device__ __forceinline__ void black_row(double SorF, double K, double tau, dou
       if (!pos_fin(F) || !pos_fin(D)) bad = true;
     }
   }
-  const double rootFK = sqrt(F * K);
+  const double FK = F * K;
   const double lo = fmin(F, K), hi = fmax(F, K);
-  if (!pos_fin(rootFK) || !(lo * 0x1p500 >= rootFK)) bad = true;
+  const double rootFK = (FK >= 0x1p-1000 && FK <= 0x1p1000) ? sqrt_nr2(FK) : sqrt(FK);
+  if (!pos_fin(rootFK) || !(lo * 0x1p500 >= rootFK)) bad = true;   // same domain as the forward pass
   if (bad) return;
   const bool call = flag > 0.0;
   const double iota = fmax(call ? F - K : K - F, 0.0);
-  const double rt = sqrt(tau);
+  const double rt = (tau >= 0x1p-1000 && tau <= 0x1p1000) ? sqrt_nr2(tau) : sqrt(tau);
   const double s = sigma * rt;
   double b = 0.0, v = 0.0;
   if (s > 0.0) {
-    const double x = -log1p_fast((hi - lo) / lo);
+    // b_max = lo / sqrt(FK) and qrel = (hi - lo)/lo by Newton reciprocals (as lbr_normalise: lo is never inverted)
+    const double r = rcp_nr2(rootFK);
+    double qq = lo * r;
+    const double bmax = fma(fma(-rootFK, qq, lo), r, qq);
+    const double rl = r * rcp_nr2(bmax), d = hi - lo;
+    qq = d * rl;
+    const double x = -log1p_fast(fma(fma(-lo, qq, d), rl, qq));
     const WEval w = eval_W(x, s);
     v = kPhi0 * exp_fast(-w.E);
-    b = w.have_W ? w.Wd * v : fma(-w.Wd, v, lo / rootFK);
+    b = w.have_W ? w.Wd * v : fma(-w.Wd, v, bmax);
   }
   price = D * fma(rootFK, b, iota);
   vega = D * rootFK * v * rt;
