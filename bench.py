@@ -158,6 +158,42 @@ def run_sweep(pv, wl, hbm_peak, flops_mixed):
     return res
 
 
+def run_configs(pv, wl):
+    """Forward ms at 2^24 rows on the four workload shapes of the A/B table: 10 launches, CUDA events."""
+    n = 1 << 24
+    stream = torch.cuda.current_stream()
+    cases = {"config4_mixed": lambda: wl.config4(n, device="cuda"),
+             "config4_1solve": lambda: wl.config4(n, device="cuda", solve_only=True),
+             "config0": lambda: wl.config0(n, device="cuda"),
+             "config2_bsm_chains": lambda: wl.config2(days=n // 16000, device="cuda")}
+    res = {}
+    for name, mk in cases.items():
+        cfg = mk()
+        a = [cfg[k] for k in KEYS]
+        m = a[0].numel()
+        out = (torch.empty(m, dtype=torch.float64, device="cuda"), torch.empty(m, dtype=torch.float64, device="cuda"),
+               torch.empty(m, dtype=torch.uint8, device="cuda"))
+        for _ in range(3):
+            pv.pivot_iv_forward(*a, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(10):
+            pv.pivot_iv_forward(*a, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
+        e1.record(stream); e1.synchronize()
+        ms = e0.elapsed_time(e1) / 10
+        res[name] = {"rows": m, "ms": ms, "iv_per_s": m / (ms * 1e-3), "solved_fraction": float((out[2] == 0).double().mean().item())}
+        # the same workload through the explicit row-per-thread organisation (pivot_iv_forward_ex, PIVOT_FWD_ROWWISE)
+        for _ in range(3):
+            pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
+        e0.record(stream)
+        for _ in range(10):
+            pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
+        e1.record(stream); e1.synchronize()
+        res[name]["ms_rowwise_hint"] = e0.elapsed_time(e1) / 10
+        del cfg, a, out
+    return res
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -197,6 +233,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--configs", action="store_true",
+                    help="forward-only timing of the other workload shapes at 2^24 rows (config 4 mixed, 1-solve, config 0, "
+                         "config 2 BSM chains); adds a 'configs' dict to the JSON line.  With PIVOT_IV_FWD_KERNEL=rowwise "
+                         "this is the A/B of DESIGN.md section 8")
     ap.add_argument("--sweep", action="store_true",
                     help="config 4: forward-only size sweep n = 2^10 .. 2^28 (all rows and the 1-solve variant); adds a "
                          "'sweep' list to the JSON line")
@@ -406,11 +446,14 @@ def main():
                                          "hbm_frac": bb * n / (ms_b * 1e-3) / 1e9 / hbm_peak}}
         del sig_in
 
-    sweep = None
-    if args.sweep and rank == 0 and world == 1:
+    sweep = configs = None
+    if (args.sweep or args.configs) and rank == 0 and world == 1:
         del cfg, a, out, gP, gsig
         torch.cuda.empty_cache()
-        sweep = run_sweep(pv, wl, hbm_peak, flops_all)
+        if args.sweep:
+            sweep = run_sweep(pv, wl, hbm_peak, flops_all)
+        if args.configs:
+            configs = run_configs(pv, wl)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": "rows/s", "n_gpus": world, "steps": K, "warmup": W,
@@ -428,6 +471,9 @@ def main():
         line.update(err)
         if sweep is not None:
             line["sweep"] = sweep
+        if configs is not None:
+            line["configs"] = configs
+            line["forward_kernel_variant"] = os.environ.get("PIVOT_IV_FWD_KERNEL", "tile")
         if next_rows is not None:
             line["next_rows"] = next_rows
         line["paper_context"] = {"h100_triton_fused_iv_per_s": 1.79e9, "h100_max_rel_err": 9.3e-14,

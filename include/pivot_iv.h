@@ -81,6 +81,19 @@ typedef struct CUstream_st* pivot_iv_stream; /* == cudaStream_t */
 int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
                      pivot_iv_stream stream);
 
+/* Forward pass with an explicit kernel organisation (same arithmetic per row, bit-identical results):
+ *   PIVOT_FWD_COMPACT  rows that need the solver are compacted and regrouped by LBR zone in shared memory before the
+ *                      solver passes run: best when the batch is mixed (degenerate / invalid rows, zones in random order);
+ *   PIVOT_FWD_ROWWISE  one row per thread, no shared memory, no barriers: best when nearly every row solves and
+ *                      neighbouring rows are alike (option chains in strike order: 1.3x on config 2);
+ *   PIVOT_FWD_AUTO     what pivot_iv_forward uses: COMPACT (or the PIVOT_IV_FWD_KERNEL=rowwise environment override).
+ * Returns PIVOT_ERR_BAD_ARG for any other value. */
+#define PIVOT_FWD_AUTO 0
+#define PIVOT_FWD_COMPACT 1
+#define PIVOT_FWD_ROWWISE 2
+int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
+                        pivot_iv_stream stream);
+
 /* As pivot_iv_forward, additionally writing the LBR zone taken by each OK row (0 lower tail, 1 lower middle,
  * 2 upper middle, 3 upper tail; -1 when status != 0).  Diagnostics only: zone edges are transcendental, so this
  * byte is not bit-reproducible across implementations and is not part of `status`. */
@@ -150,6 +163,8 @@ typedef struct pivot_iv_pipeline pivot_iv_pipeline;
 /* Creates a pipeline on CUDA device `device` (-1 = current).  chunk_rows > 0, 1 <= n_slots <= 8. */
 int pivot_iv_pipeline_create(pivot_iv_pipeline** out, int device, int64_t chunk_rows, int n_slots);
 int pivot_iv_pipeline_destroy(pivot_iv_pipeline* p);
+/* Kernel organisation the pipeline's forward launches use (PIVOT_FWD_*; default AUTO). */
+int pivot_iv_pipeline_set_forward_kernel(pivot_iv_pipeline* p, int kernel);
 
 /* Forward on HOST arrays: `in`, sigma, vega, status are host pointers (length n). */
 int pivot_iv_forward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega,

@@ -13,6 +13,9 @@ _SO = os.path.join(HERE, "libpivot_iv.so")
 GATE_MASK = 0
 GATE_ATTENUATE = 1
 GATE_STRICT = 2
+FWD_AUTO = 0
+FWD_COMPACT = 1
+FWD_ROWWISE = 2
 
 # every symbol include/pivot_iv.h declares
 EXPORTS = (
@@ -20,7 +23,7 @@ EXPORTS = (
     "pivot_iv_pipeline_destroy", "pivot_iv_forward_host", "pivot_iv_forward_backward_host", "pivot_iv_probe_dfma",
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
-    "pivot_iv_loss_roundtrip_workspace_bytes",
+    "pivot_iv_loss_roundtrip_workspace_bytes", "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
 )
 
 
@@ -50,6 +53,8 @@ def load_library():
     lib = C.CDLL(_SO)
     vp, i64, dbl, cint = C.c_void_p, C.c_int64, C.c_double, C.c_int
     lib.pivot_iv_forward.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
+    lib.pivot_iv_forward_ex.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, cint, vp]
+    lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
     lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
     lib.pivot_iv_backward.argtypes = [vp, vp, vp, dbl, cint, i64, vp, vp]
     lib.pivot_iv_pipeline_create.argtypes = [C.POINTER(vp), cint, i64, cint]
@@ -104,7 +109,7 @@ def _require_cuda():
         raise PivotError("no CUDA device: the PIVOT path runs only on the GPU (no CPU fallback)")
 
 
-def _forward(SorF, K, tau, P, flag, r, q, out, stream, zones):
+def _forward(SorF, K, tau, P, flag, r, q, out, stream, zones, kernel=None):
     _require_cuda()
     lib = load_library()
     n = SorF.numel()
@@ -126,8 +131,12 @@ def _forward(SorF, K, tau, P, flag, r, q, out, stream, zones):
             _check(lib.pivot_iv_forward_zones(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
                                               _dev(status, "status", torch.uint8), _dev(zone, "zone", torch.int8), sp))
             return sigma, vega, status, zone
-        _check(lib.pivot_iv_forward(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
-                                    _dev(status, "status", torch.uint8), sp))
+        if kernel is not None:
+            _check(lib.pivot_iv_forward_ex(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
+                                           _dev(status, "status", torch.uint8), int(kernel), sp))
+        else:
+            _check(lib.pivot_iv_forward(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
+                                        _dev(status, "status", torch.uint8), sp))
     return sigma, vega, status
 
 
@@ -136,6 +145,11 @@ def pivot_iv_forward(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=N
     """(sigma, vega, status) = pivot_iv_forward(...) on CUDA fp64 tensors; r = q = None selects Black-76 with D = 1.
     `out` = (sigma, vega, status) preallocated tensors; `stream` = torch.cuda.Stream (default: current)."""
     return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, False)
+
+
+def pivot_iv_forward_ex(S_or_F, K, tau, P, flag, kernel: int, r=None, q=None, out=None, stream=None):
+    """pivot_iv_forward with an explicit kernel organisation: FWD_AUTO, FWD_COMPACT or FWD_ROWWISE (same results)."""
+    return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, False, kernel=kernel)
 
 
 def pivot_iv_forward_zones(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None):
@@ -252,6 +266,9 @@ class Pipeline:
         self._lib = load_library()
         self._h = C.c_void_p()
         _check(self._lib.pivot_iv_pipeline_create(C.byref(self._h), int(device), int(chunk_rows), int(n_slots)))
+
+    def set_forward_kernel(self, kernel: int):
+        _check(self._lib.pivot_iv_pipeline_set_forward_kernel(self._h, int(kernel)))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -308,9 +308,9 @@ using namespace pivot;
 
 namespace {
 
-// Tuning knob for the ncu A/B studies: PIVOT_IV_FWD_KERNEL=rowwise selects the v3 kernel
-// (one row per thread, no compaction); anything else (default) the tile-compaction kernel.  Read once.
-bool fwd_rowwise() {
+// Kernel choice.  PIVOT_FWD_AUTO follows the environment variable PIVOT_IV_FWD_KERNEL (=rowwise: one row per thread;
+// anything else / unset: tile compaction), read once; it exists for the ncu A/B studies of DESIGN.md section 8.
+bool env_rowwise() {
   static const bool v = [] {
     const char* e = std::getenv("PIVOT_IV_FWD_KERNEL");
     return e && e[0] == 'r';
@@ -320,8 +320,9 @@ bool fwd_rowwise() {
 
 template <bool BSM, bool ZONES>
 int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
-                     cudaStream_t st) {
-  if (fwd_rowwise()) {
+                     int kernel, cudaStream_t st) {
+  const bool rowwise = kernel == PIVOT_FWD_ROWWISE || (kernel == PIVOT_FWD_AUTO && env_rowwise());
+  if (rowwise) {
     const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
     forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, 0, n, sigma, vega, status, zone);
   } else {
@@ -344,8 +345,9 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
 }
 
 int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
-                 bool zones, cudaStream_t st) {
+                 bool zones, cudaStream_t st, int kernel = PIVOT_FWD_AUTO) {
   if (!in) return PIVOT_ERR_NULL;
+  if (kernel != PIVOT_FWD_AUTO && kernel != PIVOT_FWD_COMPACT && kernel != PIVOT_FWD_ROWWISE) return PIVOT_ERR_BAD_ARG;
   if (n < 0) return PIVOT_ERR_BAD_N;
   if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
   if (n == 0) return PIVOT_OK;
@@ -353,10 +355,10 @@ int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* ve
     return PIVOT_ERR_NULL;
   if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;  // grid.x limit
   const bool bsm = in->r != nullptr;
-  if (bsm) return zones ? launch_forward_t<true, true>(*in, n, sigma, vega, status, zone, st)
-                        : launch_forward_t<true, false>(*in, n, sigma, vega, status, zone, st);
-  return zones ? launch_forward_t<false, true>(*in, n, sigma, vega, status, zone, st)
-               : launch_forward_t<false, false>(*in, n, sigma, vega, status, zone, st);
+  if (bsm) return zones ? launch_forward_t<true, true>(*in, n, sigma, vega, status, zone, kernel, st)
+                        : launch_forward_t<true, false>(*in, n, sigma, vega, status, zone, kernel, st);
+  return zones ? launch_forward_t<false, true>(*in, n, sigma, vega, status, zone, kernel, st)
+               : launch_forward_t<false, false>(*in, n, sigma, vega, status, zone, kernel, st);
 }
 
 int g_sm_count = 0;
@@ -413,6 +415,11 @@ int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double
   return forward_impl(in, n, sigma, vega, status, nullptr, false, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
+                        pivot_iv_stream stream) {
+  return forward_impl(in, n, sigma, vega, status, nullptr, false, reinterpret_cast<cudaStream_t>(stream), kernel);
+}
+
 int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
                            int8_t* zone, pivot_iv_stream stream) {
   return forward_impl(in, n, sigma, vega, status, zone, true, reinterpret_cast<cudaStream_t>(stream));
@@ -461,6 +468,7 @@ struct pivot_iv_pipeline {
   int device = 0;
   int64_t chunk = 0;
   int nslots = 0;
+  int fwd_kernel = PIVOT_FWD_AUTO;
   cudaStream_t streams[8] = {};
   double* dbl[8] = {};   // per slot: 11 fp64 arrays of `chunk` rows: S,K,tau,r,q,P,flag,sigma,vega,gs,gP
   uint8_t* st[8] = {};   // per slot: status bytes
@@ -511,7 +519,7 @@ int pipeline_run(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* 
     if (bwd && cudaMemcpyAsync(d[9], gs + off, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = PIVOT_ERR_CUDA;
     if (rc != PIVOT_OK) break;
     pivot_iv_inputs din{d[0], d[1], d[2], bsm ? d[3] : nullptr, bsm ? d[4] : nullptr, d[5], d[6]};
-    rc = forward_impl(&din, m, d[7], d[8], p->st[slot], nullptr, false, s);
+    rc = forward_impl(&din, m, d[7], d[8], p->st[slot], nullptr, false, s, p->fwd_kernel);
     if (rc == PIVOT_OK && bwd) rc = backward_impl(d[9], d[8], p->st[slot], floor_, mode, m, d[10], s);
     if (rc != PIVOT_OK) break;
     if (cudaMemcpyAsync(sigma + off, d[7], bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
@@ -554,6 +562,13 @@ int pivot_iv_pipeline_create(pivot_iv_pipeline** out, int device, int64_t chunk_
   (void)cudaSetDevice(prev);
   if (rc != PIVOT_OK) { (void)cudaGetLastError(); pivot_iv_pipeline_destroy(p); return rc; }
   *out = p;
+  return PIVOT_OK;
+}
+
+int pivot_iv_pipeline_set_forward_kernel(pivot_iv_pipeline* p, int kernel) {
+  if (!p) return PIVOT_ERR_NULL;
+  if (kernel != PIVOT_FWD_AUTO && kernel != PIVOT_FWD_COMPACT && kernel != PIVOT_FWD_ROWWISE) return PIVOT_ERR_BAD_ARG;
+  p->fwd_kernel = kernel;
   return PIVOT_OK;
 }
 

@@ -316,3 +316,31 @@ def test_kernel_variants_agree_bit_for_bit():
     assert np.array_equal(rw[0], ref[0].cpu().numpy().view(np.uint64))
     assert np.array_equal(rw[1], ref[1].cpu().numpy().view(np.uint64))
     assert np.array_equal(rw[2], ref[2].cpu().numpy().astype(np.uint64))
+
+
+def test_forward_ex_kernel_choices_are_bit_identical():
+    """pivot_iv_forward_ex: COMPACT, ROWWISE and AUTO give the same bits (Black-76 and BSM); a bad choice is an error;
+    the host pipeline honours pivot_iv_pipeline_set_forward_kernel."""
+    for cfg in (wl.config1(300_001, seed=91), wl.config2(days=4, seed=92)):
+        d = to_device(cfg)
+        a = [d[k] for k in KEYS]
+        ref = pv.pivot_iv_forward(*a, r=d.get("r"), q=d.get("q"))
+        for kern in (pv.FWD_AUTO, pv.FWD_COMPACT, pv.FWD_ROWWISE):
+            got = pv.pivot_iv_forward_ex(*a, kern, r=d.get("r"), q=d.get("q"))
+            assert torch.equal(got[2], ref[2])
+            assert np.array_equal(got[0].cpu().numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
+            assert np.array_equal(got[1].cpu().numpy().view(np.uint64), ref[1].cpu().numpy().view(np.uint64))
+        with pytest.raises(pv.PivotError):
+            pv.pivot_iv_forward_ex(*a, 7, r=d.get("r"), q=d.get("q"))
+    cfg = wl.config2(days=2, seed=93)
+    host = {k: (v.contiguous() if isinstance(v, torch.Tensor) else v) for k, v in cfg.items()}
+    pipe = pv.Pipeline(chunk_rows=10_000, n_slots=2)
+    pipe.set_forward_kernel(pv.FWD_ROWWISE)
+    hs, hv, hst = pipe.forward_host(*[host[k] for k in KEYS], r=host["r"], q=host["q"])
+    with pytest.raises(pv.PivotError):
+        pipe.set_forward_kernel(9)
+    pipe.close()
+    d = to_device(cfg)
+    ref = pv.pivot_iv_forward(*[d[k] for k in KEYS], r=d["r"], q=d["q"])
+    assert np.array_equal(hs.numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
+    assert np.array_equal(hst.numpy(), ref[2].cpu().numpy())
