@@ -190,6 +190,16 @@ def run_configs(pv, wl):
             pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
         e1.record(stream); e1.synchronize()
         res[name]["ms_rowwise_hint"] = e0.elapsed_time(e1) / 10
+        # ... and through pivot_iv_forward_auto (probe + the chosen organisation)
+        ws = torch.zeros(16, dtype=torch.int32, device="cuda")
+        for _ in range(3):
+            pv.pivot_iv_forward_auto(*a, r=cfg["r"], q=cfg["q"], out=out, workspace=ws, stream=stream)
+        e0.record(stream)
+        for _ in range(10):
+            pv.pivot_iv_forward_auto(*a, r=cfg["r"], q=cfg["q"], out=out, workspace=ws, stream=stream)
+        e1.record(stream); e1.synchronize()
+        res[name]["ms_auto"] = e0.elapsed_time(e1) / 10
+        res[name]["auto_probe[decision,solved,alike,samples]"] = ws[:4].tolist()
         del cfg, a, out
     return res
 

@@ -86,13 +86,27 @@ int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double
  *                      solver passes run: best when the batch is mixed (degenerate / invalid rows, zones in random order);
  *   PIVOT_FWD_ROWWISE  one row per thread, no shared memory, no barriers: best when nearly every row solves and
  *                      neighbouring rows are alike (option chains in strike order: 1.3x on config 2);
- *   PIVOT_FWD_AUTO     what pivot_iv_forward uses: COMPACT (or the PIVOT_IV_FWD_KERNEL=rowwise environment override).
+ *   PIVOT_FWD_AUTO     what pivot_iv_forward uses: COMPACT (or the PIVOT_IV_FWD_KERNEL=rowwise environment override);
+ *                      pivot_iv_forward_auto decides from a sampled probe instead.
  * Returns PIVOT_ERR_BAD_ARG for any other value. */
 #define PIVOT_FWD_AUTO 0
 #define PIVOT_FWD_COMPACT 1
 #define PIVOT_FWD_ROWWISE 2
 int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
                         pivot_iv_stream stream);
+
+/* Forward pass that chooses the organisation itself.  For n >= 2^23 a probe samples 2048 (row, next row) pairs
+ * (does the row reach the solver?  are the two rows the same contract up to 2 % in F|S and K?), writes its decision to
+ * `workspace`, and both organisations are enqueued: the one not chosen returns at once.  ROWWISE is chosen when >= 95 % of
+ * the sampled rows solve and >= 90 % of the pairs are alike (option chains in strike order); COMPACT otherwise and for
+ * n < 2^23 (no probe: it and the unused launch cost ~30 us).  Same results as pivot_iv_forward, bit for bit.  3 launches.
+ *   workspace [device, pivot_iv_forward_auto_workspace_bytes() bytes, 4-byte aligned]; afterwards, as ints:
+ *             [0] decision (1 = ROWWISE), [1] sampled rows that solve, [2] alike pairs, [3] samples; [4..6] are the
+ *             probe's counters and MUST BE ZERO before the first call (the probe leaves them zero).  May be NULL if n < 2^23.
+ * Returns as pivot_iv_forward, plus PIVOT_ERR_BAD_ARG for a misaligned workspace. */
+int64_t pivot_iv_forward_auto_workspace_bytes(void);
+int pivot_iv_forward_auto(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                          void* workspace, pivot_iv_stream stream);
 
 /* As pivot_iv_forward, additionally writing the LBR zone taken by each OK row (0 lower tail, 1 lower middle,
  * 2 upper middle, 3 upper tail; -1 when status != 0).  Diagnostics only: zone edges are transcendental, so this

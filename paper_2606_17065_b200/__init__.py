@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     pivot_iv_backward,
     pivot_iv_backward_inputs,
     pivot_iv_forward,
+    pivot_iv_forward_auto,
     pivot_iv_forward_ex,
     pivot_iv_forward_zones,
     pivot_iv_loss_price,
@@ -34,5 +35,5 @@ __all__ = [
     "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "Pipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
-    "GATE_ATTENUATE", "GATE_STRICT", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "pivot_iv_forward_ex", "EXPORTS",
+    "GATE_ATTENUATE", "GATE_STRICT", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "pivot_iv_forward_ex", "pivot_iv_forward_auto", "EXPORTS",
 ]

@@ -24,6 +24,7 @@ EXPORTS = (
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_loss_roundtrip_workspace_bytes", "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
+    "pivot_iv_forward_auto", "pivot_iv_forward_auto_workspace_bytes",
 )
 
 
@@ -55,6 +56,8 @@ def load_library():
     lib.pivot_iv_forward.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
     lib.pivot_iv_forward_ex.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, cint, vp]
     lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
+    lib.pivot_iv_forward_auto.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
+    lib.pivot_iv_forward_auto_workspace_bytes.argtypes = []
     lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
     lib.pivot_iv_backward.argtypes = [vp, vp, vp, dbl, cint, i64, vp, vp]
     lib.pivot_iv_pipeline_create.argtypes = [C.POINTER(vp), cint, i64, cint]
@@ -70,9 +73,11 @@ def load_library():
     lib.pivot_iv_loss_roundtrip.argtypes = [C.POINTER(_Inputs), vp, vp, dbl, i64, vp, vp, vp]
     lib.pivot_iv_loss_roundtrip_workspace_bytes.argtypes = [i64]
     for name in EXPORTS:
-        if name not in ("pivot_iv_strerror", "pivot_iv_loss_roundtrip_workspace_bytes"):
+        if name not in ("pivot_iv_strerror", "pivot_iv_loss_roundtrip_workspace_bytes",
+                        "pivot_iv_forward_auto_workspace_bytes"):
             getattr(lib, name).restype = cint
     lib.pivot_iv_loss_roundtrip_workspace_bytes.restype = i64
+    lib.pivot_iv_forward_auto_workspace_bytes.restype = i64
     _lib = lib
     return lib
 
@@ -150,6 +155,25 @@ def pivot_iv_forward(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=N
 def pivot_iv_forward_ex(S_or_F, K, tau, P, flag, kernel: int, r=None, q=None, out=None, stream=None):
     """pivot_iv_forward with an explicit kernel organisation: FWD_AUTO, FWD_COMPACT or FWD_ROWWISE (same results)."""
     return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, False, kernel=kernel)
+
+
+def pivot_iv_forward_auto(S_or_F, K, tau, P, flag, r=None, q=None, out=None, workspace=None, stream=None):
+    """pivot_iv_forward that picks COMPACT or ROWWISE from a sampled probe (n >= 2^23).  Returns (sigma, vega, status,
+    workspace); workspace (int32 CUDA tensor) holds [decision, solved samples, alike pairs, samples] afterwards."""
+    _require_cuda()
+    lib = load_library()
+    n = S_or_F.numel()
+    inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P, "P"),
+                  _dev(flag, "flag"))
+    if out is None:
+        out = (torch.empty(n, dtype=torch.float64, device=S_or_F.device), torch.empty(n, dtype=torch.float64, device=S_or_F.device),
+               torch.empty(n, dtype=torch.uint8, device=S_or_F.device))
+    if workspace is None:
+        workspace = torch.zeros(int(lib.pivot_iv_forward_auto_workspace_bytes()) // 4, dtype=torch.int32, device=S_or_F.device)
+    with torch.cuda.device(S_or_F.device):
+        _check(lib.pivot_iv_forward_auto(C.byref(inp), n, _dev(out[0], "sigma"), _dev(out[1], "vega"),
+                                         _dev(out[2], "status", torch.uint8), workspace.data_ptr(), _stream_ptr(stream)))
+    return out[0], out[1], out[2], workspace
 
 
 def pivot_iv_forward_zones(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None):

@@ -34,15 +34,28 @@ __device__ __forceinline__ void solve_and_store(int64_t i, double S, double K, d
   if (ZONES) zone[i] = o.zone;
 }
 
-template <bool BSM, bool ZONES>
+// SEL = false: one launch covers the rows (grid = ceil(n / 128)).  SEL = true (pivot_iv_forward_auto): small grid-stride
+// grid that first reads the probe's decision and returns at once when the other organisation was chosen.
+template <bool BSM, bool ZONES, bool SEL = false>
 __global__ void __launch_bounds__(kFwdThreads)
 forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __restrict__ sigma,
-                      double* __restrict__ vega, uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
-  const int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
-  solve_and_store<BSM, ZONES>(i, __ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(in.P + i),
-                              __ldcs(in.flag + i), sigma, vega, status, zone);
+                      double* __restrict__ vega, uint8_t* __restrict__ status, int8_t* __restrict__ zone,
+                      const int* __restrict__ sel, int want) {
+  if (SEL) {
+    if (*sel != want) return;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+      const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+      solve_and_store<BSM, ZONES>(i, __ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(in.P + i),
+                                  __ldcs(in.flag + i), sigma, vega, status, zone);
+    }
+  } else {
+    const int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+    solve_and_store<BSM, ZONES>(i, __ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(in.P + i),
+                                __ldcs(in.flag + i), sigma, vega, status, zone);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -81,10 +94,11 @@ struct TileSmem {
   int count;                  // queued rows
 };
 
-template <bool BSM, bool ZONES, int RPT>
+template <bool BSM, bool ZONES, int RPT, bool SEL = false>
 __global__ void __launch_bounds__(kTileThreads, BSM ? 3 : 4)
 forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
-                    uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
+                    uint8_t* __restrict__ status, int8_t* __restrict__ zone, const int* __restrict__ sel, int want) {
+  if (SEL && *sel != want) return;   // pivot_iv_forward_auto: the probe chose the other organisation
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int kTileRows = kTileThreads * RPT;
   TileSmem<RPT>& sm = *reinterpret_cast<TileSmem<RPT>*>(smem_raw);
@@ -297,6 +311,44 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(int64_t iters, double* 
   if (sum == 123.456) sink[0] = sum;  // never true; keeps the chains alive
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Probe of pivot_iv_forward_auto: 2048 sampled (row, next row) pairs.  ws[0] = 1 (row-per-thread organisation) when at
+// least 95 % of the sampled rows reach the solver AND at least 90 % of the pairs are the same contract up to 2 % in F|S
+// and K (an option chain in strike order: warps are zone-uniform by themselves); else 0 (compaction).  ws[1..3] = rows
+// that solve, alike pairs, samples.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kProbePairs = 2048;
+constexpr int kProbeBlocks = 8;   // 8 x 256 threads: one pair per thread, every load of the probe is in flight at once
+template <bool BSM>
+__global__ void __launch_bounds__(256) forward_probe_kernel(pivot_iv_inputs in, int64_t n, int* __restrict__ ws) {
+  // ws[1], ws[2] accumulate; ws[4] is the ticket; the last CTA to arrive decides and resets the accumulators' ticket
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t i = (int64_t)(((n - 2) / kProbePairs) * (int64_t)k);
+  const double F0 = in.S_or_F[i], K0 = in.K[i], F1 = in.S_or_F[i + 1], K1 = in.K[i + 1];
+  const double r = BSM ? in.r[i] : 0.0, q = BSM ? in.q[i] : 0.0;
+  const Prelude pr = lbr_prelude<BSM>(F0, K0, in.tau[i], r, q, in.P[i], in.flag[i]);
+  const unsigned mo = __ballot_sync(0xffffffffu, pr.status == PIVOT_ST_OK);
+  const unsigned ma = __ballot_sync(0xffffffffu, fabs(K1 - K0) <= 0.02 * K0 && fabs(F1 - F0) <= 0.02 * F0);
+  __shared__ int last;
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&ws[5], __popc(mo));
+    atomicAdd(&ws[6], __popc(ma));
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    last = atomicAdd(&ws[4], 1) == kProbeBlocks - 1;
+  }
+  __syncthreads();
+  if (last && threadIdx.x == 0) {
+    __threadfence();
+    const int ok = atomicAdd(&ws[5], 0), alike = atomicAdd(&ws[6], 0);
+    ws[1] = ok; ws[2] = alike; ws[3] = kProbePairs;
+    ws[0] = (ok * 100 >= 95 * kProbePairs && alike * 100 >= 90 * kProbePairs) ? 1 : 0;
+    ws[4] = 0; ws[5] = 0; ws[6] = 0;   // ready for the next call on this stream
+  }
+}
+
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace pivot
@@ -324,7 +376,7 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
   const bool rowwise = kernel == PIVOT_FWD_ROWWISE || (kernel == PIVOT_FWD_AUTO && env_rowwise());
   if (rowwise) {
     const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
-    forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, 0, n, sigma, vega, status, zone);
+    forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, 0, n, sigma, vega, status, zone, nullptr, 0);
   } else {
     // small launches use 256-row tiles so that the grid still covers the chip (n <= 2^19: at most 2048 CTAs)
     if (n <= ((int64_t)1 << 19)) {
@@ -332,13 +384,13 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
                                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<1>));
       if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
       const int64_t blocks = (n + kTileThreads - 1) / kTileThreads;
-      forward_kernel_tile<BSM, ZONES, 1><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<1>), st>>>(in, n, sigma, vega, status, zone);
+      forward_kernel_tile<BSM, ZONES, 1><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<1>), st>>>(in, n, sigma, vega, status, zone, nullptr, 0);
     } else {
       static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES, 4>,
                                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<4>));
       if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
       const int64_t blocks = (n + 4 * kTileThreads - 1) / (4 * kTileThreads);
-      forward_kernel_tile<BSM, ZONES, 4><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<4>), st>>>(in, n, sigma, vega, status, zone);
+      forward_kernel_tile<BSM, ZONES, 4><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<4>), st>>>(in, n, sigma, vega, status, zone, nullptr, 0);
     }
   }
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
@@ -370,6 +422,25 @@ int sm_count() {
     g_sm_count = sms;
   }
   return g_sm_count;
+}
+
+// pivot_iv_forward_auto: probe, then both organisations are enqueued and the one the probe did not choose returns at
+// once (the row-per-thread kernel as a small grid-stride grid, so that its early exit costs microseconds).
+template <bool BSM>
+int launch_forward_auto_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int* ws,
+                          cudaStream_t st) {
+  static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, false, 4, true>,
+                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<4>));
+  if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
+  forward_probe_kernel<BSM><<<kProbeBlocks, kProbePairs / kProbeBlocks, 0, st>>>(in, n, ws);
+  const int64_t rblocks = (n + kFwdThreads - 1) / kFwdThreads;
+  const int64_t rcap = (int64_t)sm_count() * 6 * 8;    // 80 registers: 6 resident CTAs of 128 threads per SM; 8 waves' worth, grid-stride
+  forward_kernel_scalar<BSM, false, true><<<(unsigned)(rblocks < rcap ? rblocks : rcap), kFwdThreads, 0, st>>>(
+      in, 0, n, sigma, vega, status, nullptr, ws, 1);
+  const int64_t tblocks = (n + 4 * kTileThreads - 1) / (4 * kTileThreads);
+  forward_kernel_tile<BSM, false, 4, true><<<(unsigned)tblocks, kTileThreads, sizeof(TileSmem<4>), st>>>(in, n, sigma, vega,
+                                                                                                       status, nullptr, ws, 0);
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 
 template <int MODE>
@@ -418,6 +489,24 @@ int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double
 int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
                         pivot_iv_stream stream) {
   return forward_impl(in, n, sigma, vega, status, nullptr, false, reinterpret_cast<cudaStream_t>(stream), kernel);
+}
+
+int64_t pivot_iv_forward_auto_workspace_bytes(void) { return 64; }
+
+int pivot_iv_forward_auto(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                          void* workspace, pivot_iv_stream stream) {
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < ((int64_t)1 << 23))   // no probe below 2^23 rows (probe + the unused launch cost ~30 us); workspace not used
+    return forward_impl(in, n, sigma, vega, status, nullptr, false, st, PIVOT_FWD_COMPACT);
+  if (!workspace) return PIVOT_ERR_NULL;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status) return PIVOT_ERR_NULL;
+  if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;
+  if ((reinterpret_cast<uintptr_t>(workspace) & 3u) != 0) return PIVOT_ERR_BAD_ARG;
+  int* ws = static_cast<int*>(workspace);
+  return in->r ? launch_forward_auto_t<true>(*in, n, sigma, vega, status, ws, st)
+               : launch_forward_auto_t<false>(*in, n, sigma, vega, status, ws, st);
 }
 
 int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,

@@ -344,3 +344,27 @@ def test_forward_ex_kernel_choices_are_bit_identical():
     ref = pv.pivot_iv_forward(*[d[k] for k in KEYS], r=d["r"], q=d["q"])
     assert np.array_equal(hs.numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
     assert np.array_equal(hst.numpy(), ref[2].cpu().numpy())
+
+
+def test_forward_auto_chooses_and_matches():
+    """pivot_iv_forward_auto: ordered dense chains -> ROWWISE, mixed rows -> COMPACT, small n -> no probe; same bits."""
+    chains = to_device(wl.config2(days=1100, seed=95))          # 17.6 M rows >= 2^24
+    a = [chains[k] for k in KEYS]
+    ref = pv.pivot_iv_forward(*a, r=chains["r"], q=chains["q"])
+    for _ in range(2):                                           # second call reuses the workspace
+        ws = torch.zeros(16, dtype=torch.int32, device="cuda") if _ == 0 else ws
+        s, v, st, ws = pv.pivot_iv_forward_auto(*a, r=chains["r"], q=chains["q"], workspace=ws)
+        w = ws.cpu().numpy()
+        assert w[0] == 1 and w[3] == 2048 and w[1] >= 0.95 * 2048 and w[2] >= 0.9 * 2048 and not w[4:7].any()
+        assert torch.equal(st, ref[2]) and torch.equal(s.view(torch.int64), ref[0].view(torch.int64))
+        assert torch.equal(v.view(torch.int64), ref[1].view(torch.int64))
+    del chains, a, ref
+    mixed = to_device(wl.config1(1 << 24, seed=96))
+    a = [mixed[k] for k in KEYS]
+    ref = pv.pivot_iv_forward(*a)
+    s, v, st, ws = pv.pivot_iv_forward_auto(*a)
+    assert ws[0].item() == 0
+    assert torch.equal(st, ref[2]) and torch.equal(s.view(torch.int64), ref[0].view(torch.int64))
+    small = [t[:100_000] for t in a]
+    s2, v2, st2, ws2 = pv.pivot_iv_forward_auto(*small)
+    assert ws2[3].item() == 0 and torch.equal(s2.view(torch.int64), ref[0][:100_000].view(torch.int64))
