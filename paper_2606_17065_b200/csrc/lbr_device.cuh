@@ -8,10 +8,12 @@
 //   z1 >= 0:  W    = c [erfcx(z1) - erfcx(z2)]                       Wbar = b_max/b' - W
 //   z1 <  0:  Wbar = c [erfcx(-z1) + erfcx(z2)]                      W    = b_max/b' - Wbar
 //   t < 0.1:  W    = 2 sum_j w^(2j+1)(h) t^(2j+1)/(2j+1)!,  w(z) = Phi(z)/phi(z) = c erfcx(-z/sqrt2)   (no cancellation)
-// The solve is split in two passes so that the kernel can regroup rows in shared memory between them (pivot_iv.cu):
-// lbr_seed (boundary point, zone, rational seed; seed-grade arithmetic) and lbr_refine (Householder(3) steps at full
-// precision).  exp / log / log1p / erfcx / reciprocals are this file's own, with coefficients in constant memory
-// (gen_coeffs.py): no slow paths, no 64-bit immediates.  See DESIGN.md section 5.
+// The solve is split in passes so that the kernel can regroup rows in shared memory between them (pivot_iv.cu):
+// lbr_seed_head (boundary point, node, zone), lbr_seed_tail0 / _tail3 (tail seeds) and lbr_refine (Householder(3) steps).
+// Precision tiers: the seed and every Householder step but the last run at "seed grade" (fp32 erfcx, MUFU exp / log,
+// one-Newton reciprocals); the normalisation, ln(beta), the last step and b' at the final s run at full fp64.
+// exp / log / log1p / erfcx / reciprocals are this file's own, with coefficients in constant memory (gen_coeffs.py):
+// no slow paths, no 64-bit immediates.  See DESIGN.md section 5.
 // This file shares nothing with oracle/ (the CPU checker).
 #pragma once
 #include <cstdint>

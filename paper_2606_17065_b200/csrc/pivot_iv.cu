@@ -1,7 +1,9 @@
 // pivot_iv.cu -- kernels and C ABI (include/pivot_iv.h) of the PIVOT implied-volatility hot path, sm_100a.
 //
-// Forward: one fused kernel; every intermediate of the per-row LBR solve lives in registers, HBM is touched once per
-// element (57 B/row Black-76, 73 B/row BSM).  Backward: one streaming elementwise kernel (25 B/row).
+// Forward: one fused kernel; every intermediate of the per-row LBR solve lives in registers or shared memory, HBM is
+// touched once per element (57 B/row Black-76, 73 B/row BSM).  Two organisations of the same per-row arithmetic:
+// forward_kernel_tile (rows compacted and regrouped by LBR zone in shared memory; the default) and
+// forward_kernel_scalar (one row per thread).  Backward: one streaming elementwise kernel (25 B/row).
 // No tensor cores: the path is an fp64 transcendental chain, not a contraction.
 #include <cuda_runtime.h>
 
@@ -20,8 +22,8 @@ constexpr int kBwdThreads = 256;
 constexpr int kHouseholderSteps = 2;  // north_star: two Householder(3) steps
 
 // ---------------------------------------------------------------------------------------------------------------
-// Forward kernel.  ROWS rows per thread: ROWS = 2 reads each input array with one 16-byte load (double2) per thread,
-// a warp covering 512 contiguous bytes per array; ROWS = 1 is the 8-byte-aligned fallback and the tail.
+// Forward kernel, one row per thread (PIVOT_FWD_ROWWISE): no shared memory, no barriers; coalesced 8-byte accesses.
+// Best when nearly every row solves and neighbouring rows are alike (option chains in strike order).
 // ---------------------------------------------------------------------------------------------------------------
 template <bool BSM, bool ZONES>
 __device__ __forceinline__ void solve_and_store(int64_t i, double S, double K, double tau, double r, double q, double P,
