@@ -81,38 +81,42 @@ typedef struct CUstream_st* pivot_iv_stream; /* == cudaStream_t */
 int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
                      pivot_iv_stream stream);
 
-/* Forward pass with an explicit kernel organisation (same arithmetic per row, bit-identical results):
+/* Forward pass with an explicit kernel organisation and precision tier:
  *   PIVOT_FWD_COMPACT  rows that need the solver are compacted and regrouped by LBR zone in shared memory before the
  *                      solver passes run: best when the batch is mixed (degenerate / invalid rows, zones in random order);
  *   PIVOT_FWD_ROWWISE  one row per thread, no shared memory, no barriers: best when nearly every row solves and
- *                      neighbouring rows are alike (option chains in strike order: 1.3x on config 2);
- *   PIVOT_FWD_AUTO     what pivot_iv_forward uses: COMPACT (or the PIVOT_IV_FWD_KERNEL=rowwise environment override);
- *                      pivot_iv_forward_auto decides from a sampled probe instead.
+ *                      neighbouring rows are alike (option chains in strike order);
+ *   PIVOT_FWD_AUTO     what pivot_iv_forward uses (COMPACT).
+ * COMPACT and ROWWISE run the same per-row arithmetic: bit-identical results.
+ *   PIVOT_FWD_FP64_ONLY (flag, OR it into any of the three): every special function, reciprocal and interpolant of the
+ *                      seed and of the first Householder step at full fp64 instead of "seed grade" (fp32 erfcx, MUFU
+ *                      exp / log, fp32 rational cubics).  The default tiering only has to land inside the basin of the
+ *                      last, full-precision Householder step (PAPER.md:125 says fp64 throughout; DESIGN.md section 5
+ *                      bounds what the tiering changes: the two agree to <= 1e-13 relative in sigma).  Diagnostic / A-B.
  * Returns PIVOT_ERR_BAD_ARG for any other value. */
 #define PIVOT_FWD_AUTO 0
 #define PIVOT_FWD_COMPACT 1
 #define PIVOT_FWD_ROWWISE 2
+#define PIVOT_FWD_FP64_ONLY 4
 int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
                         pivot_iv_stream stream);
-
-/* Forward pass that chooses the organisation itself.  For n >= 2^23 a probe samples 2048 (row, next row) pairs
- * (does the row reach the solver?  are the two rows the same contract up to 2 % in F|S and K?), writes its decision to
- * `workspace`, and both organisations are enqueued: the one not chosen returns at once.  ROWWISE is chosen when >= 95 % of
- * the sampled rows solve and >= 90 % of the pairs are alike (option chains in strike order); COMPACT otherwise and for
- * n < 2^23 (no probe: it and the unused launch cost ~30 us).  Same results as pivot_iv_forward, bit for bit.  3 launches.
- *   workspace [device, pivot_iv_forward_auto_workspace_bytes() bytes, 4-byte aligned]; afterwards, as ints:
- *             [0] decision (1 = ROWWISE), [1] sampled rows that solve, [2] alike pairs, [3] samples; [4..6] are the
- *             probe's counters and MUST BE ZERO before the first call (the probe leaves them zero).  May be NULL if n < 2^23.
- * Returns as pivot_iv_forward, plus PIVOT_ERR_BAD_ARG for a misaligned workspace. */
-int64_t pivot_iv_forward_auto_workspace_bytes(void);
-int pivot_iv_forward_auto(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
-                          void* workspace, pivot_iv_stream stream);
 
 /* As pivot_iv_forward, additionally writing the LBR zone taken by each OK row (0 lower tail, 1 lower middle,
  * 2 upper middle, 3 upper tail; -1 when status != 0).  Diagnostics only: zone edges are transcendental, so this
  * byte is not bit-reproducible across implementations and is not part of `status`. */
 int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
                            int8_t* zone, pivot_iv_stream stream);
+
+/* Diagnostics of the solve (rational seed, then Householder(3) steps), per row, in total
+ * volatility s = sigma sqrt(tau):
+ *   zone     [out, device, n bytes or NULL]    as pivot_iv_forward_zones
+ *   s_seed   [out, device, n doubles or NULL]  the rational initial guess s0 (0 when status != 0)
+ *   s_step1  [out, device, n doubles or NULL]  the iterate after the first Householder(3) step, i.e. what the last,
+ *                                              full-precision step starts from (0 when status != 0)
+ *   kernel   PIVOT_FWD_* as in pivot_iv_forward_ex
+ * sigma / vega / status as pivot_iv_forward (same bits).  Used by the tests that bound the seed-grade tier. */
+int pivot_iv_forward_diag(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                          int8_t* zone, double* s_seed, double* s_step1, int kernel, pivot_iv_stream stream);
 
 /* Backward pass, one fused elementwise kernel (PAPER.md:100-103 Alg.1 l.4-6; :107 eq.(7); :131 eq.(8) first half;
  * :144 eq.(9); :150 eq.(10)).  Reads only what the forward emitted: 25 B per row.

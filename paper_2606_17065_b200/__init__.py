@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     FWD_AUTO,
     FWD_COMPACT,
     FWD_ROWWISE,
+    FWD_FP64_ONLY,
     PivotError,
     Pipeline,
     library_path,
@@ -19,7 +20,7 @@ from .binding import (  # noqa: F401
     pivot_iv_backward,
     pivot_iv_backward_inputs,
     pivot_iv_forward,
-    pivot_iv_forward_auto,
+    pivot_iv_forward_diag,
     pivot_iv_forward_ex,
     pivot_iv_forward_zones,
     pivot_iv_loss_price,
@@ -35,5 +36,5 @@ __all__ = [
     "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "Pipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
-    "GATE_ATTENUATE", "GATE_STRICT", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "pivot_iv_forward_ex", "pivot_iv_forward_auto", "EXPORTS",
+    "GATE_ATTENUATE", "GATE_STRICT", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "EXPORTS",
 ]

@@ -16,6 +16,7 @@ GATE_STRICT = 2
 FWD_AUTO = 0
 FWD_COMPACT = 1
 FWD_ROWWISE = 2
+FWD_FP64_ONLY = 4   # flag: OR into FWD_AUTO / FWD_COMPACT / FWD_ROWWISE
 
 # every symbol include/pivot_iv.h declares
 EXPORTS = (
@@ -24,7 +25,7 @@ EXPORTS = (
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_loss_roundtrip_workspace_bytes", "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
-    "pivot_iv_forward_auto", "pivot_iv_forward_auto_workspace_bytes",
+    "pivot_iv_forward_diag",
 )
 
 
@@ -56,8 +57,7 @@ def load_library():
     lib.pivot_iv_forward.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
     lib.pivot_iv_forward_ex.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, cint, vp]
     lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
-    lib.pivot_iv_forward_auto.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
-    lib.pivot_iv_forward_auto_workspace_bytes.argtypes = []
+    lib.pivot_iv_forward_diag.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp, vp, cint, vp]
     lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
     lib.pivot_iv_backward.argtypes = [vp, vp, vp, dbl, cint, i64, vp, vp]
     lib.pivot_iv_pipeline_create.argtypes = [C.POINTER(vp), cint, i64, cint]
@@ -73,11 +73,9 @@ def load_library():
     lib.pivot_iv_loss_roundtrip.argtypes = [C.POINTER(_Inputs), vp, vp, dbl, i64, vp, vp, vp]
     lib.pivot_iv_loss_roundtrip_workspace_bytes.argtypes = [i64]
     for name in EXPORTS:
-        if name not in ("pivot_iv_strerror", "pivot_iv_loss_roundtrip_workspace_bytes",
-                        "pivot_iv_forward_auto_workspace_bytes"):
+        if name not in ("pivot_iv_strerror", "pivot_iv_loss_roundtrip_workspace_bytes"):
             getattr(lib, name).restype = cint
     lib.pivot_iv_loss_roundtrip_workspace_bytes.restype = i64
-    lib.pivot_iv_forward_auto_workspace_bytes.restype = i64
     _lib = lib
     return lib
 
@@ -101,6 +99,19 @@ def _dev(t: Optional[torch.Tensor], name: str, dtype=torch.float64) -> Optional[
     if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.dim() == 1):
         raise PivotError(f"{name}: expected a contiguous 1-D CUDA tensor of {dtype}")
     return t.data_ptr()
+
+
+def _same_len(n: int, **tensors):
+    """Every tensor given must hold exactly n elements (None is skipped)."""
+    for nm, t in tensors.items():
+        if t is not None and t.numel() != n:
+            raise PivotError(f"{nm}: length {t.numel()} != {n}")
+
+
+def _same_device(ref: torch.Tensor, **tensors):
+    for nm, t in tensors.items():
+        if t is not None and t.device != ref.device:
+            raise PivotError(f"{nm}: on {t.device}, expected {ref.device}")
 
 
 def _stream_ptr(stream) -> int:
@@ -157,23 +168,23 @@ def pivot_iv_forward_ex(S_or_F, K, tau, P, flag, kernel: int, r=None, q=None, ou
     return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, False, kernel=kernel)
 
 
-def pivot_iv_forward_auto(S_or_F, K, tau, P, flag, r=None, q=None, out=None, workspace=None, stream=None):
-    """pivot_iv_forward that picks COMPACT or ROWWISE from a sampled probe (n >= 2^23).  Returns (sigma, vega, status,
-    workspace); workspace (int32 CUDA tensor) holds [decision, solved samples, alike pairs, samples] afterwards."""
+def pivot_iv_forward_diag(S_or_F, K, tau, P, flag, r=None, q=None, kernel: int = FWD_AUTO, stream=None):
+    """(sigma, vega, status, zone, s_seed, s_step1): pivot_iv_forward plus the per-row diagnostics of the solve (LBR
+    zone, rational seed, iterate after the first Householder step; total volatilities)."""
     _require_cuda()
     lib = load_library()
     n = S_or_F.numel()
+    _same_len(n, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
     inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P, "P"),
                   _dev(flag, "flag"))
-    if out is None:
-        out = (torch.empty(n, dtype=torch.float64, device=S_or_F.device), torch.empty(n, dtype=torch.float64, device=S_or_F.device),
-               torch.empty(n, dtype=torch.uint8, device=S_or_F.device))
-    if workspace is None:
-        workspace = torch.zeros(int(lib.pivot_iv_forward_auto_workspace_bytes()) // 4, dtype=torch.int32, device=S_or_F.device)
-    with torch.cuda.device(S_or_F.device):
-        _check(lib.pivot_iv_forward_auto(C.byref(inp), n, _dev(out[0], "sigma"), _dev(out[1], "vega"),
-                                         _dev(out[2], "status", torch.uint8), workspace.data_ptr(), _stream_ptr(stream)))
-    return out[0], out[1], out[2], workspace
+    dev = S_or_F.device
+    sigma, vega, s0, s1 = (torch.empty(n, dtype=torch.float64, device=dev) for _ in range(4))
+    status = torch.empty(n, dtype=torch.uint8, device=dev)
+    zone = torch.empty(n, dtype=torch.int8, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib.pivot_iv_forward_diag(C.byref(inp), n, sigma.data_ptr(), vega.data_ptr(), status.data_ptr(),
+                                         zone.data_ptr(), s0.data_ptr(), s1.data_ptr(), int(kernel), _stream_ptr(stream)))
+    return sigma, vega, status, zone, s0, s1
 
 
 def pivot_iv_forward_zones(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None):

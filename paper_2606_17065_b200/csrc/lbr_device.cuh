@@ -1,4 +1,4 @@
-// lbr_device.cuh -- device-side fp64 math for the fused LBR implied-volatility kernel (sm_100a).
+// lbr_device.cuh -- device-side math for the fused LBR implied-volatility kernel (sm_100a).
 //
 // Per-row solver in normalised Black coordinates (eq.(4)-(5); :359-363 A.5 stages 1-5):
 //   x = ln(F/K) reduced to x <= 0, s = sigma sqrt(tau), h = x/s, t = s/2, beta = time value / sqrt(FK),
@@ -9,14 +9,28 @@
 //   z1 <  0:  Wbar = c [erfcx(-z1) + erfcx(z2)]                      W    = b_max/b' - Wbar
 //   t < 0.1:  W    = 2 sum_j w^(2j+1)(h) t^(2j+1)/(2j+1)!,  w(z) = Phi(z)/phi(z) = c erfcx(-z/sqrt2)   (no cancellation)
 // The solve is split in passes so that the kernel can regroup rows in shared memory between them (pivot_iv.cu):
-// lbr_seed_head (boundary point, node, zone), lbr_seed_tail0 / _tail3 (tail seeds) and lbr_refine (Householder(3) steps).
-// Precision tiers: the seed and every Householder step but the last run at "seed grade" (fp32 erfcx, MUFU exp / log,
-// one-Newton reciprocals); the normalisation, ln(beta), the last step and b' at the final s run at full fp64.
+// lbr_seed_head (boundary point, node, zone, middle-zone seeds), lbr_seed_tail0 / _tail3 (tail seeds) and lbr_refine
+// (Householder(3) steps).
+//
+// Precision tiers (template parameter FULL).  FULL = false, the default instantiation: the seed and every Householder
+// step but the last run at "seed grade" -- fp32 erfcx, MUFU exp / log, one-Newton reciprocals, and the rational-cubic
+// interpolants in fp32 on O(1) quantities (the NORMALISED form below); the status decision, the normalisation, ln(beta),
+// the last Householder step and b' at the final s run at full fp64.  FULL = true (PIVOT_FWD_FP64_ONLY): the same
+// formulas with every special function and reciprocal at full fp64, for the A/B that bounds the tiering.
+//
+// Normalised rational cubic.  The Delbourgo-Gregory interpolant is affine invariant, so every seed interpolates
+// Y(u) on [0,1] with Y(0) = 0, Y(1) = 1, end slopes Dl, Dr and end curvature DD (all dimensionless):
+//   Y(u) = u G(u),  G = [u (u + (r - Dr)(1-u)) + (1-u)^2 Dl] / [1 + (r-3) u (1-u)],
+//   r = (DD/2 + Dr - Dl)/(Dr - 1) (curvature fitted at u = 1), floored for monotonicity.
+// In these variables the exponentials of the tail maps f_low, f_up cancel analytically (see lbr_seed_tail0/3), which is
+// what lets the interpolants run in fp32 for every |x| <= 693.
+//
 // exp / log / log1p / erfcx / reciprocals are this file's own, with coefficients in constant memory (gen_coeffs.py):
 // no slow paths, no 64-bit immediates.  See DESIGN.md section 5.
 // This file shares nothing with oracle/ (the CPU checker).
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 #include "coeffs.cuh"
@@ -31,25 +45,27 @@ __constant__ double kSqrtPiOver2 = 1.2533141373155002512;      // sqrt(pi/2)
 __constant__ double kSqrt2Pi = 2.5066282746310005024;          // sqrt(2 pi)
 __constant__ double kPhi0 = 0.39894228040143267794;            // 1/sqrt(2 pi)
 __constant__ double kLnPhi0 = -0.91893853320467274178;         // ln(1/sqrt(2 pi))
-__constant__ double kSqrt3 = 1.7320508075688772935;            // sqrt(3)
+__constant__ double kTwoThirdsLnPhi0 = -0.61262568880311516119;  // (2/3) ln(1/sqrt(2 pi))
 __constant__ double kInvSqrt3 = 0.57735026918962576451;        // 1/sqrt(3)
-__constant__ double kTwoPi = 6.2831853071795864769;            // 2 pi
-__constant__ double kTwoPiOver3Sqrt3 = 1.2091995761561452337;  // 2 pi / (3 sqrt 3)
-__constant__ double kPiOver6 = 0.52359877559829887308;         // pi/6
 __constant__ double kLog2e = 1.4426950408889634074;            // 1/ln 2
 __constant__ double kLn2 = 0.69314718055994530942;             // ln 2 (nearest double)
 __constant__ double kLn2Lo = 2.3190468138462995584e-17;        // ln 2 - (double)ln 2
 __constant__ double kSmallT = 0.1;                              // series / erfcx switch-over
 __constant__ double kSqrt2m1 = 0.41421356237309504880;         // sqrt(2) - 1
-__constant__ double kEightSqrt3 = 13.856406460551018348;       // 8 sqrt 3
 __constant__ double kSeriesC[5] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0};
+__constant__ double kNinvCut = -1.0651;                         // ln 0.345: domain of the Phi^-1 tail fit
 
 enum : int { KIND_LOWER = 0, KIND_LINEAR = 1, KIND_UPPER = 2 };
 
-__device__ __forceinline__ bool is_fin(double v) { return fabs(v) < __longlong_as_double(0x7ff0000000000000LL); }
+__device__ __forceinline__ int hi32(double v) { return __double2hiint(v); }
+__device__ __forceinline__ int lo32(double v) { return __double2loint(v); }
+__device__ __forceinline__ bool is_fin(double v) { return (hi32(v) & 0x7fffffff) < 0x7ff00000; }   // not NaN, not +-inf
 // 0 < v < inf (false for NaN): two fp64 compares
 __device__ __forceinline__ bool pos_fin(double v) { return v > 0.0 && v < __longlong_as_double(0x7ff0000000000000LL); }
 __device__ __forceinline__ double canonical_nan() { return __longlong_as_double(0x7ff8000000000000LL); }
+// max / min of two ordinary numbers (no NaN propagation rules to honour: one compare, one select)
+__device__ __forceinline__ double dmax_nn(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double dmin_nn(double a, double b) { return a < b ? a : b; }
 
 // 1/x from MUFU.RCP64H (about 20 bits, full fp64 exponent range, no slow path) plus Newton steps.
 __device__ __forceinline__ double rcp_raw(double x) {
@@ -67,13 +83,13 @@ __device__ __forceinline__ double rcp_nr2(double x) {  // relative error ~1 ulp
   r = fma(r, fma(-x, r, 1.0), r);
   return r;
 }
-__device__ __forceinline__ double rcp_pos(double x) { return rcp_nr2(x); }
 // a/b to ~1 ulp (b normal, finite, non-zero)
 __device__ __forceinline__ double div_fast(double a, double b) {
   const double r = rcp_nr2(b);
   const double q = a * r;
   return fma(fma(-b, q, a), r, q);
 }
+__device__ __forceinline__ float rcpf(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 
 // exp(a), |a| < ~745; error ~1 ulp.  n = rint(a log2 e) through the 1.5*2^52 shift, Cody-Waite reduction by fma,
 // degree-11 polynomial (coeffs.cuh), exponent add.
@@ -137,7 +153,7 @@ __device__ __forceinline__ double log1p_fast(double q) {
 // erfcx(z1), erfcx(z2) for z1, z2 >= 0:  erfcx(z) = (2C/(z+C)) Q((z-C)/(z+C)), one shared reciprocal.
 __device__ __forceinline__ void erfcx_pair(double z1, double z2, double& e1, double& e2) {
   const double d1 = z1 + kErfcxC, d2 = z2 + kErfcxC;
-  const double r12 = rcp_pos(d1 * d2);
+  const double r12 = rcp_nr2(d1 * d2);
   const double r1 = r12 * d2, r2 = r12 * d1;
   const double y1 = fma(-2.0 * kErfcxC, r1, 1.0), y2 = fma(-2.0 * kErfcxC, r2, 1.0);
   double q1 = kErfcxQ[kErfcxN], q2 = kErfcxQ[kErfcxN];
@@ -150,7 +166,17 @@ __device__ __forceinline__ void erfcx_pair(double z1, double z2, double& e1, dou
   e2 = (2.0 * kErfcxC) * r2 * q2;
 }
 
-// ---- fp32-grade helpers for the seeds (relative error ~1e-6; results carried as double for range) ----
+// erfcx(z), z >= 0 (single evaluation, same polynomial as erfcx_pair)
+__device__ __forceinline__ double erfcx_one(double z) {
+  const double r = rcp_nr2(z + kErfcxC);
+  const double y = fma(-2.0 * kErfcxC, r, 1.0);
+  double q = kErfcxQ[kErfcxN];
+#pragma unroll
+  for (int k = kErfcxN - 1; k >= 0; --k) q = fma(q, y, kErfcxQ[k]);
+  return (2.0 * kErfcxC) * r * q;
+}
+
+// ---- fp32-grade helpers for the seeds (relative error ~1e-6; results carried as double where the range needs it) ----
 __device__ __forceinline__ float ex2_approx(float f) { float r; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(f)); return r; }
 __device__ __forceinline__ float lg2_approx(float f) { float r; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(f)); return r; }
 
@@ -162,6 +188,9 @@ __device__ __forceinline__ double exp_seed(double a) {
   const int e = (int)n;
   return (double)m * __hiloint2double((e + 1023) << 20, 0);
 }
+// exp(a) for a float in [-87, 87]
+__device__ __forceinline__ float expf_seed(float a) { return ex2_approx(a * 1.4426950408889634f); }
+__device__ __forceinline__ float logf_seed(float v) { return lg2_approx(v) * 0.6931471805599453f; }
 
 // ln(v) for v > 0, absolute error ~1e-7 * max(1, |ln v|)
 __device__ __forceinline__ double log_seed(double v) {
@@ -175,8 +204,7 @@ __device__ __forceinline__ double log_seed(double v) {
 
 // erfcx(z), z >= 0, fp32
 __device__ __forceinline__ float erfcx_seed(float z) {
-  float r;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(z + kErfcxCf));
+  const float r = rcpf(z + kErfcxCf);
   const float y = fmaf(-2.0f * kErfcxCf, r, 1.0f);
   float q = kErfcxQf[kErfcxNf];
 #pragma unroll
@@ -185,24 +213,24 @@ __device__ __forceinline__ float erfcx_seed(float z) {
 }
 
 // -Phi^-1(p) from lnp = ln p, p <= 0.345: u = sqrt(-2 ln p), z = u - R(1/(1+u)); relative error ~2e-5
-__device__ __forceinline__ double ninv_tail_seed(double lnp) {
-  const float u = sqrtf(__double2float_rn(-2.0 * lnp));
-  float w;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(w) : "f"(1.0f + u));
+__device__ __forceinline__ float ninv_tail_seed(float lnp) {
+  const float u = sqrtf(-2.0f * lnp);
+  const float w = rcpf(1.0f + u);
   float R = kNinvR[kNinvN];
 #pragma unroll
   for (int k = kNinvN - 1; k >= 0; --k) R = fmaf(R, w, kNinvR[k]);
-  return (double)(u - R);
+  return u - R;
 }
-
-// erfcx(z), z >= 0 (single evaluation, same polynomial as erfcx_pair)
-__device__ __forceinline__ double erfcx_one(double z) {
-  const double r = rcp_nr2(z + kErfcxC);
-  const double y = fma(-2.0 * kErfcxC, r, 1.0);
-  double q = kErfcxQ[kErfcxN];
-#pragma unroll
-  for (int k = kErfcxN - 1; k >= 0; --k) q = fma(q, y, kErfcxQ[k]);
-  return (2.0 * kErfcxC) * r * q;
+// ... refined at full fp64 by two Newton steps on ln Phi(-z) = ln(erfcx(z/sqrt2)/2) - z^2/2 (FULL instantiation only)
+__device__ __forceinline__ double ninv_tail_full(double lnp) {
+  double z = (double)ninv_tail_seed(__double2float_rn(lnp));
+#pragma unroll 1
+  for (int it = 0; it < 2; ++it) {
+    const double e = erfcx_one(z * kInvSqrt2);
+    const double f = log_fast(0.5 * e) - 0.5 * z * z - lnp;
+    z = fma(f, kSqrtPiOver2 * e, z);   // z - f/f',  f' = -1/(c erfcx(z/sqrt2))
+  }
+  return z;
 }
 
 // sqrt(v), v >= 0, relative error ~1e-12 (MUFU.RSQ64H + one Newton step); seeds only
@@ -211,6 +239,28 @@ __device__ __forceinline__ double sqrt_nr1(double v) {
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(v));
   y = y * fma(-0.5 * v, y * y, 1.5);
   return (v > 0.0) ? v * y : 0.0;
+}
+
+// sqrt(v) and 1/sqrt(v), v > 0 normal, ~1 ulp, no slow path: MUFU.RSQ64H + two Newton steps + one residual correction
+__device__ __forceinline__ double sqrt_nr2(double v, double& rinv) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(v));
+  const double hv = -0.5 * v;
+  y = y * fma(hv, y * y, 1.5);
+  y = y * fma(hv, y * y, 1.5);
+  const double s = v * y;
+  rinv = y;
+  return fma(fma(-s, s, v), 0.5 * y, s);
+}
+
+__device__ __forceinline__ double sqrt_nr2(double v) { double r; return sqrt_nr2(v, r); }
+
+// grade-dependent primitives
+template <bool FULL> __device__ __forceinline__ double g_rcp(double x) { return FULL ? rcp_nr2(x) : rcp_nr1(x); }
+template <bool FULL> __device__ __forceinline__ double g_exp(double a) { return FULL ? exp_fast(a) : exp_seed(a); }
+template <bool FULL> __device__ __forceinline__ double g_log(double v) { return FULL ? log_fast(v) : log_seed(v); }
+template <bool FULL> __device__ __forceinline__ double g_erfcx(double z) {
+  return FULL ? erfcx_one(z) : (double)erfcx_seed(__double2float_rn(z));
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -276,42 +326,38 @@ __device__ __forceinline__ WEval eval_W(double x, double s) {
   return w;
 }
 
-// sqrt(v), v > 0 normal, ~1 ulp, no slow path: MUFU.RSQ64H + two Newton steps + one residual correction
-__device__ __forceinline__ double sqrt_nr2(double v) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(v));
-  y = y * fma(-0.5 * v, y * y, 1.5);
-  y = y * fma(-0.5 * v, y * y, 1.5);
-  const double s = v * y;
-  return fma(fma(-s, s, v), 0.5 * y, s);
+// ---------------------------------------------------------------------------------------------------------------
+// Normalised rational cubic (header comment): R = float at seed grade, double in the FULL instantiation.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename R> __device__ __forceinline__ R r_rcp(R x);
+template <> __device__ __forceinline__ float r_rcp<float>(float x) { return rcpf(x); }
+template <> __device__ __forceinline__ double r_rcp<double>(double x) { return rcp_nr2(x); }
+template <typename R> __device__ __forceinline__ R r_max(R a, R b) { return a > b ? a : b; }
+template <> __device__ __forceinline__ float r_max<float>(float a, float b) { return fmaxf(a, b); }
+template <typename R> __device__ __forceinline__ R r_abs(R a) { return a < R(0) ? -a : a; }
+template <> __device__ __forceinline__ float r_abs<float>(float a) { return fabsf(a); }
+template <> __device__ __forceinline__ double r_abs<double>(double a) { return fabs(a); }
+
+// control parameter: curvature DD fitted at u = 1; floored by the monotonicity / convexity bounds
+// (Delta = 1 in these variables); +inf = linear interpolant
+template <typename R>
+__device__ __forceinline__ R rcn_control(R Dl, R Dr, R DD) {
+  const R dR = Dr - R(1), dL = R(1) - Dl, span = Dr - Dl;
+  const R rR = r_rcp<R>(dR), rL = r_rcp<R>(dL);
+  R r = fma(R(0.5), DD, span) * rR;
+  R rmin = r_max<R>(R(-0.999), Dl + Dr);
+  if (dR != R(0)) rmin = r_max<R>(rmin, r_abs<R>(span * rR));
+  if (dL != R(0)) rmin = r_max<R>(rmin, r_abs<R>(span * rL));
+  if (dR == R(0)) r = R(3e38);
+  return (r > rmin) ? r : rmin;     // a NaN r falls to rmin
 }
 
-// Rational cubic on [0,1] (Delbourgo-Gregory form), H = interval width, u and omu = 1-u both supplied.
-// Seed-grade arithmetic: reciprocals carry ~1e-12.
-__device__ __forceinline__ double rc_eval(double u, double omu, double H, double yl, double yr, double dl, double dr,
-                                          double r) {
-  if (!(r < 1e300)) return fma(yr, u, yl * omu);
-  const double c2 = fma(r, yr, -H * dr), c1 = fma(r, yl, H * dl);
-  const double num = fma(u * u, fma(yr, u, c2 * omu), omu * omu * fma(c1, u, yl * omu));
-  return num * rcp_nr1(fma(r - 3.0, u * omu, 1.0));
-}
-
-// control parameter: fit the second derivative `dd` at the left (side = 0) or right (side = 1) end, floored by the
-// monotonicity / convexity bounds.  rH = 1/H.
-__device__ __forceinline__ double rc_control(int side, double H, double rH, double yl, double yr, double dl, double dr,
-                                             double dd) {
-  const double Delta = (yr - yl) * rH;
-  const double dR = dr - Delta, dL = Delta - dl;
-  const double rR = rcp_nr1(dR), rL = rcp_nr1(dL), rD = rcp_nr1(Delta);
-  const double span = dr - dl;
-  const double den = side ? dR : dL;
-  double r = fma(0.5 * H, dd, span) * (side ? rR : rL);
-  double rmin = -1.0 + 1e-9;
-  if (Delta != 0.0) rmin = fmax(rmin, (dl + dr) * rD);
-  if (dR != 0.0) rmin = fmax(rmin, fabs(span * rR));
-  if (dL != 0.0) rmin = fmax(rmin, fabs(span * rL));
-  if (den == 0.0) r = __longlong_as_double(0x7ff0000000000000LL);
-  return (r > rmin) ? r : rmin;
+// G(u) = Y(u)/u
+template <typename R>
+__device__ __forceinline__ R rcn_G(R u, R omu, R Dl, R Dr, R r) {
+  if (!(r < R(1e30))) return R(1);
+  const R num = fma(u, fma(r - Dr, omu, u), omu * omu * Dl);
+  return num * r_rcp<R>(fma(r - R(3), u * omu, R(1)));
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -325,15 +371,22 @@ __device__ __forceinline__ double rc_control(int side, double H, double rH, doub
 //        KIND_LOWER : p1 = ln beta,          p2 unused       g = 1/ln b - 1/ln beta
 //        KIND_LINEAR: p1 = beta,             p2 = bbar       g = b - beta
 //        KIND_UPPER : p1 = ln(b_max - beta), p2 unused       g = ln((b_max - beta)/(b_max - b))
-// Everything here only has to deliver a seed good to ~1e-3 (Householder(3) is fourth order), so reciprocals and
-// square roots carry ~1e-12 and the tail maps use fp32-grade exp / log / erfcx / Phi^-1 on MUFU.
 // ---------------------------------------------------------------------------------------------------------------
 struct SeedHead {
-  int zone;        // 0: tail pending, v = (x, s_n, b_n, beta);  3: tail pending, v = (x, s_n, b_n, bbar);
-                   // 1, 2: finished, v = (x, s0, beta, bbar)
+  int zone;        // 0: tail pending, v = (x, s_n, beta, pack(W_n, beta/b_n));  3: tail pending, v = (x, s_n, bbar,
+                   // pack(Wbar_n, bbar/bbar_n));  1, 2: finished, v = (x, s0, beta, bbar)
   double v0, v1, v2, v3;
 };
 
+__device__ __forceinline__ double pack2f(float a, float b) {
+  return __hiloint2double(__float_as_int(b), __float_as_int(a));
+}
+__device__ __forceinline__ void unpack2f(double p, float& a, float& b) {
+  a = __int_as_float(__double2loint(p));
+  b = __int_as_float(__double2hiint(p));
+}
+
+template <bool FULL>
 __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, double bbar, double bmax) {
   SeedHead o;
   const double x = -log1p_fast(qrel);
@@ -347,7 +400,7 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   //   s_l = s_c (t w0 - t^2 w3/6 - t^4 w5/120 - t^6 w7/5040),  w(.) at h = -t, w0 = c erfcx(t/sqrt2)
   const double tc = 0.5 * sc;
   const bool small_c = tc < kSmallT;
-  const double ec = (double)erfcx_seed(__double2float_rn(small_c ? tc * kInvSqrt2 : sc * kInvSqrt2));   // seed grade (2e-7)
+  const double ec = g_erfcx<FULL>((small_c ? tc : sc) * kInvSqrt2);
   double Wc, sl;
   if (small_c) {
     const double w0 = kSqrtPiOver2 * ec;
@@ -366,33 +419,51 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
     Wc = kSqrtPiOver2 * (1.0 - ec);
     sl = sc - Wc;
   }
+  const double Wbc = kSqrt2Pi - Wc;           // (b_max - b_c)/b'(s_c)
   const double bc = vc * Wc;
-  const double su = sc + (kSqrt2Pi - Wc);     // ... and the tangent hits b_max at s_u
   const bool lower = beta < bc;
   o.v2 = beta; o.v3 = bbar;
-  if (lower && !(sl > 0.0)) {  // rounding guard, |x| below ~1e-30: linear seed
+  if (lower && !(sl > 1e-30)) {  // rounding / fp32-range guard, |x| below ~1e-30: linear seed
     o.zone = 1;
     o.v1 = sc * beta * rcp_nr1(bc);
     return o;
   }
-  const double sn = lower ? sl : su;
-  const WEval w = eval_W<true>(x, sn);
-  const double vn = kPhi0 * exp_seed(-w.E);  // b'(s_n), seed grade
-  const double bn = w.have_W ? w.Wd * vn : fma(-w.Wd, vn, bmax);
+  const double sn = lower ? sl : sc + Wbc;    // s_l, or s_u where the tangent at the inflection point hits b_max
+  const WEval w = eval_W<!FULL>(x, sn);
+  const double vn = kPhi0 * g_exp<FULL>(-w.E);  // b'(s_n)
+  const double wv = w.Wd * vn;
+  const double bn = w.have_W ? wv : bmax - wv;       // b(s_n)
+  const double bbn = w.have_W ? bmax - wv : wv;      // b_max - b(s_n)
   if (lower ? (beta < bn) : (beta > bn)) {   // a tail: hand the node over
+    // W_n (lower) or Wbar_n (upper), and the interpolation abscissa beta/b_n or bbar/bbar_n, as floats
+    const double den = lower ? bn : bbn;
+    const double rden = g_rcp<FULL>(den);
+    const double Wn = (lower == w.have_W) ? w.Wd : den * g_rcp<FULL>(vn);
     o.zone = lower ? 0 : 3;
-    o.v1 = sn; o.v2 = bn; o.v3 = lower ? beta : bbar;
+    o.v1 = sn;
+    o.v2 = lower ? beta : bbar;
+    o.v3 = pack2f(__double2float_rn(Wn), __double2float_rn((lower ? beta : bbar) * rden));
     return o;
   }
-  // zones 1 and 2: s(beta) between the node and the inflection point, s'' = 0 at the inflection point
+  // zones 1 and 2: s(beta) from the node (u = 0) to the inflection point (u = 1), s'' = 0 at the inflection point.
+  // With kappa = b'(s_c)/b'(s_n) = exp(E_n - |x|/2) and rho = b_n/b_c (lower) or (b_max-b_n)/(b_max-b_c) (upper):
+  //   Dr = 1 - rho,  Dl = kappa (1 - rho),  DD = 0.
+  typedef typename std::conditional<FULL, double, float>::type R;
   o.zone = lower ? 1 : 2;
-  const double inv_vn = rcp_nr1(vn), rvc = kSqrt2Pi * rcp_nr1(bmax);
-  const double xl = lower ? bn : bc, xr = lower ? bc : bn;
-  const double yl = lower ? sn : sc, yr = lower ? sc : sn;
-  const double dl = lower ? inv_vn : rvc, dr = lower ? rvc : inv_vn;
-  const double H = xr - xl, rH = rcp_nr1(H);
-  const double r = rc_control(lower ? 1 : 0, H, rH, yl, yr, dl, dr, 0.0);
-  const double s = rc_eval((beta - xl) * rH, (xr - beta) * rH, H, yl, yr, dl, dr, r);
+  const double bbc = vc * Wbc;
+  const double rho = (lower ? bn : bbn) * g_rcp<FULL>(lower ? bc : bbc);
+  const double kappa = vc * g_rcp<FULL>(vn);
+  const double H = bc - bn, rH = g_rcp<FULL>(H);
+  const R u = (R)((beta - bn) * rH), omu = (R)((bc - beta) * rH);
+  const R Dr = (R)(1.0 - rho);
+  const double Dld = kappa * (1.0 - rho);
+  const R Dl = (R)dmin_nn(Dld, 1e30);
+  const R r = rcn_control<R>(Dl, Dr, R(0));
+  // evaluated from the end with the SMALLER s (the node s_l below the inflection point, the inflection point itself
+  // above it), so that s keeps its relative accuracy when s_c -> 0 (|x| -> 0): the interpolant is reversal invariant
+  const R wq = lower ? u : omu, omw = lower ? omu : u;
+  const R Y = wq * rcn_G<R>(wq, omw, lower ? Dl : Dr, lower ? Dr : Dl, r);
+  const double s = fma(fabs(sc - sn), (double)Y, lower ? sn : sc);
   o.v1 = (s > 0.0 && is_fin(s)) ? s : sc;   // a failed interpolant falls back to the inflection point
   return o;
 }
@@ -402,70 +473,102 @@ struct Seed {
   int kind, zone;
 };
 
-// zone 0: f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l]
-__device__ __forceinline__ Seed lbr_seed_tail0(double x, double sn, double bn, double beta) {
+// zone 0: f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l].
+// In normalised variables (u = beta/b_l, Y = f/f_low(s_l)) with q = |x|/s_l = sqrt3 z, omega = W_l/s_l,
+// Ym = Phi(-z)/phi(z) (Mills ratio), m = 1/Ym, every exponential of f', f'' cancels against b(s_l) = W_l phi0 e^{-E}:
+//   Dl = 3 sqrt3 omega m^3 e^{-s_l^2/8} / q,   Dr = sqrt3 q omega m,
+//   DD = (sqrt3/12) q [(3 (s_l^2 - 8) - 8 q^2) Ym + 8 sqrt3 q] (omega m)^2,
+// and  ln Phi(-z(beta)) = ln Ym + (2/3) ln phi0 + s_l^2/24 + (ln beta - ln W_l + ln G(u))/3.
+template <bool FULL>
+__device__ __forceinline__ Seed lbr_seed_tail0(double x, double sn, double beta, double packed) {
+  typedef typename std::conditional<FULL, double, float>::type R;
   const double a = -x;
-  const double rs = rcp_nr1(sn);
-  const double z = a * rs * kInvSqrt3;
-  const double Y = kSqrtPiOver2 * (double)erfcx_seed(__double2float_rn(z * kInvSqrt2));  // Phi(-z)/phi(z)
-  const double Yp = Y * kPhi0;
-  const double A = exp_seed(-0.5 * z * z), B = exp_seed(0.125 * sn * sn);
-  const double Phz = Yp * A;
-  const double sn2 = sn * sn;
-  const double rA = rcp_nr1(A);
-  const double yr = kTwoPiOver3Sqrt3 * a * Phz * Phz * Phz;
-  const double dr = kTwoPi * z * z * Yp * Yp * B;
-  const double dd = kPiOver6 * (z * z * rs * rs * rs) * Yp *
-                    fma(fma(3.0 * sn2, sn2 - 8.0, -8.0 * a * a), Y, kEightSqrt3 * sn * a) * (B * B) * (rA * rA * rA);
-  const double H = bn, rH = rcp_nr1(bn);
-  const double r = rc_control(1, H, rH, 0.0, yr, 1.0, dr, dd);
-  const double u = beta * rH, omu = (bn - beta) * rH;
-  double y = rc_eval(u, omu, H, 0.0, yr, 1.0, dr, r);
-  if (!(y > 0.0)) y = fma(yr, u, bn * omu) * u;
-  // Phi(-z) = (f/c)^{1/3}  ->  ln p = ln(f/c)/3
-  const double lnp = fmin(log_seed(y * rcp_nr1(kTwoPiOver3Sqrt3 * a)) * (1.0 / 3.0), -1.0651);
-  double s = a * kInvSqrt3 * rcp_nr1(ninv_tail_seed(lnp));
-  if (!(s > 0.0) || !is_fin(s)) s = sn;
   Seed o;
-  o.x = x; o.s = s; o.zone = 0;
-  o.kind = KIND_LOWER; o.p1 = log_fast(beta); o.p2 = 0.0;   // b_max = e^{x/2} is rebuilt by lbr_refine if ever needed
+  o.x = x; o.zone = 0; o.kind = KIND_LOWER; o.p2 = 0.0;
+  o.p1 = log_fast(beta);     // ln beta: the objective's target, full precision
+  R Wn, u;
+  if (FULL) {
+    const WEval w = eval_W<false>(x, sn);        // have_W holds at s_l (z1 > 0 below the inflection point)
+    const double bn = w.Wd * kPhi0 * exp_fast(-w.E);
+    Wn = (R)w.Wd; u = (R)(beta * rcp_nr2(bn));
+  } else {
+    float fw, fu; unpack2f(packed, fw, fu); Wn = (R)fw; u = (R)fu;
+  }
+  const R snr = (R)sn, ar = (R)a;
+  const R rs = r_rcp<R>(snr);
+  const R q = ar * rs;
+  const R Ym = (R)kSqrtPiOver2 * (R)g_erfcx<FULL>((double)(q * R(0.40824829046386301637)));   // z/sqrt2 = q/sqrt6
+  const R m = r_rcp<R>(Ym);
+  const R om = Wn * rs * m;
+  const R sn2 = snr * snr;
+  const R iB = FULL ? (R)exp_fast(-0.125 * (double)sn2) : (R)expf_seed(-0.125f * (float)sn2);
+  const R Dr = R(1.7320508075688772935) * q * om;
+  const R DD = R(0.14433756729740644113) * q * om * om *
+               fma(fma(R(3), sn2, fma(R(-8), q * q, R(-24))), Ym, R(13.856406460551018348) * q);
+  const R Dl = R(5.1961524227066318806) * om * m * m * iB * (snr * r_rcp<R>(ar));
+  const R r = rcn_control<R>(Dl, Dr, DD);
+  R G = rcn_G<R>(u, R(1) - u, Dl, Dr, r);
+  if (!(G > R(0))) G = fma(Dl, R(1) - u, u);
+  const double lnWG = FULL ? log_fast((double)G * rcp_nr2((double)Wn)) : (double)logf_seed((float)G * rcpf((float)Wn));
+  const double lnY = FULL ? log_fast((double)Ym) : (double)logf_seed((float)Ym);
+  const double lnp = dmin_nn(lnY + kTwoThirdsLnPhi0 + (double)sn2 * (1.0 / 24.0) + (o.p1 + lnWG) * (1.0 / 3.0), kNinvCut);
+  const double zz = FULL ? ninv_tail_full(lnp) : (double)ninv_tail_seed(__double2float_rn(lnp));
+  double s = a * kInvSqrt3 * g_rcp<FULL>(zz);
+  if (!(s > 0.0) || !is_fin(s)) s = sn;
+  o.s = s;
   return o;
 }
 
-// zone 3: f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max]
-__device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bn, double bbar) {
+// zone 3: f_up(s) = Phi(-s/2) as a function of beta on [b_u, b_max].  Interpolated from the b_max end (v = 0, f = 0) to
+// the node (v = 1): v = bbar/bbar_u, Ybar = f/f_up(s_u) = v G(v), with h = x/s_u, e = erfcx(s_u/(2 sqrt2)):
+//   slope at the node  Dn = Wbar_u phi0 / e,   slope at b_max  Dm = Dn e^{-h^2/2},
+//   curvature at the node  DDn = 2 c (h^2/s_u) Wbar_u phi0 Dn,
+// and  ln f = ln bbar + h^2/2 + ln(G(v) / (2 Dn)).
+template <bool FULL>
+__device__ __forceinline__ Seed lbr_seed_tail3(double x, double sn, double bbar, double packed) {
+  typedef typename std::conditional<FULL, double, float>::type R;
   const double bmax = exp_fast(0.5 * x);   // e^{x/2} (the handover carries four words: beta = b_max - bbar)
-  const double beta = bmax - bbar;
-  const double rs = rcp_nr1(sn);
-  const double h = x * rs;
-  const double hu2 = h * h;
-  const double tn = 0.5 * sn;
-  const double A = exp_seed(0.5 * hu2), B = exp_seed(0.125 * sn * sn);
-  const double yl = 0.5 * (double)erfcx_seed(__double2float_rn(tn * kInvSqrt2)) * rcp_nr1(B);  // Phi(-t)
-  const double dl = -0.5 * A;
-  const double dd = kSqrtPiOver2 * (A * A) * B * hu2 * rs;
-  const double H = bmax - bn, rH = rcp_nr1(H);
-  const double r = rc_control(0, H, rH, yl, 0.0, dl, -0.5, dd);
-  const double u = (beta - bn) * rH, omu = bbar * rH;
-  double y = rc_eval(u, omu, H, yl, 0.0, dl, -0.5, r);
-  if (!(y > 0.0)) y = fma(yl, omu, 0.5 * H * u) * omu;
-  double s = 2.0 * ninv_tail_seed(fmin(log_seed(y), -1.0651));
-  if (!(s > 0.0) || !is_fin(s)) s = sn;
   Seed o;
-  o.x = x; o.s = s; o.zone = 3;
-  if (bbar < 0.5 * bmax) {
-    o.kind = KIND_UPPER; o.p1 = log_fast(bbar); o.p2 = 0.0;
+  o.x = x; o.zone = 3;
+  const bool upper = bbar < 0.5 * bmax;
+  double lnbbar;
+  if (upper) {
+    o.kind = KIND_UPPER; o.p1 = log_fast(bbar); o.p2 = 0.0; lnbbar = o.p1;
   } else {
-    o.kind = KIND_LINEAR; o.p1 = beta; o.p2 = bbar;
+    o.kind = KIND_LINEAR; o.p1 = bmax - bbar; o.p2 = bbar; lnbbar = g_log<FULL>(bbar);
   }
+  const double rs = g_rcp<FULL>(sn);
+  const double h = x * rs;
+  const double hh2 = 0.5 * h * h;
+  R Wbn, v;
+  if (FULL) {
+    const WEval w = eval_W<false>(x, sn);        // z1 < 0 above the inflection point: Wd = Wbar
+    const double bbn = w.Wd * kPhi0 * exp_fast(-w.E);
+    Wbn = (R)w.Wd; v = (R)(bbar * rcp_nr2(bbn));
+  } else {
+    float fw, fv; unpack2f(packed, fw, fv); Wbn = (R)fw; v = (R)fv;
+  }
+  const R e = (R)g_erfcx<FULL>(0.5 * sn * kInvSqrt2);
+  const R Dn = Wbn * (R)kPhi0 * r_rcp<R>(e);
+  const R Dm = Dn * (R)g_exp<FULL>(-hh2);
+  const R DDn = R(5.0132565492620010048) * (R)(hh2 * rs) * Wbn * (R)kPhi0 * Dn;     // 2c h^2/s = 4c (h^2/2)/s
+  const R r = rcn_control<R>(Dm, Dn, DDn);
+  R G = rcn_G<R>(v, R(1) - v, Dm, Dn, r);
+  if (!(G > R(0))) G = fma(Dm, R(1) - v, v);
+  const double lnG = FULL ? log_fast((double)G * rcp_nr2(2.0 * (double)Dn)) : (double)logf_seed((float)G * rcpf(2.0f * (float)Dn));
+  const double lnf = dmin_nn(lnbbar + hh2 + lnG, kNinvCut);
+  double s = 2.0 * (FULL ? ninv_tail_full(lnf) : (double)ninv_tail_seed(__double2float_rn(lnf)));
+  if (!(s > 0.0) || !is_fin(s)) s = sn;
+  o.s = s;
   return o;
 }
 
 // one-call form (row-per-thread kernel)
+template <bool FULL>
 __device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, double bmax) {
-  const SeedHead hd = lbr_seed_head(qrel, beta, bbar, bmax);
-  if (hd.zone == 0) return lbr_seed_tail0(hd.v0, hd.v1, hd.v2, hd.v3);
-  if (hd.zone == 3) return lbr_seed_tail3(hd.v0, hd.v1, hd.v2, hd.v3);
+  const SeedHead hd = lbr_seed_head<FULL>(qrel, beta, bbar, bmax);
+  if (hd.zone == 0) return lbr_seed_tail0<FULL>(hd.v0, hd.v1, hd.v2, hd.v3);
+  if (hd.zone == 3) return lbr_seed_tail3<FULL>(hd.v0, hd.v1, hd.v2, hd.v3);
   Seed o;
   o.x = hd.v0; o.s = hd.v1; o.p1 = hd.v2; o.p2 = hd.v3; o.kind = KIND_LINEAR; o.zone = hd.zone;
   return o;
@@ -481,6 +584,7 @@ __device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, 
 // ---------------------------------------------------------------------------------------------------------------
 struct NormSolve {
   double s;     // total volatility after NITER Householder steps
+  double s1;    // ... after NITER - 1 steps (diagnostics)
   double vfin;  // b'(x, s) at that s
 };
 
@@ -527,46 +631,51 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
   return s + ds;
 }
 
-template <int NITER>
+template <int NITER, bool FULL>
 __device__ __forceinline__ NormSolve lbr_refine(double x, double s, double p1, double p2, int kind) {
 #pragma unroll 1
-  for (int it = 0; it < NITER - 1; ++it) s = householder_step<true>(x, s, p1, p2, kind);
+  for (int it = 0; it < NITER - 1; ++it) s = householder_step<!FULL>(x, s, p1, p2, kind);
+  NormSolve o;
+  o.s1 = s;
   s = householder_step<false>(x, s, p1, p2, kind);
   const double rs = rcp_nr2(s);
   const double h = x * rs, t = 0.5 * s;
-  NormSolve o;
   o.s = s;
   o.vfin = kPhi0 * exp_fast(-0.5 * fma(h, h, t * t));
   return o;
 }
 
-// one-call form (row-per-thread kernel): seed + refine
-template <int NITER>
-__device__ __forceinline__ NormSolve lbr_solve(double qrel, double beta, double bmax, double bbar, int& zone) {
-  const Seed sd = lbr_seed(qrel, beta, bbar, bmax);
-  zone = sd.zone;
-  return lbr_refine<NITER>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
-}
-
-// Row prelude (Alg.1 l.1 and l.3; A.5 stages 1-2): validity and status for EVERY row, with no division:
+// ---------------------------------------------------------------------------------------------------------------
+// Row prelude (Alg.1 l.1 and l.3; A.5 stages 1-2): validity and status for EVERY row.
+//
+// EXACT form (lbr_prelude_exact; the definition, and the path of unusual rows): only correctly rounded IEEE operations
+// issued through intrinsics, so the decision cannot be contracted into FMAs and is bit-reproducible against any
+// IEEE-754 implementation of the same sequence; no division:
 //   beta = RN(tv / rootFK) < DBL_MIN   <=>   tv * 2^1022 < rootFK     (exact: the scaling is exact, and for doubles
 //   bmax = RN(lo / rootFK) >= 2^-500   <=>   lo * 2^500 >= rootFK      a < b implies a <= b - ulp(b) < b (1 - 2^-53))
-// so the status byte equals the one obtained from the correctly rounded quotients, bit for bit, and rows that leave
-// here (57.8 % of config 1/4) cost no division (a zero numerator would even take the divide's slow path).
-// The status decision uses only correctly rounded IEEE operations issued through intrinsics, so it cannot be
-// contracted into FMAs and is bit-reproducible against any IEEE-754 implementation of the same sequence.
+//
+// FAST form (lbr_prelude): the same decision for the COMMON case, classified on the high words:
+//   F (or S e^{(r-q)tau}), K in [2^-400, 2^400), tau positive normal, P (B) finite, flag = +-1  [, D in [2^-300, 2^300)].
+// Then sqrt(FK) is in [2^-400, 2^400), so  lo 2^500 >= sqrt(FK)  holds and sqrt(FK) is positive finite;  tv <= 0  =>
+// AT_INTRINSIC;  and  tv 2^1022 < sqrt(FK)  is decided from the exponents of tv, F and K except in a band two binades wide
+// around beta = 2^-1022 (kD2Solve / kD2Zero below).  So no square root is needed to decide the status; rows outside the
+// common case, and rows inside that band, take the exact form (status 5 = "rare" asks the caller to do so).  The remaining operations (F-K, U-B, lo-(U-B), B-iota and
+// the comparisons) are the exact form's own, operation for operation, with U = the strike-side bound and O = the other
+// one of (F, K):  iota = max(U - O, 0),  in the money <=> U > O,  lo = O and hi = U when in the money.
+// BSM mode: F = S e^{(r-q)tau}, D = e^{-r tau}, B = P/D with this file's exp_fast / div_fast (<= 1 ulp) on the fast path
+// and CUDA's exp / IEEE division on the exact path (reading 17: each side of the parity uses its own exp).
+// ---------------------------------------------------------------------------------------------------------------
 struct Prelude {
-  double F;       // forward (BSM: S e^{(r-q) tau})
+  double U;       // upper bound of the undiscounted price: F (call) or K (put)
+  double O;       // the other one of (F, K)
   double B;       // undiscounted price (BSM: P / D)
-  double rootFK;  // sqrt(F K)
-  double scale;   // D sqrt(FK): vega = scale * b'(x,s) * sqrt(tau)
-  int status;
-  bool call;
+  double D;       // discount factor (1 in Black-76 mode)
+  int status;     // 0..4; lbr_prelude only: 5 = rare, take lbr_prelude_exact
 };
 
 template <bool BSM>
-__device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau, double r, double q, double P,
-                                               double flag) {
+__device__ __noinline__ Prelude lbr_prelude_exact(double SorF, double K, double tau, double r, double q, double P,
+                                                  double flag) {
   Prelude p;
   bool bad = !pos_fin(SorF) || !pos_fin(K) || !pos_fin(tau) || !is_fin(P) || !(flag == 1.0 || flag == -1.0);
   double F = SorF, D = 1.0, B = P;
@@ -595,67 +704,130 @@ __device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau
   else if (B >= U) st = 2;
   else if (__dmul_rn(tv, 0x1p1022) < rootFK) st = 4;
   p.status = st;
-  p.F = F;
+  p.U = U;
+  p.O = call ? K : F;
   p.B = B;
-  p.rootFK = rootFK;
-  p.scale = BSM ? D * rootFK : rootFK;
-  p.call = call;
+  p.D = D;
   return p;
 }
 
-// Normalised solver inputs of a row that reached the solver (A.5 stage 2).  Quotients by Newton
-// reciprocal + one residual correction (~1 ulp, no slow path): sqrt(FK) lies in [2^-537, 2^512] and b_max in
-// [2^-500, 1], so the MUFU reciprocal seeds never leave the normal range; lo itself is never inverted.
+constexpr unsigned kExpLo400 = (1023u - 400u) << 20;   // high word of 2^-400
+constexpr unsigned kExpSpan800 = 800u << 20;
+constexpr unsigned kExpLo300 = (1023u - 300u) << 20;
+constexpr unsigned kExpSpan600 = 600u << 20;
+// AT_INTRINSIC band on the high words.  With L(v) = hi32(v)/2^20 - 1023:  L(v) <= log2 v <= L(v) + 0.0861 for normal v,
+// and log2 v <= L(v) + 1 for subnormal v.  d2 = hi32(tv) - (hi32(F) + hi32(K))/2 therefore brackets
+// log2(tv / sqrt(FK)) = log2(beta):   d2 >= kD2Solve and tv normal  =>  beta > 2^-1022 (the row solves);
+//                                     d2 <= kD2Zero   =>  beta < 2^-1022 (AT_INTRINSIC);  in between: the exact form decides.
+constexpr int kD2Solve = -(1022 << 20) + (1 << 19);
+constexpr int kD2Zero = -(1023 << 20) - (1 << 19);
+
+template <bool BSM>
+__device__ __forceinline__ Prelude lbr_prelude(double SorF, double K, double tau, double r, double q, double P,
+                                               double flag) {
+  Prelude p;
+  const int hf = hi32(flag), hK = hi32(K);
+  bool common = ((unsigned)(hK - (int)kExpLo400) < kExpSpan800) & ((unsigned)(hi32(tau) - 0x00100000) < 0x7fe00000u) &
+                ((hf & 0x7fffffff) == 0x3ff00000) & (lo32(flag) == 0);
+  double F = SorF, B = P, D = 1.0;
+  if (BSM) {
+    common = common & is_fin(r) & is_fin(q) & ((unsigned)(hi32(SorF) - (int)kExpLo400) < kExpSpan800);
+    F = __dmul_rn(SorF, exp_fast(__dmul_rn(__dsub_rn(r, q), tau)));
+    D = exp_fast(__dmul_rn(-r, tau));
+    common = common & ((unsigned)(hi32(D) - (int)kExpLo300) < kExpSpan600);
+    B = div_fast(P, D);
+  }
+  const int hF = hi32(F);
+  common = common & ((unsigned)(hF - (int)kExpLo400) < kExpSpan800) & is_fin(B);
+  const bool call = hf >= 0;
+  const double U = call ? F : K, O = call ? K : F;
+  const double d = __dsub_rn(U, O);
+  const bool itm = d > 0.0;
+  const double iota = itm ? d : 0.0;
+  const double ub = __dsub_rn(U, B);
+  const bool big = itm & (U > __dadd_rn(O, O));
+  const double tv = big ? __dsub_rn(O, ub) : __dsub_rn(B, iota);
+  const int d2 = hi32(tv) - (int)(((unsigned)hF + (unsigned)hK) >> 1);
+  int st = ((d2 >= kD2Solve) & (hi32(tv) >= 0x00100000)) ? 0 : ((d2 <= kD2Zero) ? 4 : 5);   // the lower bound needs a normal tv
+  st = (tv > 0.0) ? st : 4;
+  st = (B >= U) ? 2 : st;
+  st = (B < iota) ? 1 : st;
+  p.status = common ? st : 5;
+  p.U = U; p.O = O; p.B = B; p.D = D;
+  return p;
+}
+
+// Normalised solver inputs of a row that reached the solver (A.5 stage 2), from (U, O, B) of the prelude.
+// Quotients by reciprocal + one residual correction (~1 ulp, no slow path).  Common rows: sqrt(FK) and 1/sqrt(FK) from
+// MUFU.RSQ64H + Newton (FK in [2^-800, 2^800): normal);  rare rows (flag set by the prelude): the IEEE square root, since
+// FK may be subnormal there, and sqrt(FK) in [2^-537, 2^512].
 struct Norm {
   double qrel;    // (hi - lo)/lo, hi = max(F,K), lo = min(F,K):  x = -log1p(qrel)
   double beta;    // time value / sqrt(FK)
   double bbar;    // (U - B)/sqrt(FK) = b_max - beta, formed without cancellation
   double bmax;    // lo / sqrt(FK) = e^{x/2}
+  double rootFK;  // sqrt(F K)
 };
 
-__device__ __forceinline__ Norm lbr_normalise(double F, double K, double B, double rootFK, bool call) {
+__device__ __forceinline__ Norm lbr_normalise(double U, double O, double B, bool rare) {
   Norm n;
-  const double lo = fmin(F, K), hi = fmax(F, K);
-  const double iota = fmax(call ? __dsub_rn(F, K) : __dsub_rn(K, F), 0.0);
-  const double U = call ? F : K;
-  const double ub = __dsub_rn(U, B), d = __dsub_rn(hi, lo);
-  const double tv = (iota > 0.0 && hi > __dmul_rn(2.0, lo)) ? __dsub_rn(lo, ub) : __dsub_rn(B, iota);  // as in lbr_prelude
-  const double r = rcp_nr2(rootFK);
+  const double d = __dsub_rn(U, O);
+  const bool itm = d > 0.0;
+  const double iota = itm ? d : 0.0;
+  const double ub = __dsub_rn(U, B);
+  const bool big = itm && (U > __dadd_rn(O, O));
+  const double tv = big ? __dsub_rn(O, ub) : __dsub_rn(B, iota);   // as in the prelude
+  const double lo = itm ? O : U, hi = itm ? U : O;
+  const double dabs = fabs(d);
+  const double FK = __dmul_rn(U, O);
+  double r, rl;
+  if (rare) {
+    n.rootFK = __dsqrt_rn(FK);
+    r = rcp_nr2(n.rootFK);
+  } else {
+    n.rootFK = sqrt_nr2(FK, r);
+  }
   double q = lo * r;
-  n.bmax = fma(fma(-rootFK, q, lo), r, q);
+  n.bmax = fma(fma(-n.rootFK, q, lo), r, q);
   q = tv * r;
-  n.beta = fma(fma(-rootFK, q, tv), r, q);
+  n.beta = fma(fma(-n.rootFK, q, tv), r, q);
   q = ub * r;
-  n.bbar = fma(fma(-rootFK, q, ub), r, q);
-  const double rl = r * rcp_nr2(n.bmax);  // ~ 1/lo, formed without inverting lo
-  q = d * rl;
-  n.qrel = fma(fma(-lo, q, d), rl, q);
+  n.bbar = fma(fma(-n.rootFK, q, ub), r, q);
+  if (rare) rl = r * rcp_nr2(n.bmax);   // ~ 1/lo, formed without inverting lo (may be subnormal)
+  else rl = r * r * hi;                 // 1/lo = hi/(lo hi)
+  q = dabs * rl;
+  n.qrel = fma(fma(-lo, q, dabs), rl, q);
   return n;
 }
 
 struct RowOut {
   double sigma, vega;
+  double s0, s1;      // total volatility of the seed and after the first Householder step (diagnostics)
   uint8_t status;
   int8_t zone;
 };
 
 // Full row (Alg.1 l.1-3).  BSM = true: (S,K,tau,r,q,P,flag); false: Black-76 with discount factor 1.
-template <bool BSM, int NITER>
+template <bool BSM, int NITER, bool FULL>
 __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, double r, double q, double P, double flag) {
   RowOut o;
-  const Prelude p = lbr_prelude<BSM>(SorF, K, tau, r, q, P, flag);
+  Prelude p = lbr_prelude<BSM>(SorF, K, tau, r, q, P, flag);
+  const bool rare = p.status == 5;
+  if (rare) p = lbr_prelude_exact<BSM>(SorF, K, tau, r, q, P, flag);
   o.sigma = (p.status == 4) ? 0.0 : canonical_nan();
   o.vega = 0.0;
   o.zone = -1;
+  o.s0 = o.s1 = 0.0;
   o.status = (uint8_t)p.status;
   if (p.status == 0) {
-    int zone;
-    const Norm nm = lbr_normalise(p.F, K, p.B, p.rootFK, p.call);
-    const NormSolve ns = lbr_solve<NITER>(nm.qrel, nm.beta, nm.bmax, nm.bbar, zone);
+    const Norm nm = lbr_normalise(p.U, p.O, p.B, rare);
+    const Seed sd = lbr_seed<FULL>(nm.qrel, nm.beta, nm.bbar, nm.bmax);
+    const NormSolve ns = lbr_refine<NITER, FULL>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
     const double rinv = rsqrt(tau);
     o.sigma = ns.s * rinv;
-    o.vega = p.scale * ns.vfin * (tau * rinv);
-    o.zone = (int8_t)zone;
+    o.vega = (BSM ? p.D * nm.rootFK : nm.rootFK) * ns.vfin * (tau * rinv);
+    o.zone = (int8_t)sd.zone;
+    o.s0 = sd.s; o.s1 = ns.s1;
   }
   return o;
 }

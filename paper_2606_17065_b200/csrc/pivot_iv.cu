@@ -7,6 +7,7 @@
 // No tensor cores: the path is an fp64 transcendental chain, not a contraction.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
@@ -21,86 +22,102 @@ constexpr int kFwdThreads = 128;
 constexpr int kBwdThreads = 256;
 constexpr int kHouseholderSteps = 2;  // north_star: two Householder(3) steps
 
+// optional per-row diagnostics of the forward kernels (pivot_iv_forward_diag): any pointer may be null
+struct DiagOut {
+  int8_t* zone;   // LBR zone 0..3, -1 for rows that never reach the solver
+  double* s0;     // total volatility of the rational seed
+  double* s1;     // ... after the first (seed-grade) Householder step
+};
+
 // ---------------------------------------------------------------------------------------------------------------
 // Forward kernel, one row per thread (PIVOT_FWD_ROWWISE): no shared memory, no barriers; coalesced 8-byte accesses.
 // Best when nearly every row solves and neighbouring rows are alike (option chains in strike order).
 // ---------------------------------------------------------------------------------------------------------------
-template <bool BSM, bool ZONES>
-__device__ __forceinline__ void solve_and_store(int64_t i, double S, double K, double tau, double r, double q, double P,
-                                                double flag, double* __restrict__ sigma, double* __restrict__ vega,
-                                                uint8_t* __restrict__ status, int8_t* __restrict__ zone) {
-  const RowOut o = lbr_row<BSM, kHouseholderSteps>(S, K, tau, r, q, P, flag);
+template <bool BSM, bool DIAG, bool FULL>
+__global__ void __launch_bounds__(kFwdThreads)
+forward_kernel_scalar(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
+                      uint8_t* __restrict__ status, DiagOut dg) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+  const RowOut o = lbr_row<BSM, kHouseholderSteps, FULL>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q,
+                                                         __ldcs(in.P + i), __ldcs(in.flag + i));
   __stcs(sigma + i, o.sigma);
   __stcs(vega + i, o.vega);
   status[i] = o.status;
-  if (ZONES) zone[i] = o.zone;
-}
-
-// SEL = false: one launch covers the rows (grid = ceil(n / 128)).  SEL = true (pivot_iv_forward_auto): small grid-stride
-// grid that first reads the probe's decision and returns at once when the other organisation was chosen.
-template <bool BSM, bool ZONES, bool SEL = false>
-__global__ void __launch_bounds__(kFwdThreads)
-forward_kernel_scalar(pivot_iv_inputs in, int64_t begin, int64_t n, double* __restrict__ sigma,
-                      double* __restrict__ vega, uint8_t* __restrict__ status, int8_t* __restrict__ zone,
-                      const int* __restrict__ sel, int want) {
-  if (SEL) {
-    if (*sel != want) return;
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-      const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
-      solve_and_store<BSM, ZONES>(i, __ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(in.P + i),
-                                  __ldcs(in.flag + i), sigma, vega, status, zone);
-    }
-  } else {
-    const int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
-    solve_and_store<BSM, ZONES>(i, __ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(in.P + i),
-                                __ldcs(in.flag + i), sigma, vega, status, zone);
+  if (DIAG) {
+    if (dg.zone) dg.zone[i] = o.zone;
+    if (dg.s0) dg.s0[i] = o.s0;
+    if (dg.s1) dg.s1[i] = o.s1;
   }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 // Forward kernel, "tile compaction".  A CTA owns a tile of kTileRows consecutive rows.
-//   Phase A  (all rows, coalesced 8-byte loads): prelude -> status, with exact IEEE operations and no division.  Rows
-//            that need the solver are appended to a compact queue in shared memory (one warp prefix scan and one shared
-//            atomic per warp per tile); the others get their final sigma / vega straight away.  For queued rows the
-//            staged output slots carry tau and D sqrt(FK) meanwhile.
-//   Phase B1 (queued rows, DENSE warps): lbr_normalise + lbr_seed_head: x, boundary point, node, zone; the middle zones
-//            get their seed here; rows are regrouped by zone class (warp ballots + three shared counters).
+//   Phase A  (all rows, coalesced 8-byte loads): lbr_prelude -> status, decided on the high words and five exact
+//            subtractions / comparisons; no square root, no division.  Rows that need the solver are appended to a
+//            compact queue (U, O, B) in shared memory (one warp prefix scan and one shared atomic per warp per tile);
+//            the others get their final sigma / vega straight away.  For queued rows the staged sigma slot carries tau
+//            meanwhile (and the vega slot the discount factor in BSM mode).
+//   Phase B1 (queued rows, DENSE warps): lbr_normalise (sqrt(FK) and the four quotients) + lbr_seed_head: x, boundary
+//            point, node, zone; the middle zones get their seed here; rows are regrouped by zone class (warp ballots +
+//            one packed shared counter).
 //   Phase B2 (queued rows, grouped zone 0 / middle / zone 3): the tail seeds (lbr_seed_tail0 / _tail3) fused with the
 //            two Householder(3) steps (lbr_refine); sigma and vega into the staged output slots of the row.
 //   Phase C: the staged sigma, vega and status of the tile are streamed out with coalesced stores.
 // Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); both partitions cost shared-memory traffic only.
-// The ncu capture of the one-row-per-thread kernel (profiles/r1a_*, r1d_ab_*) shows ~11 of 32 lanes active because more
-// than half of config 1/4's rows leave at the validity check; here the solver's warps are full (26.6 of 32).
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
-// RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers) for large n; 1 (256-row tiles) for
-// small n, so that a launch of 65,536 rows still spreads over every SM.
+// RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers) for large n; 1 (256-row
+// tiles) for small n, so that a launch of 65,536 rows still spreads over every SM.
 
 template <int RPT>
 struct TileSmem {
   static constexpr int kTileRows = kTileThreads * RPT;
   double sig[kTileRows];      // phase A: tau (queued rows) or final sigma;  phase B2: final sigma
-  double veg[kTileRows];      // phase A: D sqrt(FK) (queued rows) or 0;      phase B2: final vega
-  double q0[kTileRows];       // compact queue.  after A: F, K, B, sqrt(FK);  after B1: x, s0, p1, p2 (lbr_seed)
+  double veg[kTileRows];      // phase A: D (queued rows, BSM) or 0; phase B1: D sqrt(FK); phase B2: final vega
+  double q0[kTileRows];       // compact queue.  after A: U, O, B;  after B1: the four handover words of lbr_seed_head
   double q1[kTileRows];
   double q2[kTileRows];
   double q3[kTileRows];
-  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = call
+  uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = rare row (exact prelude, IEEE square root)
   uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, finished middle-zone rows from the back
   uint16_t permU[kTileRows];  // ... and zone 3 rows
   uint8_t status[kTileRows];
-  unsigned long long nclass;  // rows per class, three 21-bit fields: zone 0 | zones 1-2 << 21 | zone 3 << 42
+  unsigned n01;               // rows per class: zone 0 | zones 1-2 << 16  (one native 32-bit shared atomic per warp)
+  unsigned n2;                // ... zone 3
   int count;                  // queued rows
 };
 
-template <bool BSM, bool ZONES, int RPT, bool SEL = false>
-__global__ void __launch_bounds__(kTileThreads, BSM ? 3 : 4)
+// A row the fast prelude could not classify (status 5): lbr_prelude_exact on its inputs, staged outputs, and its own
+// queue slot (flagged: lbr_normalise then takes the IEEE square root).
+template <bool BSM, bool DIAG, int RPT>
+__device__ __noinline__ void tile_rare_row(pivot_iv_inputs in, int64_t base, int p, TileSmem<RPT>& sm, DiagOut dg) {
+  const int64_t i = base + p;
+  const double tau = in.tau[i];
+  const Prelude pr = lbr_prelude_exact<BSM>(in.S_or_F[i], in.K[i], tau, BSM ? in.r[i] : 0.0, BSM ? in.q[i] : 0.0, in.P[i],
+                                            in.flag[i]);
+  const bool queued = pr.status == 0;
+  sm.status[p] = (uint8_t)pr.status;
+  sm.sig[p] = queued ? tau : (pr.status == 4 ? 0.0 : canonical_nan());
+  sm.veg[p] = queued ? pr.D : 0.0;
+  if (queued) {
+    const int slot = atomicAdd(&sm.count, 1);
+    sm.q0[slot] = pr.U;
+    sm.q1[slot] = pr.O;
+    sm.q2[slot] = pr.B;
+    sm.pos[slot] = (uint16_t)(p | 0x8000);
+  } else if (DIAG) {
+    if (dg.zone) dg.zone[i] = -1;
+    if (dg.s0) dg.s0[i] = 0.0;
+    if (dg.s1) dg.s1[i] = 0.0;
+  }
+}
+
+template <bool BSM, bool DIAG, int RPT, bool FULL>
+__global__ void __launch_bounds__(kTileThreads, (BSM || FULL || DIAG) ? 3 : 4)
 forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
-                    uint8_t* __restrict__ status, int8_t* __restrict__ zone, const int* __restrict__ sel, int want) {
-  if (SEL && *sel != want) return;   // pivot_iv_forward_auto: the probe chose the other organisation
+                    uint8_t* __restrict__ status, DiagOut dg) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   constexpr int kTileRows = kTileThreads * RPT;
   TileSmem<RPT>& sm = *reinterpret_cast<TileSmem<RPT>*>(smem_raw);
@@ -108,7 +125,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const int lane = tid & 31;
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
   const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
-  if (tid == 0) { sm.count = 0; sm.nclass = 0ull; }
+  if (tid == 0) { sm.count = 0; sm.n01 = 0u; sm.n2 = 0u; }
   __syncthreads();
 
   // ---- phase A: all rows of the tile; every load of the thread's rows is issued before the first use
@@ -134,21 +151,27 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     vr[k] = (BSM && live) ? __ldcs(gr + p) : 0.0;
     vq[k] = (BSM && live) ? __ldcs(gq + p) : 0.0;
   }
-  unsigned qmask = 0, cmask = 0;  // bit k: row k of this thread is queued / is a call
+  unsigned qmask = 0, rmask = 0;  // bit k: row k of this thread is queued / needs the exact prelude
 #pragma unroll
   for (int k = 0; k < RPT; ++k) {
     const int p = k * kTileThreads + tid;
+    const bool live = p < rows;
     const Prelude pr = lbr_prelude<BSM>(vF[k], vK[k], vT[k], vr[k], vq[k], vP[k], vf[k]);
     const bool queued = pr.status == 0;
-    if (p < rows) {
+    if (live && pr.status != 5) {
       sm.status[p] = (uint8_t)pr.status;
       sm.sig[p] = queued ? vT[k] : (pr.status == 4 ? 0.0 : canonical_nan());
-      sm.veg[p] = queued ? pr.scale : 0.0;
-      if (ZONES && !queued) zone[base + p] = -1;
+      if (BSM) sm.veg[p] = queued ? pr.D : 0.0;
+      else if (!queued) sm.veg[p] = 0.0;
+      if (DIAG && !queued) {
+        if (dg.zone) dg.zone[base + p] = -1;
+        if (dg.s0) dg.s0[base + p] = 0.0;
+        if (dg.s1) dg.s1[base + p] = 0.0;
+      }
     }
     qmask |= queued ? (1u << k) : 0u;
-    cmask |= pr.call ? (1u << k) : 0u;
-    vF[k] = pr.F; vP[k] = pr.B; vT[k] = pr.rootFK;  // what the solver pass needs: F, K, B, sqrt(FK)
+    rmask |= (live && pr.status == 5) ? (1u << k) : 0u;
+    vF[k] = pr.U; vK[k] = pr.O; vP[k] = pr.B;   // what the solver pass needs
   }
   {
     // one warp scan and one shared atomic per warp for the whole tile
@@ -168,37 +191,46 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
         sm.q0[slot] = vF[k];
         sm.q1[slot] = vK[k];
         sm.q2[slot] = vP[k];
-        sm.q3[slot] = vT[k];
-        sm.pos[slot] = (uint16_t)((k * kTileThreads + tid) | ((cmask >> k) & 1u ? 0x8000 : 0));
+        sm.pos[slot] = (uint16_t)(k * kTileThreads + tid);
         ++slot;
       }
     }
   }
+  if (rmask) {   // unusual rows: the exact prelude decides, from the row's inputs re-read (rare, divergent)
+#pragma unroll 1
+    for (int k = 0; k < RPT; ++k)
+      if ((rmask >> k) & 1u) tile_rare_row<BSM, DIAG, RPT>(in, base, k * kTileThreads + tid, sm, dg);
+  }
   __syncthreads();
 
-  // ---- phase B1a: x, boundary point, node, zone; middle zones (1, 2) finished; rows regrouped by zone class
+  // ---- phase B1: normalisation, x, boundary point, node, zone; middle zones (1, 2) finished; rows regrouped by zone class
   //      lists: zone 0 (-> LOWER) from the front of perm, finished LINEAR rows from the back, zone 3 in permU
   const int cnt = sm.count;
   for (int j0 = 0; j0 < cnt; j0 += kTileThreads) {   // j0 is CTA-uniform: every lane reaches the ballots
     const int j = j0 + tid;
     int cls = -1;  // 0: zone 0, 1: finished (zones 1, 2), 2: zone 3
     if (j < cnt) {
-      const Norm nm = lbr_normalise(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j], (sm.pos[j] & 0x8000) != 0);
-      const SeedHead hd = lbr_seed_head(nm.qrel, nm.beta, nm.bbar, nm.bmax);
+      const int pj = sm.pos[j];
+      const Norm nm = lbr_normalise(sm.q0[j], sm.q1[j], sm.q2[j], (pj & 0x8000) != 0);
+      const SeedHead hd = lbr_seed_head<FULL>(nm.qrel, nm.beta, nm.bbar, nm.bmax);
       sm.q0[j] = hd.v0; sm.q1[j] = hd.v1; sm.q2[j] = hd.v2; sm.q3[j] = hd.v3;
+      const int p = pj & 0x3fff;
+      sm.veg[p] = BSM ? sm.veg[p] * nm.rootFK : nm.rootFK;    // D sqrt(FK)
       cls = (hd.zone == 0) ? 0 : ((hd.zone == 3) ? 2 : 1);
-      if (ZONES) zone[base + (sm.pos[j] & 0x3fff)] = (int8_t)hd.zone;
+      if (DIAG && dg.zone) dg.zone[base + p] = (int8_t)hd.zone;
     }
     const unsigned m0 = __ballot_sync(0xffffffffu, cls == 0);
     const unsigned m1 = __ballot_sync(0xffffffffu, cls == 1);
     const unsigned m2 = __ballot_sync(0xffffffffu, cls == 2);
-    // one 64-bit shared atomic per warp hands out the three list offsets at once
-    unsigned long long base3 = 0ull;
-    if (lane == 0)
-      base3 = atomicAdd(&sm.nclass, (unsigned long long)__popc(m0) | ((unsigned long long)__popc(m1) << 21) |
-                                        ((unsigned long long)__popc(m2) << 42));
-    base3 = __shfl_sync(0xffffffffu, base3, 0);
-    const int b0 = (int)(base3 & 0x1fffffu), b1 = (int)((base3 >> 21) & 0x1fffffu), b2 = (int)(base3 >> 42);
+    // native 32-bit shared atomics hand out the list offsets: one for zone 0 / middle, one for zone 3 (if any)
+    unsigned base01 = 0u, base2 = 0u;
+    if (lane == 0) {
+      base01 = atomicAdd(&sm.n01, (unsigned)__popc(m0) | ((unsigned)__popc(m1) << 16));
+      if (m2) base2 = atomicAdd(&sm.n2, (unsigned)__popc(m2));
+    }
+    base01 = __shfl_sync(0xffffffffu, base01, 0);
+    base2 = __shfl_sync(0xffffffffu, base2, 0);
+    const int b0 = (int)(base01 & 0xffffu), b1 = (int)(base01 >> 16), b2 = (int)base2;
     const unsigned lt = (1u << lane) - 1u;
     if (cls == 0) sm.perm[b0 + __popc(m0 & lt)] = (uint16_t)j;
     else if (cls == 1) sm.perm[kTileRows - 1 - (b1 + __popc(m1 & lt))] = (uint16_t)j;
@@ -209,28 +241,32 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   // ---- phase B2: the tail seeds (zone 0 rows, zone 3 rows) fused with the Householder steps; rows ordered zone 0
   //      (LOWER), finished middle rows (LINEAR), zone 3 (UPPER or LINEAR): a warp sees one zone and one objective kind
   //      except at the two group boundaries
-  const int n0 = (int)(sm.nclass & 0x1fffffu), n1 = (int)((sm.nclass >> 21) & 0x1fffffu);
+  const int n0 = (int)(sm.n01 & 0xffffu), n1 = (int)(sm.n01 >> 16);
   for (int k = tid; k < cnt; k += kTileThreads) {
     int j, kind;
     double x, s0, p1, p2;
     if (k < n0) {
       j = sm.perm[k];
-      const Seed sd = lbr_seed_tail0(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+      const Seed sd = lbr_seed_tail0<FULL>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
       x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = KIND_LOWER;
     } else if (k < n0 + n1) {
       j = sm.perm[kTileRows - 1 - (k - n0)];
       x = sm.q0[j]; s0 = sm.q1[j]; p1 = sm.q2[j]; p2 = sm.q3[j]; kind = KIND_LINEAR;
     } else {
       j = sm.permU[k - n0 - n1];
-      const Seed sd = lbr_seed_tail3(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+      const Seed sd = lbr_seed_tail3<FULL>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
       x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = sd.kind;
     }
-    const NormSolve ns = lbr_refine<kHouseholderSteps>(x, s0, p1, p2, kind);
+    const NormSolve ns = lbr_refine<kHouseholderSteps, FULL>(x, s0, p1, p2, kind);
     const int p = sm.pos[j] & 0x3fff;
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
     sm.sig[p] = ns.s * rinv;
     sm.veg[p] = sm.veg[p] * ns.vfin * (tau * rinv);
+    if (DIAG) {
+      if (dg.s0) dg.s0[base + p] = s0;
+      if (dg.s1) dg.s1[base + p] = ns.s1;
+    }
   }
   __syncthreads();
 
@@ -269,10 +305,11 @@ __device__ __forceinline__ double backward_row(double gs, double V, uint8_t st, 
 }
 
 // 4 rows per thread per iteration (two 16-byte loads per fp64 array, one 4-byte status load), grid-stride.
+// grad_P may alias grad_sigma (include/pivot_iv.h): neither pointer is __restrict__, and a thread loads its rows before it stores them.
 template <int MODE>
 __global__ void __launch_bounds__(kBwdThreads)
-backward_kernel_vec4(const double* __restrict__ gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
-                     double floor_, int64_t n4, double* __restrict__ gP) {
+backward_kernel_vec4(const double* gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
+                     double floor_, int64_t n4, double* gP) {
   const double floor2 = __dmul_rn(floor_, floor_);
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n4; j += stride) {
@@ -293,8 +330,8 @@ backward_kernel_vec4(const double* __restrict__ gs, const double* __restrict__ v
 
 template <int MODE>
 __global__ void __launch_bounds__(kBwdThreads)
-backward_kernel_scalar(const double* __restrict__ gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
-                       double floor_, int64_t begin, int64_t n, double* __restrict__ gP) {
+backward_kernel_scalar(const double* gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
+                       double floor_, int64_t begin, int64_t n, double* gP) {
   const double floor2 = __dmul_rn(floor_, floor_);
   const int64_t i = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) gP[i] = backward_row<MODE>(gs[i], vega[i], status[i], floor_, floor2);
@@ -313,44 +350,6 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(int64_t iters, double* 
   if (sum == 123.456) sink[0] = sum;  // never true; keeps the chains alive
 }
 
-// ---------------------------------------------------------------------------------------------------------------
-// Probe of pivot_iv_forward_auto: 2048 sampled (row, next row) pairs.  ws[0] = 1 (row-per-thread organisation) when at
-// least 95 % of the sampled rows reach the solver AND at least 90 % of the pairs are the same contract up to 2 % in F|S
-// and K (an option chain in strike order: warps are zone-uniform by themselves); else 0 (compaction).  ws[1..3] = rows
-// that solve, alike pairs, samples.
-// ---------------------------------------------------------------------------------------------------------------
-constexpr int kProbePairs = 2048;
-constexpr int kProbeBlocks = 8;   // 8 x 256 threads: one pair per thread, every load of the probe is in flight at once
-template <bool BSM>
-__global__ void __launch_bounds__(256) forward_probe_kernel(pivot_iv_inputs in, int64_t n, int* __restrict__ ws) {
-  // ws[1], ws[2] accumulate; ws[4] is the ticket; the last CTA to arrive decides and resets the accumulators' ticket
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  const int64_t i = (int64_t)(((n - 2) / kProbePairs) * (int64_t)k);
-  const double F0 = in.S_or_F[i], K0 = in.K[i], F1 = in.S_or_F[i + 1], K1 = in.K[i + 1];
-  const double r = BSM ? in.r[i] : 0.0, q = BSM ? in.q[i] : 0.0;
-  const Prelude pr = lbr_prelude<BSM>(F0, K0, in.tau[i], r, q, in.P[i], in.flag[i]);
-  const unsigned mo = __ballot_sync(0xffffffffu, pr.status == PIVOT_ST_OK);
-  const unsigned ma = __ballot_sync(0xffffffffu, fabs(K1 - K0) <= 0.02 * K0 && fabs(F1 - F0) <= 0.02 * F0);
-  __shared__ int last;
-  if ((threadIdx.x & 31) == 0) {
-    atomicAdd(&ws[5], __popc(mo));
-    atomicAdd(&ws[6], __popc(ma));
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    __threadfence();
-    last = atomicAdd(&ws[4], 1) == kProbeBlocks - 1;
-  }
-  __syncthreads();
-  if (last && threadIdx.x == 0) {
-    __threadfence();
-    const int ok = atomicAdd(&ws[5], 0), alike = atomicAdd(&ws[6], 0);
-    ws[1] = ok; ws[2] = alike; ws[3] = kProbePairs;
-    ws[0] = (ok * 100 >= 95 * kProbePairs && alike * 100 >= 90 * kProbePairs) ? 1 : 0;
-    ws[4] = 0; ws[5] = 0; ws[6] = 0;   // ready for the next call on this stream
-  }
-}
-
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 }  // namespace pivot
@@ -362,87 +361,93 @@ using namespace pivot;
 
 namespace {
 
-// Kernel choice.  PIVOT_FWD_AUTO follows the environment variable PIVOT_IV_FWD_KERNEL (=rowwise: one row per thread;
-// anything else / unset: tile compaction), read once; it exists for the ncu A/B studies of DESIGN.md section 8.
-bool env_rowwise() {
-  static const bool v = [] {
-    const char* e = std::getenv("PIVOT_IV_FWD_KERNEL");
-    return e && e[0] == 'r';
-  }();
-  return v;
+constexpr int kMaxDevices = 64;
+
+// cudaFuncSetAttribute applies to the CURRENT device only: remember per kernel and per device ordinal where the dynamic
+// shared-memory opt-in has been made (a failure is not cached, it is retried by the next call).
+template <auto Kernel>
+int ensure_dynamic_smem(int bytes) {
+  static std::atomic<unsigned long long> done{0ull};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PIVOT_ERR_CUDA;
+  if (dev >= 0 && dev < kMaxDevices && ((done.load(std::memory_order_relaxed) >> dev) & 1ull)) return PIVOT_OK;
+  if (cudaFuncSetAttribute(Kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return PIVOT_ERR_CUDA;
+  }
+  if (dev >= 0 && dev < kMaxDevices) done.fetch_or(1ull << dev, std::memory_order_relaxed);
+  return PIVOT_OK;
 }
 
-template <bool BSM, bool ZONES>
-int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
-                     int kernel, cudaStream_t st) {
-  const bool rowwise = kernel == PIVOT_FWD_ROWWISE || (kernel == PIVOT_FWD_AUTO && env_rowwise());
+// SM count of the current device (cached per device ordinal)
+int sm_count() {
+  static std::atomic<int> cache[kMaxDevices];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return 148; }
+  if (dev >= 0 && dev < kMaxDevices) {
+    const int c = cache[dev].load(std::memory_order_relaxed);
+    if (c > 0) return c;
+  }
+  int sms = 0;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+    (void)cudaGetLastError();
+    return 148;
+  }
+  if (dev >= 0 && dev < kMaxDevices) cache[dev].store(sms, std::memory_order_relaxed);
+  return sms;
+}
+
+template <bool BSM, bool DIAG, int RPT, bool FULL>
+int launch_tile(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, const DiagOut& dg,
+                cudaStream_t st) {
+  const int rc = ensure_dynamic_smem<forward_kernel_tile<BSM, DIAG, RPT, FULL>>((int)sizeof(TileSmem<RPT>));
+  if (rc != PIVOT_OK) return rc;
+  const int64_t blocks = (n + RPT * kTileThreads - 1) / (RPT * kTileThreads);
+  forward_kernel_tile<BSM, DIAG, RPT, FULL><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<RPT>), st>>>(in, n, sigma, vega,
+                                                                                                         status, dg);
+  return PIVOT_OK;
+}
+
+template <bool BSM, bool DIAG, bool FULL>
+int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, const DiagOut& dg,
+                     bool rowwise, cudaStream_t st) {
+  int rc = PIVOT_OK;
   if (rowwise) {
     const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
-    forward_kernel_scalar<BSM, ZONES><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, 0, n, sigma, vega, status, zone, nullptr, 0);
-  } else {
+    forward_kernel_scalar<BSM, DIAG, FULL><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, n, sigma, vega, status, dg);
+  } else if (!DIAG && !FULL && n <= ((int64_t)1 << 19)) {
     // small launches use 256-row tiles so that the grid still covers the chip (n <= 2^19: at most 2048 CTAs)
-    if (n <= ((int64_t)1 << 19)) {
-      static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES, 1>,
-                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<1>));
-      if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
-      const int64_t blocks = (n + kTileThreads - 1) / kTileThreads;
-      forward_kernel_tile<BSM, ZONES, 1><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<1>), st>>>(in, n, sigma, vega, status, zone, nullptr, 0);
-    } else {
-      static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, ZONES, 4>,
-                                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<4>));
-      if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
-      const int64_t blocks = (n + 4 * kTileThreads - 1) / (4 * kTileThreads);
-      forward_kernel_tile<BSM, ZONES, 4><<<(unsigned)blocks, kTileThreads, sizeof(TileSmem<4>), st>>>(in, n, sigma, vega, status, zone, nullptr, 0);
-    }
+    rc = launch_tile<BSM, false, 1, false>(in, n, sigma, vega, status, dg, st);
+  } else {
+    rc = launch_tile<BSM, DIAG, 4, FULL>(in, n, sigma, vega, status, dg, st);
   }
+  if (rc != PIVOT_OK) return rc;
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 
-int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int8_t* zone,
-                 bool zones, cudaStream_t st, int kernel = PIVOT_FWD_AUTO) {
+int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, const DiagOut* dg,
+                 cudaStream_t st, int kernel = PIVOT_FWD_AUTO) {
   if (!in) return PIVOT_ERR_NULL;
-  if (kernel != PIVOT_FWD_AUTO && kernel != PIVOT_FWD_COMPACT && kernel != PIVOT_FWD_ROWWISE) return PIVOT_ERR_BAD_ARG;
+  const int org = kernel & ~PIVOT_FWD_FP64_ONLY;
+  if (kernel < 0 || (org != PIVOT_FWD_AUTO && org != PIVOT_FWD_COMPACT && org != PIVOT_FWD_ROWWISE)) return PIVOT_ERR_BAD_ARG;
   if (n < 0) return PIVOT_ERR_BAD_N;
   if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
   if (n == 0) return PIVOT_OK;
-  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status || (zones && !zone))
-    return PIVOT_ERR_NULL;
+  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status) return PIVOT_ERR_NULL;
   if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;  // grid.x limit
-  const bool bsm = in->r != nullptr;
-  if (bsm) return zones ? launch_forward_t<true, true>(*in, n, sigma, vega, status, zone, kernel, st)
-                        : launch_forward_t<true, false>(*in, n, sigma, vega, status, zone, kernel, st);
-  return zones ? launch_forward_t<false, true>(*in, n, sigma, vega, status, zone, kernel, st)
-               : launch_forward_t<false, false>(*in, n, sigma, vega, status, zone, kernel, st);
-}
-
-int g_sm_count = 0;
-int sm_count() {
-  if (g_sm_count == 0) {
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-      sms = 148;
-    g_sm_count = sms;
+  const bool bsm = in->r != nullptr, full = (kernel & PIVOT_FWD_FP64_ONLY) != 0, rowwise = org == PIVOT_FWD_ROWWISE;
+  const DiagOut none{nullptr, nullptr, nullptr};
+  const DiagOut& d = dg ? *dg : none;
+#define PIVOT_DISPATCH(B, G, F) return launch_forward_t<B, G, F>(*in, n, sigma, vega, status, d, rowwise, st)
+  if (dg) {
+    if (bsm) { if (full) PIVOT_DISPATCH(true, true, true); PIVOT_DISPATCH(true, true, false); }
+    if (full) PIVOT_DISPATCH(false, true, true);
+    PIVOT_DISPATCH(false, true, false);
   }
-  return g_sm_count;
-}
-
-// pivot_iv_forward_auto: probe, then both organisations are enqueued and the one the probe did not choose returns at
-// once (the row-per-thread kernel as a small grid-stride grid, so that its early exit costs microseconds).
-template <bool BSM>
-int launch_forward_auto_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, int* ws,
-                          cudaStream_t st) {
-  static const cudaError_t attr = cudaFuncSetAttribute(forward_kernel_tile<BSM, false, 4, true>,
-                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TileSmem<4>));
-  if (attr != cudaSuccess) return PIVOT_ERR_CUDA;
-  forward_probe_kernel<BSM><<<kProbeBlocks, kProbePairs / kProbeBlocks, 0, st>>>(in, n, ws);
-  const int64_t rblocks = (n + kFwdThreads - 1) / kFwdThreads;
-  const int64_t rcap = (int64_t)sm_count() * 6 * 8;    // 80 registers: 6 resident CTAs of 128 threads per SM; 8 waves' worth, grid-stride
-  forward_kernel_scalar<BSM, false, true><<<(unsigned)(rblocks < rcap ? rblocks : rcap), kFwdThreads, 0, st>>>(
-      in, 0, n, sigma, vega, status, nullptr, ws, 1);
-  const int64_t tblocks = (n + 4 * kTileThreads - 1) / (4 * kTileThreads);
-  forward_kernel_tile<BSM, false, 4, true><<<(unsigned)tblocks, kTileThreads, sizeof(TileSmem<4>), st>>>(in, n, sigma, vega,
-                                                                                                       status, nullptr, ws, 0);
-  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+  if (bsm) { if (full) PIVOT_DISPATCH(true, false, true); PIVOT_DISPATCH(true, false, false); }
+  if (full) PIVOT_DISPATCH(false, false, true);
+  PIVOT_DISPATCH(false, false, false);
+#undef PIVOT_DISPATCH
 }
 
 template <int MODE>
@@ -485,35 +490,25 @@ extern "C" {
 
 int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
                      pivot_iv_stream stream) {
-  return forward_impl(in, n, sigma, vega, status, nullptr, false, reinterpret_cast<cudaStream_t>(stream));
+  return forward_impl(in, n, sigma, vega, status, nullptr, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
                         pivot_iv_stream stream) {
-  return forward_impl(in, n, sigma, vega, status, nullptr, false, reinterpret_cast<cudaStream_t>(stream), kernel);
-}
-
-int64_t pivot_iv_forward_auto_workspace_bytes(void) { return 64; }
-
-int pivot_iv_forward_auto(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
-                          void* workspace, pivot_iv_stream stream) {
-  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (!in) return PIVOT_ERR_NULL;
-  if (n < ((int64_t)1 << 23))   // no probe below 2^23 rows (probe + the unused launch cost ~30 us); workspace not used
-    return forward_impl(in, n, sigma, vega, status, nullptr, false, st, PIVOT_FWD_COMPACT);
-  if (!workspace) return PIVOT_ERR_NULL;
-  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
-  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status) return PIVOT_ERR_NULL;
-  if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;
-  if ((reinterpret_cast<uintptr_t>(workspace) & 3u) != 0) return PIVOT_ERR_BAD_ARG;
-  int* ws = static_cast<int*>(workspace);
-  return in->r ? launch_forward_auto_t<true>(*in, n, sigma, vega, status, ws, st)
-               : launch_forward_auto_t<false>(*in, n, sigma, vega, status, ws, st);
+  return forward_impl(in, n, sigma, vega, status, nullptr, reinterpret_cast<cudaStream_t>(stream), kernel);
 }
 
 int pivot_iv_forward_zones(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
                            int8_t* zone, pivot_iv_stream stream) {
-  return forward_impl(in, n, sigma, vega, status, zone, true, reinterpret_cast<cudaStream_t>(stream));
+  if (n > 0 && !zone) return PIVOT_ERR_NULL;
+  const DiagOut dg{zone, nullptr, nullptr};
+  return forward_impl(in, n, sigma, vega, status, &dg, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int pivot_iv_forward_diag(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                          int8_t* zone, double* s_seed, double* s_step1, int kernel, pivot_iv_stream stream) {
+  const DiagOut dg{zone, s_seed, s_step1};
+  return forward_impl(in, n, sigma, vega, status, &dg, reinterpret_cast<cudaStream_t>(stream), kernel);
 }
 
 int pivot_iv_backward(const double* grad_sigma, const double* vega, const uint8_t* status, double vega_floor, int mode,
@@ -610,7 +605,7 @@ int pipeline_run(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* 
     if (bwd && cudaMemcpyAsync(d[9], gs + off, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = PIVOT_ERR_CUDA;
     if (rc != PIVOT_OK) break;
     pivot_iv_inputs din{d[0], d[1], d[2], bsm ? d[3] : nullptr, bsm ? d[4] : nullptr, d[5], d[6]};
-    rc = forward_impl(&din, m, d[7], d[8], p->st[slot], nullptr, false, s, p->fwd_kernel);
+    rc = forward_impl(&din, m, d[7], d[8], p->st[slot], nullptr, s, p->fwd_kernel);
     if (rc == PIVOT_OK && bwd) rc = backward_impl(d[9], d[8], p->st[slot], floor_, mode, m, d[10], s);
     if (rc != PIVOT_OK) break;
     if (cudaMemcpyAsync(sigma + off, d[7], bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
@@ -658,7 +653,8 @@ int pivot_iv_pipeline_create(pivot_iv_pipeline** out, int device, int64_t chunk_
 
 int pivot_iv_pipeline_set_forward_kernel(pivot_iv_pipeline* p, int kernel) {
   if (!p) return PIVOT_ERR_NULL;
-  if (kernel != PIVOT_FWD_AUTO && kernel != PIVOT_FWD_COMPACT && kernel != PIVOT_FWD_ROWWISE) return PIVOT_ERR_BAD_ARG;
+  const int org = kernel & ~PIVOT_FWD_FP64_ONLY;
+  if (kernel < 0 || (org != PIVOT_FWD_AUTO && org != PIVOT_FWD_COMPACT && org != PIVOT_FWD_ROWWISE)) return PIVOT_ERR_BAD_ARG;
   p->fwd_kernel = kernel;
   return PIVOT_OK;
 }
