@@ -68,8 +68,8 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma,
 // Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); both partitions cost shared-memory traffic only.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
-// RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers) for large n; 1 (256-row
-// tiles) for small n, so that a launch of 65,536 rows still spreads over every SM.
+// RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers, both modes) for large n;
+// 1 (256-row tiles) for small n, so that a launch of 65,536 rows still spreads over every SM.
 
 template <int RPT>
 struct TileSmem {
@@ -115,7 +115,7 @@ __device__ __noinline__ void tile_rare_row(pivot_iv_inputs in, int64_t base, int
 }
 
 template <bool BSM, bool DIAG, int RPT, bool FULL>
-__global__ void __launch_bounds__(kTileThreads, (BSM || FULL || DIAG) ? 3 : 4)
+__global__ void __launch_bounds__(kTileThreads, (FULL || DIAG) ? 3 : 4)
 forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                     uint8_t* __restrict__ status, DiagOut dg) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -174,26 +174,30 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     vF[k] = pr.U; vK[k] = pr.O; vP[k] = pr.B;   // what the solver pass needs
   }
   {
-    // one warp scan and one shared atomic per warp for the whole tile
-    const int c = __popc(qmask);
-    int incl = c;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const int v = __shfl_up_sync(0xffffffffu, incl, d);
-      if (lane >= d) incl += v;
-    }
-    int wbase = 0;
-    if (lane == 31 && incl > 0) wbase = atomicAdd(&sm.count, incl);
-    int slot = __shfl_sync(0xffffffffu, wbase, 31) + incl - c;
+    // Queue slots, warp by warp: within a warp the order is k-major then lane, so that a run of 32 CONSECUTIVE rows stays
+    // contiguous in the queue (on option chains in strike order the dense warps of phase B1 then see neighbouring rows:
+    // one zone).  RPT ballots and one shared atomic per warp per tile.
+    unsigned bal[RPT];
+    int total = 0;
 #pragma unroll
     for (int k = 0; k < RPT; ++k) {
-      if (qmask & (1u << k)) {
-        sm.q0[slot] = vF[k];
-        sm.q1[slot] = vK[k];
-        sm.q2[slot] = vP[k];
-        sm.pos[slot] = (uint16_t)(k * kTileThreads + tid);
-        ++slot;
+      bal[k] = __ballot_sync(0xffffffffu, (qmask >> k) & 1u);
+      total += __popc(bal[k]);
+    }
+    int wbase = 0;
+    if (lane == 0 && total > 0) wbase = atomicAdd(&sm.count, total);
+    int slot = __shfl_sync(0xffffffffu, wbase, 0);
+    const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      if ((qmask >> k) & 1u) {
+        const int j = slot + __popc(bal[k] & lt);
+        sm.q0[j] = vF[k];
+        sm.q1[j] = vK[k];
+        sm.q2[j] = vP[k];
+        sm.pos[j] = (uint16_t)(k * kTileThreads + tid);
       }
+      slot += __popc(bal[k]);
     }
   }
   if (rmask) {   // unusual rows: the exact prelude decides, from the row's inputs re-read (rare, divergent)
