@@ -200,6 +200,33 @@ int pivot_iv_forward_backward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* 
  * `sink` is a device buffer of at least 8 bytes. */
 int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivot_iv_stream stream);
 
+/* Test-only: evaluates ONE function of the device math library elementwise, out[i] = fn(a[i] [, b[i]]), so that its error
+ * can be measured on the device against a multiprecision reference (tests/test_gpu_mathlib.py; DESIGN.md section 5 lists
+ * the measured bounds).  a, b, out: device, n doubles; b is read only by the two-argument functions (erfcx pair: the pair
+ * is erfcx(a), erfcx(b); div_fast: a / b).  fp32-grade functions take and return doubles (converted inside).
+ * Returns PIVOT_ERR_BAD_ARG for an unknown fn, PIVOT_ERR_NULL / _BAD_N / _CUDA as usual. */
+#define PIVOT_DBG_ERFCX_ONE 0      /* erfcx(a), a >= 0, fp64 (degree-22 form) */
+#define PIVOT_DBG_ERFCX_PAIR_1 1   /* first of erfcx_pair(a, b) */
+#define PIVOT_DBG_ERFCX_PAIR_2 2   /* second of erfcx_pair(a, b) */
+#define PIVOT_DBG_ERFCX_SEED 3     /* erfcx(a), fp32 seed grade */
+#define PIVOT_DBG_EXP_FAST 4       /* exp(a), full range incl. the under / overflow branches */
+#define PIVOT_DBG_EXP_SEED 5       /* exp(a), |a| < 700, MUFU.EX2 grade */
+#define PIVOT_DBG_LOG_FAST 6       /* ln(a), a positive normal */
+#define PIVOT_DBG_LOG_SEED 7       /* ln(a), a > 0 incl. subnormal, MUFU.LG2 grade */
+#define PIVOT_DBG_LOG1P_FAST 8     /* ln(1 + a), a >= 0 */
+#define PIVOT_DBG_RCP_NR1 9        /* 1/a, one Newton step */
+#define PIVOT_DBG_RCP_NR2 10       /* 1/a, two Newton steps */
+#define PIVOT_DBG_DIV_FAST 11      /* a / b */
+#define PIVOT_DBG_SQRT_NR1 12      /* sqrt(a), one Newton step */
+#define PIVOT_DBG_SQRT_NR2 13      /* sqrt(a), a positive normal */
+#define PIVOT_DBG_RSQRT_NR2 14     /* 1/sqrt(a) as returned beside sqrt_nr2 */
+#define PIVOT_DBG_NINV_TAIL_SEED 15 /* -Phi^-1(e^a), a <= ln 0.345, fp32 seed grade */
+#define PIVOT_DBG_NINV_TAIL_FULL 16 /* ... refined by two Newton steps at fp64 */
+#define PIVOT_DBG_EXPF_SEED 17     /* exp(a) in fp32 (MUFU.EX2), |a| <= 87 */
+#define PIVOT_DBG_LOGF_SEED 18     /* ln(a) in fp32 (MUFU.LG2) */
+#define PIVOT_DBG_COUNT 19
+int pivot_iv_debug_math(int fn, const double* a, const double* b, int64_t n, double* out, pivot_iv_stream stream);
+
 /* Number of kernels a call launches (for bench.py's `gpu_launches` bookkeeping). */
 int pivot_iv_launches_per_forward(void);
 int pivot_iv_launches_per_backward(void);

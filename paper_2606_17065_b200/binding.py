@@ -25,7 +25,7 @@ EXPORTS = (
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_loss_roundtrip_workspace_bytes", "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
-    "pivot_iv_forward_diag",
+    "pivot_iv_forward_diag", "pivot_iv_debug_math",
 )
 
 
@@ -57,6 +57,7 @@ def load_library():
     lib.pivot_iv_forward.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
     lib.pivot_iv_forward_ex.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, cint, vp]
     lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
+    lib.pivot_iv_debug_math.argtypes = [cint, vp, vp, i64, vp, vp]
     lib.pivot_iv_forward_diag.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp, vp, cint, vp]
     lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
     lib.pivot_iv_backward.argtypes = [vp, vp, vp, dbl, cint, i64, vp, vp]
@@ -185,6 +186,24 @@ def pivot_iv_forward_diag(S_or_F, K, tau, P, flag, r=None, q=None, kernel: int =
         _check(lib.pivot_iv_forward_diag(C.byref(inp), n, sigma.data_ptr(), vega.data_ptr(), status.data_ptr(),
                                          zone.data_ptr(), s0.data_ptr(), s1.data_ptr(), int(kernel), _stream_ptr(stream)))
     return sigma, vega, status, zone, s0, s1
+
+
+DBG = {name: i for i, name in enumerate((
+    "erfcx_one", "erfcx_pair_1", "erfcx_pair_2", "erfcx_seed", "exp_fast", "exp_seed", "log_fast", "log_seed", "log1p_fast",
+    "rcp_nr1", "rcp_nr2", "div_fast", "sqrt_nr1", "sqrt_nr2", "rsqrt_nr2", "ninv_tail_seed", "ninv_tail_full", "expf_seed",
+    "logf_seed"))}
+
+
+def pivot_iv_debug_math(fn: str, a: torch.Tensor, b: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """Test-only: out = fn(a [, b]) evaluated by the device math library (see PIVOT_DBG_* in include/pivot_iv.h)."""
+    _require_cuda()
+    n = a.numel()
+    _same_len(n, b=b)
+    out = torch.empty_like(a)
+    with torch.cuda.device(a.device):
+        _check(load_library().pivot_iv_debug_math(DBG[fn], _dev(a, "a"), _dev(b, "b"), n, _dev(out, "out"),
+                                                  _stream_ptr(stream)))
+    return out
 
 
 def pivot_iv_forward_zones(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None):

@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SO = os.path.join(HERE, "libpivot_iv.so")
-SRC = [os.path.join(HERE, "csrc", "pivot_iv.cu"), os.path.join(HERE, "csrc", "pivot_greeks.cu")]
+SRC = [os.path.join(HERE, "csrc", f) for f in ("pivot_iv.cu", "pivot_greeks.cu", "pivot_debug.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "lbr_device.cuh"), os.path.join(HERE, "csrc", "coeffs.cuh"), os.path.join(ROOT, "include", "pivot_iv.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
