@@ -209,7 +209,7 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     from oracle import pyoracle as po
-    from paper_2606_17065_b200 import workloads as wl
+    import workloads as wl
     m = min(args.rows, 1 << 22)
     cfg = wl.config4(m, device="cpu")
     c = {k: cfg[k].numpy() for k in KEYS}
@@ -255,7 +255,7 @@ def main():
         return run_reference(args)
 
     import paper_2606_17065_b200 as pv
-    from paper_2606_17065_b200 import workloads as wl
+    import workloads as wl
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -155,21 +155,35 @@ int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, con
                              double* grad_S_or_F, double* grad_K, double* grad_tau, double* grad_r, double* grad_q,
                              pivot_iv_stream stream);
 
-/* The two PIVOT objectives as sums, so that the caller normalises by the rows used:
+/* The two PIVOT objectives as sums, so that the caller normalises by the rows used, each fused with its
+ * gradient with respect to sigma_hat in the same pass (one kernel each; every intermediate in registers, no workspace):
  *   eq.(11)  L_price = (out3[0]/out3[2]) / (out3[1]/out3[2])^2,  out3 += { sum (P_BS(xi, sigma_hat) - P*)^2, sum |P*|, rows used }
+ *            grad_sigma_hat[i] = grad_scale * 2 (P_BS - P*) V_hat           (V_hat = vega at sigma_hat; eq.(14))
  *   eq.(12)  L_rt    =  out3[0]/out3[2],                         out3 += { sum w (JaeckelIV(P~) - sigma*)^2, sum w, rows used },
- *            w = V_hat^2/(V_hat^2 + vega_floor^2) (eq.(10)), V_hat = vega at sigma_hat, P~ = model price where |V_hat| > vega_floor,
- *            else the sentinel market price P* (in->P); the inversion is the same fused forward kernel as pivot_iv_forward.
- * Rows with a non-finite model price or P* are skipped by (11); rows whose inversion is not OK or whose sigma* is not finite by (12).
- * out3 [device, 3 doubles] is ACCUMULATED into (zero it first).  sigma_hat, sigma_star [in, device, n doubles].
- * workspace [device, pivot_iv_loss_roundtrip_workspace_bytes(n) bytes, 8-byte aligned] is scratch of the round trip
- * (P~, V_hat, the inversion's sigma / vega / status).  Launches: 1 kernel (price loss), 3 kernels (round trip).
- * Returns PIVOT_ERR_NULL / _BAD_N / _BAD_FLOOR / _MIXED_RQ / _BAD_ARG / _CUDA. */
-int pivot_iv_loss_price(const pivot_iv_inputs* in, const double* sigma_hat, int64_t n, double* out3,
-                        pivot_iv_stream stream);
-int64_t pivot_iv_loss_roundtrip_workspace_bytes(int64_t n);
+ *            w = V_hat^2/(V_hat^2 + vega_floor^2) (eq.(10)), P~ = the model price where |V_hat| > vega_floor, else the sentinel
+ *            market price P* (in->P), which carries no gradient; the inversion is the forward pass's own per-row arithmetic.
+ *            grad_sigma_hat[i] = grad_scale * { [|V_hat| > floor] w 2 (sigma_rt - sigma*) (1/V_rt) V_hat
+ *                                               + w'(V_hat) (sigma_rt - sigma*)^2 dV_hat/dsigma_hat }
+ *            -- eq.(17): the 1/V_rt of the inverse channel (MASK rule at vega_floor) against the V_hat of the
+ *            price node; w' = 2 V floor^2/(V^2 + floor^2)^2, dV/dsigma = V d1 d2 / sigma.
+ *   mode PIVOT_RT_NAIVE (the NaN-poisoning diagnostic): no gate, no sentinel, no sanitisation:
+ *            out3 += { sum (JaeckelIV(P_BS(sigma_hat)) - sigma*)^2, rows, rows },
+ *            grad_sigma_hat[i] = grad_scale * STRICT(2 (sigma_rt - sigma*), V_rt; vega_floor) V_hat: NaN wherever the inverse channel is
+ *            singular (|V_rt| <= vega_floor or the inversion is not OK) unless the cotangent is exactly 0; a row with a non-finite
+ *            sigma_hat contributes NaN to the sum and to its gradient.
+ * Rows with a non-finite model price or P* are skipped by (11); rows whose inversion is not OK or whose sigma* is not finite
+ * by the gated (12); skipped rows have gradient +0.
+ *   out3 [device, 3 doubles] is ACCUMULATED into (zero it first).  sigma_hat, sigma_star [in, device, n doubles].
+ *   grad_sigma_hat [out, device, n doubles] or NULL (sums only); grad_scale: the caller's normalisation, e.g. 1/(|B| m^2) with
+ *   m = mean |P*| for eq.(11), 1/|B| for eq.(12).
+ * Returns PIVOT_ERR_NULL / _BAD_N / _BAD_FLOOR / _BAD_MODE / _MIXED_RQ / _CUDA. */
+#define PIVOT_RT_GATED 0
+#define PIVOT_RT_NAIVE 1
+int pivot_iv_loss_price(const pivot_iv_inputs* in, const double* sigma_hat, int64_t n, double* out3, double* grad_sigma_hat,
+                        double grad_scale, pivot_iv_stream stream);
 int pivot_iv_loss_roundtrip(const pivot_iv_inputs* in, const double* sigma_hat, const double* sigma_star, double vega_floor,
-                            int64_t n, void* workspace, double* out3, pivot_iv_stream stream);
+                            int mode, int64_t n, double* out3, double* grad_sigma_hat, double grad_scale,
+                            pivot_iv_stream stream);
 
 /* ---- host-buffer pipeline (the streaming label-generation setting: batches of rows, H2D included) ----
  * A pipeline owns `n_slots` device staging slots of `chunk_rows` rows each, one CUDA stream per slot and pinned

@@ -277,4 +277,75 @@ void oracle_loss_roundtrip(int64_t n, const double* SorF, const double* Kk, cons
   out3[0] = (double)acc; out3[1] = (double)wsum; out3[2] = (double)cnt;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Gradients of the two objectives with respect to sigma_hat, row by row (plain loops).
+// eq.(11):  d/d sigma_hat_i (P_model_i - P*_i)^2 = 2 (P_model_i - P*_i) V_hat_i.
+// eq.(12) per-row term T_i = w(V_hat_i) (sigma_rt_i - sigma*_i)^2, sigma_rt = IV(P~):
+//   on the gate (|V_hat| > tau: P~ = P_model(sigma_hat)), by eq.(17)
+//     dT/d sigma_hat = w 2 (sigma_rt - sigma*) (1/V_rt) V_hat  +  w'(V_hat) (sigma_rt - sigma*)^2 dV_hat/d sigma_hat,
+//   with the inverse channel 1/V_rt under the MASK rule at the same floor (backward_row mode 0);
+//   off the gate (P~ = the sentinel P*, which carries no gradient) only the w' term.
+//   w'(V) = 2 V tau^2 / (V^2 + tau^2)^2,  dV/d sigma = V d1 d2 / sigma (Black vomma).
+// NAIVE composition (Fig.6: no gate, no sentinel, no sanitisation): T_i = (IV(P_model) - sigma*)^2 and
+//   dT/d sigma_hat = STRICT(2 (sigma_rt - sigma*), V_rt; floor) V_hat  (backward_row mode 2: NaN off the gate unless the
+//   cotangent is 0); a row whose inversion returns NaN has a NaN term and a NaN gradient.
+// The results are NOT normalised by |B|.  Rows skipped by the loss (non-finite sigma_hat / price / sigma*, or, gated only,
+// an inversion that is not OK) have gradient 0 in the gated form.
+// ---------------------------------------------------------------------------------------------
+static double vomma_of(double SorF, double Kk, double tau, const double* r, const double* q, double sigma, double vh) {
+  double F = SorF;
+  if (r && q) F = SorF * std::exp((*r - *q) * tau);
+  const double s = sigma * std::sqrt(tau);
+  if (!(s > 0.0)) return 0.0;
+  const double d1 = (std::log(F / Kk) + 0.5 * s * s) / s, d2 = d1 - s;
+  return vh * d1 * d2 / sigma;
+}
+
+void oracle_loss_price_grad(int64_t n, const double* SorF, const double* Kk, const double* tau, const double* r, const double* q,
+                            const double* Pstar, const double* flag, const double* sig_hat, double* g) {
+  for (int64_t i = 0; i < n; ++i) {
+    double rr = r ? r[i] : 0, qq = q ? q[i] : 0;
+    const double* pr = (r && q) ? &rr : nullptr; const double* pq = (r && q) ? &qq : nullptr;
+    const double pm = black_price<double>(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i], flag[i]);
+    const double vh = black_vega_eq14<double>(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i]);
+    g[i] = 0.0;
+    if (!std::isfinite(sig_hat[i]) || !std::isfinite(pm) || !std::isfinite(Pstar[i])) continue;
+    g[i] = 2.0 * (pm - Pstar[i]) * vh;
+  }
+}
+
+void oracle_loss_roundtrip_grad(int64_t n, const double* SorF, const double* Kk, const double* tau, const double* r,
+                                const double* q, const double* Pstar, const double* flag, const double* sig_hat,
+                                const double* sig_star, double vega_floor, int naive, double* g, double* term) {
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  for (int64_t i = 0; i < n; ++i) {
+    double rr = r ? r[i] : 0, qq = q ? q[i] : 0;
+    const double* pr = (r && q) ? &rr : nullptr; const double* pq = (r && q) ? &qq : nullptr;
+    const double pm = black_price<double>(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i], flag[i]);
+    const double vh = black_vega_eq14<double>(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i]);
+    const bool usable = std::isfinite(sig_hat[i]) && std::isfinite(pm) && std::isfinite(vh) && std::isfinite(sig_star[i]);
+    g[i] = 0.0; if (term) term[i] = 0.0;
+    if (naive) {
+      if (!usable) { g[i] = nan; if (term) term[i] = nan; continue; }
+      const RowResult<double> o = lbr_row<double>(SorF[i], Kk[i], tau[i], pr, pq, pm, flag[i]);
+      const double d = o.sigma - sig_star[i];                 // NaN for status 1-3, -sigma* for AT_INTRINSIC (sigma = +0)
+      if (term) term[i] = d * d;
+      g[i] = backward_row<double>(2.0 * d, o.vega, o.status, vega_floor, 2) * vh;
+      continue;
+    }
+    if (!usable) continue;
+    const bool on = std::fabs(vh) > vega_floor;
+    const RowResult<double> o = lbr_row<double>(SorF[i], Kk[i], tau[i], pr, pq, on ? pm : Pstar[i], flag[i]);
+    if (o.status != ST_OK) continue;
+    const double f2 = vega_floor * vega_floor, v2 = vh * vh;
+    const double w = v2 / (v2 + f2);
+    const double wp = (v2 + f2 > 0.0) ? 2.0 * vh * f2 / ((v2 + f2) * (v2 + f2)) : 0.0;
+    const double d = o.sigma - sig_star[i];
+    if (term) term[i] = w * d * d;
+    double gi = wp * d * d * vomma_of(SorF[i], Kk[i], tau[i], pr, pq, sig_hat[i], vh);
+    if (on) gi += w * backward_row<double>(2.0 * d, o.vega, o.status, vega_floor, 0) * vh;
+    g[i] = gi;
+  }
+}
+
 }  // extern "C"

@@ -237,3 +237,26 @@ def loss_roundtrip(SorF, K, tau, Pstar, flag, sigma_hat, sigma_star, vega_floor,
     lib().oracle_loss_roundtrip(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(Pstar), _p(flag),
                                 _p(sigma_hat), _p(sigma_star), C.c_double(vega_floor), _p(out))
     return out
+
+
+def loss_price_grad(SorF, K, tau, Pstar, flag, sigma_hat, r=None, q=None):
+    """d/d sigma_hat_i of (P_model_i - P*_i)^2 (eq.(11), unnormalised): 2 (P_model - P*) V_hat."""
+    SorF, K, tau, Pstar, flag, sigma_hat = map(_d, (SorF, K, tau, Pstar, flag, sigma_hat))
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    g = np.empty(SorF.size)
+    lib().oracle_loss_price_grad(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(Pstar), _p(flag),
+                                 _p(sigma_hat), _p(g))
+    return g
+
+
+def loss_roundtrip_grad(SorF, K, tau, Pstar, flag, sigma_hat, sigma_star, vega_floor, naive=False, r=None, q=None):
+    """(d T_i / d sigma_hat_i, T_i) of the per-row round-trip terms of eq.(12) (gated) or of the naive composition."""
+    SorF, K, tau, Pstar, flag, sigma_hat, sigma_star = map(_d, (SorF, K, tau, Pstar, flag, sigma_hat, sigma_star))
+    r = None if r is None else _d(r)
+    q = None if q is None else _d(q)
+    g = np.empty(SorF.size); term = np.empty(SorF.size)
+    lib().oracle_loss_roundtrip_grad(C.c_int64(SorF.size), _p(SorF), _p(K), _p(tau), _p(r), _p(q), _p(Pstar), _p(flag),
+                                     _p(sigma_hat), _p(sigma_star), C.c_double(vega_floor), C.c_int(int(naive)), _p(g),
+                                     _p(term))
+    return g, term

@@ -8,6 +8,8 @@ from .binding import (  # noqa: F401
     GATE_ATTENUATE,
     GATE_MASK,
     GATE_STRICT,
+    RT_GATED,
+    RT_NAIVE,
     FWD_AUTO,
     FWD_COMPACT,
     FWD_ROWWISE,
@@ -37,5 +39,5 @@ __all__ = [
     "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "Pipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
-    "GATE_ATTENUATE", "GATE_STRICT", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "pivot_iv_debug_math", "EXPORTS",
+    "GATE_ATTENUATE", "GATE_STRICT", "RT_GATED", "RT_NAIVE", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "pivot_iv_debug_math", "EXPORTS",
 ]

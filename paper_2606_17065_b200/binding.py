@@ -24,7 +24,7 @@ EXPORTS = (
     "pivot_iv_pipeline_destroy", "pivot_iv_forward_host", "pivot_iv_forward_backward_host", "pivot_iv_probe_dfma",
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
-    "pivot_iv_loss_roundtrip_workspace_bytes", "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
+    "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
     "pivot_iv_forward_diag", "pivot_iv_debug_math",
 )
 
@@ -70,13 +70,11 @@ def load_library():
     lib.pivot_iv_backward_inputs.argtypes = [C.POINTER(_Inputs), vp, vp, vp, vp, dbl, cint, i64, vp, vp, vp, vp, vp, vp, vp]
     lib.pivot_iv_strerror.argtypes = [cint]
     lib.pivot_iv_strerror.restype = C.c_char_p
-    lib.pivot_iv_loss_price.argtypes = [C.POINTER(_Inputs), vp, i64, vp, vp]
-    lib.pivot_iv_loss_roundtrip.argtypes = [C.POINTER(_Inputs), vp, vp, dbl, i64, vp, vp, vp]
-    lib.pivot_iv_loss_roundtrip_workspace_bytes.argtypes = [i64]
+    lib.pivot_iv_loss_price.argtypes = [C.POINTER(_Inputs), vp, i64, vp, vp, dbl, vp]
+    lib.pivot_iv_loss_roundtrip.argtypes = [C.POINTER(_Inputs), vp, vp, dbl, cint, i64, vp, vp, dbl, vp]
     for name in EXPORTS:
-        if name not in ("pivot_iv_strerror", "pivot_iv_loss_roundtrip_workspace_bytes"):
+        if name != "pivot_iv_strerror":
             getattr(lib, name).restype = cint
-    lib.pivot_iv_loss_roundtrip_workspace_bytes.restype = i64
     _lib = lib
     return lib
 
@@ -260,38 +258,47 @@ def pivot_iv_backward_inputs(S_or_F, K, tau, flag, sigma, vega, status, grad_sig
     return tuple(outs)
 
 
-def pivot_iv_loss_price(S_or_F, K, tau, P_star, flag, sigma_hat, r=None, q=None, stream=None) -> torch.Tensor:
-    """eq.(11) as sums: returns a CUDA tensor [sum (P_model - P*)^2, sum |P*|, rows used]."""
+RT_GATED = 0
+RT_NAIVE = 1
+
+
+def pivot_iv_loss_price(S_or_F, K, tau, P_star, flag, sigma_hat, r=None, q=None, grad_scale: Optional[float] = None,
+                        stream=None):
+    """eq.(11) as sums: returns a CUDA tensor [sum (P_model - P*)^2, sum |P*|, rows used]; with grad_scale also the
+    gradient grad_scale * 2 (P_model - P*) V_hat with respect to sigma_hat: (sums, grad)."""
     _require_cuda()
     lib = load_library()
     n = S_or_F.numel()
+    _same_len(n, K=K, tau=tau, P_star=P_star, flag=flag, sigma_hat=sigma_hat, r=r, q=q)
+    _same_device(S_or_F, K=K, tau=tau, P_star=P_star, flag=flag, sigma_hat=sigma_hat, r=r, q=q)
     inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P_star, "P"),
                   _dev(flag, "flag"))
     out = torch.zeros(3, dtype=torch.float64, device=S_or_F.device)
+    grad = torch.empty(n, dtype=torch.float64, device=S_or_F.device) if grad_scale is not None else None
     with torch.cuda.device(S_or_F.device):
-        _check(lib.pivot_iv_loss_price(C.byref(inp), _dev(sigma_hat, "sigma_hat"), n, _dev(out, "out"), _stream_ptr(stream)))
-    return out
+        _check(lib.pivot_iv_loss_price(C.byref(inp), _dev(sigma_hat, "sigma_hat"), n, _dev(out, "out"), _dev(grad, "grad"),
+                                       float(grad_scale or 0.0), _stream_ptr(stream)))
+    return out if grad is None else (out, grad)
 
 
 def pivot_iv_loss_roundtrip(S_or_F, K, tau, P_star, flag, sigma_hat, sigma_star, vega_floor: float, r=None, q=None,
-                            workspace=None, stream=None) -> torch.Tensor:
-    """eq.(12) as sums: returns a CUDA tensor [sum w (IV(P~) - sigma*)^2, sum w, rows used]."""
+                            mode: int = RT_GATED, grad_scale: Optional[float] = None, stream=None):
+    """eq.(12) as sums (mode RT_GATED) or the naive ungated composition (RT_NAIVE): returns a CUDA tensor
+    [sum w (IV(P~) - sigma*)^2, sum w, rows used]; with grad_scale also the gradient w.r.t. sigma_hat: (sums, grad)."""
     _require_cuda()
     lib = load_library()
     n = S_or_F.numel()
+    _same_len(n, K=K, tau=tau, P_star=P_star, flag=flag, sigma_hat=sigma_hat, sigma_star=sigma_star, r=r, q=q)
+    _same_device(S_or_F, K=K, tau=tau, P_star=P_star, flag=flag, sigma_hat=sigma_hat, sigma_star=sigma_star, r=r, q=q)
     inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P_star, "P"),
                   _dev(flag, "flag"))
-    need = int(lib.pivot_iv_loss_roundtrip_workspace_bytes(n))
-    if workspace is None:
-        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=S_or_F.device)
-    if workspace.numel() * workspace.element_size() < need:
-        raise PivotError(f"workspace too small: {need} bytes needed")
     out = torch.zeros(3, dtype=torch.float64, device=S_or_F.device)
+    grad = torch.empty(n, dtype=torch.float64, device=S_or_F.device) if grad_scale is not None else None
     with torch.cuda.device(S_or_F.device):
         _check(lib.pivot_iv_loss_roundtrip(C.byref(inp), _dev(sigma_hat, "sigma_hat"), _dev(sigma_star, "sigma_star"),
-                                           float(vega_floor), n, workspace.data_ptr(), _dev(out, "out"),
-                                           _stream_ptr(stream)))
-    return out
+                                           float(vega_floor), int(mode), n, _dev(out, "out"), _dev(grad, "grad"),
+                                           float(grad_scale or 0.0), _stream_ptr(stream)))
+    return out if grad is None else (out, grad)
 
 
 def pivot_iv_probe_dfma(iters: int, stream=None) -> float:

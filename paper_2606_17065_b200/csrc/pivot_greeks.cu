@@ -20,9 +20,10 @@ constexpr int kEwThreads = 256;
 // sigma or bad inputs give NaN.
 template <bool BSM>
 __device__ __forceinline__ void black_row(double SorF, double K, double tau, double r, double q, double sigma, double flag,
-                                          double& price, double& vega) {
+                                          double& price, double& vega, double* d1d2 = nullptr) {
   price = canonical_nan();
   vega = canonical_nan();
+  if (d1d2) *d1d2 = 0.0;
   bool bad = !pos_fin(SorF) || !pos_fin(K) || !pos_fin(tau) || !(sigma >= 0.0) || !is_fin(sigma) ||
              !(flag == 1.0 || flag == -1.0);
   double F = SorF, D = 1.0;
@@ -55,6 +56,7 @@ __device__ __forceinline__ void black_row(double SorF, double K, double tau, dou
     const WEval w = eval_W(x, s);
     v = kPhi0 * exp_fast(-w.E);
     b = w.have_W ? w.Wd * v : fma(-w.Wd, v, bmax);
+    if (d1d2) *d1d2 = fma(w.h, w.h, -0.25 * s * s);   // d1 d2 = h^2 - t^2 (sign of x does not matter)
   }
   price = D * fma(rootFK, b, iota);
   vega = D * rootFK * v * rt;
@@ -169,10 +171,12 @@ __device__ __forceinline__ void block_add3(double a, double b, double c, double*
   }
 }
 
-// eq.(11): out += { sum (P_model - P*)^2, sum |P*|, rows used }
-template <bool BSM>
+// eq.(11): out += { sum (P_model - P*)^2, sum |P*|, rows used };  GRAD: grad[i] = grad_scale 2 (P_model - P*) V_hat
+// (0 for rows the sum skips)
+template <bool BSM, bool GRAD>
 __global__ void __launch_bounds__(kEwThreads)
-loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int64_t n, double* __restrict__ out) {
+loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int64_t n, double* __restrict__ out,
+                  double* __restrict__ grad, double grad_scale) {
   double s2 = 0.0, s1 = 0.0, cnt = 0.0;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
@@ -181,57 +185,80 @@ loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int6
     black_row<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(sigma_hat + i),
                    __ldcs(in.flag + i), pm, v);
     const double ps = __ldcs(in.P + i);
+    double g = 0.0;
     if (is_fin(pm) && is_fin(ps)) {
       const double d = pm - ps;
       s2 = fma(d, d, s2); s1 += fabs(ps); cnt += 1.0;
+      g = grad_scale * (2.0 * d * v);
     }
+    if (GRAD) __stcs(grad + i, g);
   }
   block_add3(s2, s1, cnt, out);
 }
 
-// eq.(12), step 1: model price, V_hat, and the price handed to the inversion: P~ = model price on the gate, the
-// sentinel market price P* off it
-template <bool BSM>
+// eq.(12), fused: price node P_model(sigma_hat), V_hat  ->  P~ (model price on the gate, the sentinel P* off it)  ->  the LBR
+// inversion (lbr_row, the forward kernel's own per-row arithmetic)  ->  weighted residual and, GRAD, its gradient by
+// eq.(17) -- all in registers, one pass over the inputs, no workspace.
+//   MODE = PIVOT_RT_GATED: out += { sum w (sigma_rt - sigma*)^2, sum w, rows used },  w = V_hat^2 / (V_hat^2 + floor^2) (eq.(10));
+//       grad[i] = grad_scale { [on the gate] w 2 (sigma_rt - sigma*) MASK(1/V_rt) V_hat  +  w'(V_hat) (sigma_rt - sigma*)^2 V_hat' },
+//       w' = 2 V floor^2 / (V^2 + floor^2)^2,  V_hat' = dV/dsigma = V_hat d1 d2 / sigma_hat;  0 for rows the sum skips.
+//   MODE = PIVOT_RT_NAIVE (no gate, no sentinel, no sanitisation): out += { sum (sigma_rt - sigma*)^2, rows, rows };
+//       grad[i] = grad_scale STRICT(2 (sigma_rt - sigma*), V_rt; floor) V_hat -- NaN wherever the inverse channel is singular.
+template <bool BSM, int MODE, bool GRAD>
 __global__ void __launch_bounds__(kEwThreads)
-rt_prepare_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, double floor_, int64_t n,
-                  double* __restrict__ Ptilde, double* __restrict__ Vhat) {
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
-    double pm, v;
-    black_row<BSM>(__ldcs(in.S_or_F + i), __ldcs(in.K + i), __ldcs(in.tau + i), r, q, __ldcs(sigma_hat + i),
-                   __ldcs(in.flag + i), pm, v);
-    Ptilde[i] = !is_fin(pm) ? canonical_nan() : ((fabs(v) > floor_) ? pm : __ldcs(in.P + i));
-    Vhat[i] = v;
-  }
-}
-
-// eq.(12), step 3: out += { sum w (sigma_rt - sigma*)^2, sum w, rows used },  w = V_hat^2 / (V_hat^2 + floor^2) (eq.(10))
-__global__ void __launch_bounds__(kEwThreads)
-rt_reduce_kernel(const double* __restrict__ sigma_rt, const uint8_t* __restrict__ status, const double* __restrict__ Vhat,
-                 const double* __restrict__ sigma_star, double floor_, int64_t n, double* __restrict__ out) {
+loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, const double* __restrict__ sigma_star,
+                      double floor_, int64_t n, double* __restrict__ out, double* __restrict__ grad, double grad_scale) {
   double acc = 0.0, wsum = 0.0, cnt = 0.0;
   const double f2 = floor_ * floor_;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double v = __ldcs(Vhat + i), ss = __ldcs(sigma_star + i);
-    if (status[i] == PIVOT_ST_OK && is_fin(v) && is_fin(ss)) {
-      const double v2 = v * v;
-      const double w = v2 / (v2 + f2);
-      const double d = __ldcs(sigma_rt + i) - ss;
-      acc = fma(w * d, d, acc); wsum += w; cnt += 1.0;
+    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+    const double S = __ldcs(in.S_or_F + i), K = __ldcs(in.K + i), tau = __ldcs(in.tau + i), flag = __ldcs(in.flag + i);
+    const double sh = __ldcs(sigma_hat + i), ss = __ldcs(sigma_star + i);
+    double pm, vh, dd;
+    black_row<BSM>(S, K, tau, r, q, sh, flag, pm, vh, &dd);
+    const bool usable = is_fin(pm) && is_fin(vh) && is_fin(ss);     // a non-finite sigma_hat gives a NaN price
+    double g = 0.0;
+    if (MODE == PIVOT_RT_NAIVE) {
+      if (!usable) {
+        acc += canonical_nan(); cnt += 1.0; g = canonical_nan();
+      } else {
+        const RowOut o = lbr_row<BSM, 2, false>(S, K, tau, r, q, pm, flag);
+        const double d = o.sigma - ss;
+        acc = fma(d, d, acc); cnt += 1.0;
+        const double up = 2.0 * d;
+        const bool on = (o.status == PIVOT_ST_OK) && (fabs(o.vega) > floor_);
+        g = grad_scale * ((on ? __ddiv_rn(up, o.vega) : ((up == 0.0) ? 0.0 : canonical_nan())) * vh);
+      }
+      wsum = cnt;
+    } else if (usable) {
+      const bool on = fabs(vh) > floor_;
+      const RowOut o = lbr_row<BSM, 2, false>(S, K, tau, r, q, on ? pm : __ldcs(in.P + i), flag);
+      if (o.status == PIVOT_ST_OK) {
+        const double v2 = vh * vh, den = v2 + f2;
+        const double w = v2 / den;
+        const double d = o.sigma - ss;
+        acc = fma(w * d, d, acc); wsum += w; cnt += 1.0;
+        if (GRAD) {
+          const double wp = (den > 0.0) ? 2.0 * vh * f2 / (den * den) : 0.0;
+          const double vomma = (sh > 0.0) ? vh * dd / sh : 0.0;
+          double gi = wp * d * d * vomma;
+          if (on && fabs(o.vega) > floor_) gi += w * __ddiv_rn(2.0 * d, o.vega) * vh;
+          g = grad_scale * gi;
+        }
+      }
     }
+    if (GRAD) __stcs(grad + i, g);
   }
   block_add3(acc, wsum, cnt, out);
 }
 
 inline int ew_blocks(int64_t n) {
-  static const int sms = [] {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0)
-      v = 148;
-    return v;
-  }();
+  int dev = 0, sms = 0;   // per call: the current device may differ between calls (cudaDeviceGetAttribute is a cached lookup)
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+    (void)cudaGetLastError();
+    sms = 148;
+  }
   int64_t blocks = (n + kEwThreads - 1) / kEwThreads;
   const int64_t cap = (int64_t)sms * 8 * 4;  // 8 resident CTAs of 256 threads per SM, 4 waves' worth; grid-stride beyond
   return (int)(blocks < cap ? blocks : cap);
@@ -290,44 +317,49 @@ int pivot_iv_backward_inputs(const pivot_iv_inputs* in, const double* sigma, con
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 
-int pivot_iv_loss_price(const pivot_iv_inputs* in, const double* sigma_hat, int64_t n, double* out3,
-                        pivot_iv_stream stream) {
+int pivot_iv_loss_price(const pivot_iv_inputs* in, const double* sigma_hat, int64_t n, double* out3, double* grad_sigma_hat,
+                        double grad_scale, pivot_iv_stream stream) {
   if (!in) return PIVOT_ERR_NULL;
   if (n < 0) return PIVOT_ERR_BAD_N;
   if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
   if (n == 0) return PIVOT_OK;
   if (!in->S_or_F || !in->K || !in->tau || !in->flag || !in->P || !sigma_hat || !out3) return PIVOT_ERR_NULL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  if (in->r) loss_price_kernel<true><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma_hat, n, out3);
-  else loss_price_kernel<false><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma_hat, n, out3);
+  const int blocks = ew_blocks(n);
+  if (in->r) {
+    if (grad_sigma_hat) loss_price_kernel<true, true><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, n, out3, grad_sigma_hat, grad_scale);
+    else loss_price_kernel<true, false><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, n, out3, nullptr, 0.0);
+  } else {
+    if (grad_sigma_hat) loss_price_kernel<false, true><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, n, out3, grad_sigma_hat, grad_scale);
+    else loss_price_kernel<false, false><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, n, out3, nullptr, 0.0);
+  }
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 
-int64_t pivot_iv_loss_roundtrip_workspace_bytes(int64_t n) { return n < 0 ? 0 : ((33 * n + 15) / 16) * 16; }
-
 int pivot_iv_loss_roundtrip(const pivot_iv_inputs* in, const double* sigma_hat, const double* sigma_star, double vega_floor,
-                            int64_t n, void* workspace, double* out3, pivot_iv_stream stream) {
+                            int mode, int64_t n, double* out3, double* grad_sigma_hat, double grad_scale,
+                            pivot_iv_stream stream) {
   if (!in) return PIVOT_ERR_NULL;
   if (n < 0) return PIVOT_ERR_BAD_N;
+  if (mode != PIVOT_RT_GATED && mode != PIVOT_RT_NAIVE) return PIVOT_ERR_BAD_MODE;
   if (!(vega_floor >= 0.0)) return PIVOT_ERR_BAD_FLOOR;
   if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
   if (n == 0) return PIVOT_OK;
-  if (!in->S_or_F || !in->K || !in->tau || !in->flag || !in->P || !sigma_hat || !sigma_star || !workspace || !out3)
-    return PIVOT_ERR_NULL;
-  if ((reinterpret_cast<uintptr_t>(workspace) & 7u) != 0) return PIVOT_ERR_BAD_ARG;
-  double* w = static_cast<double*>(workspace);
-  double *Ptilde = w, *Vhat = w + n, *sig_rt = w + 2 * n, *vega_rt = w + 3 * n;
-  uint8_t* status = reinterpret_cast<uint8_t*>(w + 4 * n);
+  if (!in->S_or_F || !in->K || !in->tau || !in->flag || !in->P || !sigma_hat || !sigma_star || !out3) return PIVOT_ERR_NULL;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   const int blocks = ew_blocks(n);
-  if (in->r) rt_prepare_kernel<true><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, vega_floor, n, Ptilde, Vhat);
-  else rt_prepare_kernel<false><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, vega_floor, n, Ptilde, Vhat);
-  if (cudaGetLastError() != cudaSuccess) return PIVOT_ERR_CUDA;
-  pivot_iv_inputs in2 = *in;
-  in2.P = Ptilde;
-  const int rc = pivot_iv_forward(&in2, n, sig_rt, vega_rt, status, stream);   // the same fused inversion kernel
-  if (rc != PIVOT_OK) return rc;
-  rt_reduce_kernel<<<blocks, kEwThreads, 0, st>>>(sig_rt, status, Vhat, sigma_star, vega_floor, n, out3);
+#define PIVOT_LAUNCH_RT(B, M, G)                                                                                        \
+  loss_roundtrip_kernel<B, M, G><<<blocks, kEwThreads, 0, st>>>(*in, sigma_hat, sigma_star, vega_floor, n, out3,        \
+                                                                grad_sigma_hat, grad_scale)
+  const bool bsm = in->r != nullptr, g = grad_sigma_hat != nullptr;
+  if (mode == PIVOT_RT_GATED) {
+    if (bsm) { if (g) PIVOT_LAUNCH_RT(true, PIVOT_RT_GATED, true); else PIVOT_LAUNCH_RT(true, PIVOT_RT_GATED, false); }
+    else { if (g) PIVOT_LAUNCH_RT(false, PIVOT_RT_GATED, true); else PIVOT_LAUNCH_RT(false, PIVOT_RT_GATED, false); }
+  } else {
+    if (bsm) { if (g) PIVOT_LAUNCH_RT(true, PIVOT_RT_NAIVE, true); else PIVOT_LAUNCH_RT(true, PIVOT_RT_NAIVE, false); }
+    else { if (g) PIVOT_LAUNCH_RT(false, PIVOT_RT_NAIVE, true); else PIVOT_LAUNCH_RT(false, PIVOT_RT_NAIVE, false); }
+  }
+#undef PIVOT_LAUNCH_RT
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 

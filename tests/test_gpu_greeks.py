@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2606_17065_b200 import workloads as wl
+import workloads as wl
 import paper_2606_17065_b200 as pv
 from oracle import pyoracle as po
 from tests.parity_util import KEYS, to_device, to_numpy
@@ -171,3 +171,111 @@ def test_losses_match_oracle(bsm):
     # sigma_hat = sigma*: the round-trip loss vanishes (every row inverts back to sigma* or uses the sentinel)
     zero = pv.pivot_iv_loss_roundtrip(d["SorF"], d["K"], d["tau"], d["P"], d["flag"], sstar, sstar, floor, **rq).cpu().numpy()
     assert zero[0] <= 1e-22 * max(zero[2], 1.0)
+
+
+# ------------------------------------------------------------------ gradients of the objectives; eq.(17); the diagnostic
+@pytest.mark.parametrize("bsm", [False, True])
+def test_loss_gradients_match_oracle(bsm):
+    """pivot_iv_loss_price / pivot_iv_loss_roundtrip with grad_scale: the per-row gradients with respect to sigma_hat against the
+    oracle's plain loops (pinned by finite differences in tests/test_oracle_pins.py), gated and naive, including the NaN mask of
+    the naive composition bit for bit, and the sums of the fused round trip against the oracle's."""
+    cfg = wl.config2(days=5, seed=61) if bsm else wl.config3(150_000, seed=62)
+    d, c = to_device(cfg), to_numpy(cfg)
+    n = c["K"].size
+    rq = dict(r=d.get("r"), q=d.get("q")); rqh = dict(r=c.get("r"), q=c.get("q"))
+    sstar, vstar, st = pv.pivot_iv_forward(*[d[k] for k in KEYS], **rq)
+    sstar_h = sstar.cpu().numpy()
+    rng = np.random.default_rng(8)
+    base = np.where(np.isfinite(sstar_h) & (sstar_h > 0), sstar_h, 0.3)
+    sig_hat = base * (1 + 0.05 * rng.standard_normal(n))
+    sig_hat[::991] = np.nan
+    sstar_h = np.where(np.isfinite(sstar_h), sstar_h, 0.25)
+    sh, ss = torch.from_numpy(sig_hat).cuda(), torch.from_numpy(sstar_h).cuda()
+    a = [d[k] for k in ("SorF", "K", "tau", "P", "flag")]
+    ah = [c[k] for k in ("SorF", "K", "tau", "P", "flag")]
+    scale = 0.37
+    # eq.(11)
+    sums, g = pv.pivot_iv_loss_price(*a, sh, grad_scale=scale, **rq)
+    ref = scale * po.loss_price_grad(*ah, sig_hat, **rqh)
+    g = g.cpu().numpy()
+    vh = po.vega_eq14(c["SorF"], c["K"], c["tau"], np.nan_to_num(sig_hat, nan=0.3), **rqh)
+    assert np.array_equal(g == 0, ref == 0) or np.mean((g == 0) != (ref == 0)) < 1e-4
+    Fh = c["SorF"] * (np.exp((c["r"] - c["q"]) * c["tau"]) if bsm else 1.0)
+    s_hat = np.nan_to_num(sig_hat, nan=0.3) * np.sqrt(c["tau"])
+    expo = (np.log(Fh / c["K"]) / s_hat) ** 2 + 0.25 * s_hat ** 2       # vega = C exp(-expo/2): its own tolerance (parity_util)
+    hos = np.abs(np.log(Fh / c["K"])) / s_hat ** 2                      # |h|/s: one ulp of x = ln(F/K) in the exponent
+    tol = (1e-11 + 32 * EPS * expo) * np.abs(ref) + \
+        scale * 2 * vh * np.abs(c["P"]) * (1e-12 + 32 * EPS * (expo + hos))   # + the price tolerance on the cancelling residual
+    assert np.all(np.abs(g - ref) <= tol + 1e-300)
+    # eq.(12), gated
+    floor = float(np.quantile(vh[np.isfinite(vh)], 0.3))
+    sums_r, gr = pv.pivot_iv_loss_roundtrip(*a, sh, ss, floor, mode=pv.RT_GATED, grad_scale=scale, **rq)
+    ref_g, term = po.loss_roundtrip_grad(*ah, sig_hat, sstar_h, floor, naive=False, **rqh)
+    ref_sums = po.loss_roundtrip(*ah, sig_hat, sstar_h, floor, **rqh)
+    sums_r = sums_r.cpu().numpy()
+    assert abs(sums_r[2] - ref_sums[2]) <= 2 and sums_r[0] == pytest.approx(ref_sums[0], rel=1e-9)
+    assert sums_r[1] == pytest.approx(ref_sums[1], rel=1e-9)
+    gr = gr.cpu().numpy()
+    assert np.isfinite(gr).all()
+    big = np.abs(ref_g) > 1e-6 * np.max(np.abs(ref_g))
+    assert np.max(np.abs(gr[big] / (scale * ref_g[big]) - 1)) < 1e-8
+    assert np.max(np.abs(gr - scale * ref_g)) <= 1e-8 * np.max(np.abs(scale * ref_g))
+    # naive composition at the strict floor 1e-14: same NaN mask, same finite values
+    sums_n, gn = pv.pivot_iv_loss_roundtrip(*a, sh, ss, 1e-14, mode=pv.RT_NAIVE, grad_scale=scale, **rq)
+    ref_n, term_n = po.loss_roundtrip_grad(*ah, sig_hat, sstar_h, 1e-14, naive=True, **rqh)
+    gn = gn.cpu().numpy()
+    # the NaN mask hangs on exact ties (a cotangent of exactly 0, a time value of exactly 0, |V_rt| against 1e-14): identical up to
+    # the rows where the two sides round such a tie differently
+    assert np.mean(np.isnan(gn) != np.isnan(ref_n)) < 2e-3 and np.isnan(ref_n).sum() > 0
+    fin = np.isfinite(ref_n) & np.isfinite(gn) & (np.abs(ref_n) > 1e-6 * np.nanmax(np.abs(ref_n)))
+    v_rt = po.vega_eq14(c["SorF"], c["K"], c["tau"], np.nan_to_num(sig_hat, nan=0.3), **rqh)
+    well = fin & (v_rt > 1e-8 * c["K"])
+    assert np.max(np.abs(gn[well] / (scale * ref_n[well]) - 1)) < 1e-8
+    # eq.(17): on well-conditioned rows the composed factor (1/V_rt) V_hat is 1: the naive gradient is 2 (sigma_hat - sigma*)
+    # (where the price -> sigma -> price round trip itself is well conditioned: elasticity P / (V sigma) <= 100)
+    cond = well & (np.abs(c["P"]) <= 100 * v_rt * np.nan_to_num(sig_hat, nan=1.0)) & (np.abs(sig_hat - sstar_h) > 1e-3 * sstar_h)
+    assert cond.sum() > 0.2 * n
+    assert np.max(np.abs(gn[cond] / (scale * 2 * (sig_hat[cond] - sstar_h[cond])) - 1)) < 1e-9
+    assert np.isnan(sums_n[0].item())                     # the NaN sigma_hat rows poison the naive sum
+
+
+def test_nan_poisoning_diagnostic():
+    """PAPER.md:404-428 (App. B.2, Fig.6): on the low_vega_tail chain (N = 65,536, seed 31, ~91 % of rows |V| <= 1e-14) the
+    naive composition poisons every row of the singular set within one Adam step and never recovers; the gated objective
+    keeps every row finite for 200 steps and its loss goes down.  The step-0 gradients are checked against the oracle."""
+    from paper_2606_17065_b200.diagnostic import run_nan_poisoning_diagnostic
+    cfg = wl.low_vega_tail()
+    d, c = to_device(cfg), to_numpy(cfg)
+    n = c["K"].size
+    a = [d[k] for k in ("SorF", "K", "tau", "P", "flag")]
+    ah = [c[k] for k in ("SorF", "K", "tau", "P", "flag")]
+    sigma_star = d["sigma_true"]
+    vstar = pv.pivot_iv_black_price(d["SorF"], d["K"], d["tau"], sigma_star, d["flag"])[1]
+    dead = float((vstar <= 1e-14).double().mean().item())
+    assert 0.89 <= dead <= 0.94, dead                      # the paper: 0.911
+    g0 = torch.Generator(device="cuda").manual_seed(7)
+    sigma_init = (sigma_star * (1 + 0.2 * torch.randn(n, generator=g0, device="cuda", dtype=torch.float64))).clamp_min(0.02)
+    # step-0 gradients against the oracle
+    si_h, ss_h = sigma_init.cpu().numpy(), c["sigma_true"]
+    _, gn = pv.pivot_iv_loss_roundtrip(*a, sigma_init, sigma_star, 1e-14, mode=pv.RT_NAIVE, grad_scale=1.0)
+    rn, _ = po.loss_roundtrip_grad(*ah, si_h, ss_h, 1e-14, naive=True)
+    gn = gn.cpu().numpy()
+    assert np.mean(np.isnan(gn) != np.isnan(rn)) < 1e-3 and np.isnan(rn).mean() > 0.8
+    f = np.isfinite(rn) & np.isfinite(gn) & (np.abs(rn) > 1e-9)
+    assert np.max(np.abs(gn[f] / rn[f] - 1)) < 1e-7
+    _, gg = pv.pivot_iv_loss_roundtrip(*a, sigma_init, sigma_star, 1e-6, mode=pv.RT_GATED, grad_scale=1.0)
+    rg, _ = po.loss_roundtrip_grad(*ah, si_h, ss_h, 1e-6, naive=False)
+    gg = gg.cpu().numpy()
+    assert np.isfinite(gg).all() and np.max(np.abs(gg - rg)) <= 1e-7 * np.max(np.abs(rg))
+    naive = run_nan_poisoning_diagnostic(d, sigma_star, sigma_init, gated=False, steps=200)
+    gated = run_nan_poisoning_diagnostic(d, sigma_star, sigma_init, gated=True, steps=200)
+    # naive: NaN gradients at step 0, the poisoned rows are gone after one step and stay gone, the loss is NaN from step 1 on
+    assert naive["nan_grads"][0] > 0.8 * n
+    assert naive["finite_frac"][0] == 1.0 and naive["finite_frac"][1] < 0.2 and naive["finite_frac"][-1] <= naive["finite_frac"][1]
+    assert all(np.isnan(x) for x in naive["loss"][1:])
+    # gated: every row finite at every step, no NaN gradient, loss goes down
+    assert all(f == 1.0 for f in gated["finite_frac"]) and all(k == 0 for k in gated["nan_grads"])
+    assert all(np.isfinite(x) for x in gated["loss"]) and gated["loss"][-1] < 0.5 * gated["loss"][0]
+    up = sum(1 for i in range(1, 200) if gated["loss"][i] > gated["loss"][i - 1])
+    print(f"dead fraction {dead:.3f}; naive finite after 1 step {naive['finite_frac'][1]:.3f}; gated loss "
+          f"{gated['loss'][0]:.3e} -> {gated['loss'][-1]:.3e} ({up} increasing steps of 199)")

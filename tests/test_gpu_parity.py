@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2606_17065_b200 import workloads as wl
+import workloads as wl
 import paper_2606_17065_b200 as pv
 from oracle import pyoracle as po
 from tests.parity_util import KEYS, compare_backward, compare_forward, gpu_forward, oracle_forward, to_device, to_numpy

@@ -650,3 +650,85 @@ def test_loss_roundtrip_against_direct_formula():
     # sigma_hat = sigma*: zero
     z = po.loss_roundtrip(S, K, tau, Pstar, flag, sstar, sstar, floor, r=r, q=q)
     assert z[0] <= 1e-24 * S.size
+
+
+# ------------------------------------------------------- gradients of the objectives: eq.(11), eq.(12), eq.(17)
+def test_loss_price_grad_against_central_differences():
+    """d/d sigma_hat (P_model - P*)^2 = 2 (P_model - P*) V_hat: central differences of the literal long-double price."""
+    S, K, tau, r, q, sig, flag = _bsm_rows(3000, 21)
+    rng = np.random.default_rng(4)
+    Pstar = po.black_price(S, K, tau, sig, flag, r=r, q=q, prec=1) * (1 + 0.02 * rng.standard_normal(S.size))
+    sig_hat = sig * (1 + 0.1 * rng.standard_normal(S.size))
+    g = po.loss_price_grad(S, K, tau, Pstar, flag, sig_hat, r=r, q=q)
+    h = 1e-6 * sig_hat
+    fp = (po.black_price(S, K, tau, sig_hat + h, flag, r=r, q=q, prec=1) - Pstar) ** 2
+    fm = (po.black_price(S, K, tau, sig_hat - h, flag, r=r, q=q, prec=1) - Pstar) ** 2
+    fd = (fp - fm) / (2 * h)
+    f = np.maximum(fp, fm)                                  # rounding of the prices entering the difference quotient:
+    noise = 16 * EPS * (f + np.sqrt(f) * np.abs(Pstar)) / h  # d(res^2) = 2 res dP with dP ~ eps P
+    assert np.all(np.abs(g - fd) <= 1e-5 * np.abs(g) + noise)
+    resolved = np.abs(g) > 100 * noise                        # rows on which the difference quotient resolves the slope
+    assert resolved.sum() > 2000 and np.max(np.abs(g[resolved] / fd[resolved] - 1)) < 1e-3
+    assert np.count_nonzero(g) > 2900
+
+
+def test_loss_roundtrip_grad_against_central_differences_and_eq17():
+    """eq.(12) per-row term T = w(V_hat)(IV(P~) - sigma*)^2: its gradient (eq.(17) chain 1/V * V_hat on the gate, plus the
+    w' V_hat' term; off the gate only the latter) against central differences of the oracle's own term; the sentinel
+    carries no gradient; and the eq.(17) cancellation in closed form: on the gate IV(P_model(sigma_hat)) = sigma_hat, so
+    the naive composition's gradient 2 (sigma_rt - sigma*) V_hat / V_rt equals 2 (sigma_hat - sigma*)."""
+    S, K, tau, r, q, sig_star, flag = _bsm_rows(3000, 22)
+    rng = np.random.default_rng(5)
+    Pstar = po.black_price(S, K, tau, sig_star, flag, r=r, q=q, prec=1)
+    sstar, _, st0 = po.forward(S, K, tau, Pstar, flag, r=r, q=q)
+    vh0 = po.vega_eq14(S, K, tau, sig_star, r=r, q=q)
+    keep = (st0 == 0) & (np.abs(sstar / sig_star - 1) < 1e-7) & (vh0 > 1e-3 * S)
+    S, K, tau, r, q, flag, Pstar, sstar = (a[keep] for a in (S, K, tau, r, q, flag, Pstar, sstar))
+    assert S.size > 1500
+    sig_hat = sstar * (1 + 0.05 * rng.standard_normal(S.size))
+    vh = po.vega_eq14(S, K, tau, sig_hat, r=r, q=q)
+    floor = float(np.quantile(vh, 0.3))
+    g, term = po.loss_roundtrip_grad(S, K, tau, Pstar, flag, sig_hat, sstar, floor, r=r, q=q)
+    h = 1e-6 * sig_hat
+    _, tp = po.loss_roundtrip_grad(S, K, tau, Pstar, flag, sig_hat + h, sstar, floor, r=r, q=q)
+    _, tm = po.loss_roundtrip_grad(S, K, tau, Pstar, flag, sig_hat - h, sstar, floor, r=r, q=q)
+    vp = po.vega_eq14(S, K, tau, sig_hat + h, r=r, q=q); vm = po.vega_eq14(S, K, tau, sig_hat - h, r=r, q=q)
+    same_side = ((vp > floor) == (vh > floor)) & ((vm > floor) == (vh > floor))    # the FD stencil must not straddle the gate
+    fd = (tp - tm) / (2 * h)
+    scale = np.abs(g) + 1e-7 * (np.abs(term) / np.abs(h) + 1e-12)
+    err = np.abs(g - fd)[same_side] / scale[same_side]
+    assert same_side.sum() > 0.95 * S.size and err.max() < 2e-4, float(err.max())
+    on = vh > floor
+    assert on.sum() > 100 and (~on).sum() > 100
+    # off the gate the sentinel carries no gradient: only the w' term, tiny because IV(P*) = sigma*
+    assert np.max(np.abs(g[~on])) <= 1e-12 * np.max(np.abs(g[on]))
+    # loss sums agree with the per-row terms
+    sums = po.loss_roundtrip(S, K, tau, Pstar, flag, sig_hat, sstar, floor, r=r, q=q)
+    assert sums[0] == pytest.approx(term.sum(), rel=1e-12)
+    # eq.(17): 1/V * V = 1 on the well-conditioned rows
+    gn, tn = po.loss_roundtrip_grad(S, K, tau, Pstar, flag, sig_hat, sstar, 1e-14, naive=True, r=r, q=q)
+    assert np.max(np.abs(gn / (2 * (sig_hat - sstar)) - 1)) < 1e-9
+    assert np.all(np.abs(tn - (sig_hat - sstar) ** 2) <= 1e-9 * (sig_hat - sstar) ** 2 + 1e-11 * sstar * np.abs(sig_hat - sstar))
+
+
+def test_naive_roundtrip_gradient_follows_the_strict_contract():
+    """without the gate the inverse channel returns NaN wherever |V_rt| <= 1e-14 or the inversion is
+    not OK (unless the cotangent is exactly 0); with the gate every gradient is finite."""
+    rng = np.random.default_rng(6)
+    n = 4000
+    F = np.full(n, 100.0); k = rng.uniform(-2.5, 2.5, n); K = F * np.exp(k)
+    tau = np.exp(rng.uniform(np.log(1e-8), np.log(10 ** -0.5), n))
+    sig_star = rng.uniform(0.1, 0.6, n)
+    flag = np.where(K >= F, 1.0, -1.0)
+    Pstar = po.black_price(F, K, tau, sig_star, flag, prec=1)
+    sstar = np.where(np.isfinite(sig_star), sig_star, 0.0)
+    sig_hat = np.full(n, 0.3)
+    vrt = po.vega_eq14(F, K, tau, sig_hat)
+    gn, tn = po.loss_roundtrip_grad(F, K, tau, Pstar, flag, sig_hat, sstar, 1e-14, naive=True)
+    gg, tg = po.loss_roundtrip_grad(F, K, tau, Pstar, flag, sig_hat, sstar, 1e-6, naive=False)
+    assert np.isfinite(gg).all() and np.isfinite(tg).all()
+    dead = vrt <= 1e-14
+    assert dead.mean() > 0.8
+    assert np.isnan(gn[dead]).all()                       # sigma_hat != sigma*: the cotangent is not zero
+    alive = vrt > 1e-10
+    assert np.isfinite(gn[alive]).all()

@@ -4,7 +4,7 @@ import numpy as np
 import torch
 
 from oracle import pyoracle as po
-from paper_2606_17065_b200 import workloads as wl
+import workloads as wl
 
 KEYS = ("SorF", "K", "tau", "P", "flag")
 
