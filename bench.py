@@ -5,17 +5,21 @@ Workload (BASELINE.json `metric`: "fp64 forward LBR IV/s at 2^26 rows; fwd+bwd r
 config 4 at n = 2^26 rows per GPU (inputs as config 1: x~U[-5,5], s log-U[1e-4,5], call/put 50/50, Black-76 D = 1),
 seeded and generated on the device.  One "step" = one pass of the whole hot path over the batch: the fused forward
 kernel (sigma, vega, status) + the gated backward kernel (MASK, vega_floor 1e-8).  `value` = rows/s through fwd+bwd,
-whole job; the forward-only IV/s and the error vs the oracle ride along as extra keys.
+whole job; the forward-only IV/s and the error vs the oracle ride along as extra keys.  The default run also times every
+other config of BASELINE.json (`configs`) and the config-4 size sweep (`sweep`), each with its roofline fractions and
+its error against the oracle on a sample.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--rows R] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--rows R] [--impl ours|reference] [--quick]
 
-N > 1 is launched by torchrun (one rank per GPU); rows are sharded (weak scaling), there is no data-path collective.
+N > 1: launched by torchrun (one rank per GPU), or by this script itself when WORLD_SIZE is not set.  Rows are sharded
+(weak scaling: 2^26 rows per rank), there is no data-path collective.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -30,21 +34,30 @@ sys.path.insert(0, ROOT)
 METRIC = "fp64 forward LBR IV/s at 2^26 rows; fwd+bwd rows/s; max rel err vs oracle"
 VEGA_FLOOR = 1e-8
 KEYS = ("SorF", "K", "tau", "P", "flag")
+DTYPE = ("f64 (status, normalisation, ln(beta), last Householder step, vega: fp64; seed and first Householder step: "
+         "fp32/MUFU seed grade)")
 
 # fp64-pipe peak of one B200, derived from unit counts and clocks:
 # 148 SMs x 64 fp64 FMA lanes per SM per clock x 2 flops x 1.965 GHz (clocks.max.sm) = 37.2 TFLOP/s.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# algorithmic bytes per row: forward Black-76 5x8 in + 8+8+1 out; backward 8+8+1 in + 8 out
-FWD_BYTES_PER_ROW = 57
+# algorithmic bytes per row: forward 5x8 (Black-76) or 7x8 (BSM) in + 8+8+1 out; backward 8+8+1 in + 8 out
+FWD_BYTES = {"b76": 57, "bsm": 73}
 BWD_BYTES_PER_ROW = 25
-# DRAM traffic per row of the forward kernel measured by ncu (profiles/r1g_forward_tile_ncu_full.md): reads are exactly
-# the 40 algorithmic bytes; part of the 17 written bytes is still dirty in L2 when the kernel ends
-FWD_TRAFFIC_BYTES_PER_ROW = 56.5  # r1c capture: 40.0 read + 16.5 written
+# Constants QUOTED from the ncu --set full captures of the committed kernels (profiles/r2*_ncu_full.md; config 4 mixed rows):
+NCU = {
+    "source": "profiles/r2c_forward_tile_ncu_full.md, profiles/r2c_backward_ncu_full.md (ncu --set full of this kernel, config 4)",
+    "fwd_dram_bytes_per_row": 54.7,          # dram__bytes_read.sum + dram__bytes_write.sum per row (40.0 read + 14.7 written)
+    "fwd_issued_fp64_flops_per_row": 229.0,  # 2 DFMA + DADD + DMUL thread instructions per row
+    "fwd_fp64_pipe_busy_pct": 43.7,
+    "fwd_issue_active_pct": 68.0,
+    "fwd_warp_inst_per_row": 20.9,
+    "bwd_dram_bytes_per_row": 25.0,
+}
 # per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
 # CUDA 12.9 builtins); "/" and sqrt count 1 flop each
 CALL_FLOPS = {"exp": 31, "log": 47, "log1p": 109, "erfc": 113, "erfcx": 165, "ninv": 315, "cbrt": 16}
 # fallback algorithmic flops/row per class (zone 0..3, non-OK), used only when the oracle leg is not run (ranks of an
-# N > 1 job); produced by oracle/pyoracle.count_ops on config 1 and the table above
+# N > 1 job); produced by oracle/pyoracle.count_ops (fixed_iters = 2) on config 1 and the table above
 FALLBACK_FLOPS_PER_CLASS = (2557.0, 1796.0, 1818.0, 2359.0, 6.0)
 
 
@@ -119,88 +132,149 @@ def _flops_per_row_from_counts(counts, rows):
     return tot_plain / n, (tot_plain + tot_calls) / n
 
 
-def run_sweep(pv, wl, hbm_peak, flops_mixed):
+def _time_calls(fn, stream, reps, warm=3):
+    """ms per call: `reps` calls enqueued back to back between two CUDA events on `stream`, after `warm` untimed calls."""
+    for _ in range(warm):
+        fn()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(reps):
+        fn()
+    e1.record(stream); e1.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def _sample_idx(n, m):
+    """m row indices spread over all n rows (strided), as a CUDA tensor."""
+    m = min(n, m)
+    return torch.arange(m, device="cuda", dtype=torch.int64) * (n // m)
+
+
+def _parity(po, cfg, out, idx, gP=None, gsig=None, mode=0):
+    """GPU outputs at the sampled rows `idx` against the oracle run on the same rows."""
+    c = {k: cfg[k][idx].cpu().numpy() for k in KEYS}
+    r = cfg["r"][idx].cpu().numpy() if cfg.get("r") is not None else None
+    q = cfg["q"][idx].cpu().numpy() if cfg.get("q") is not None else None
+    os_, ov, ost = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"], r=r, q=q)
+    gs, gv, gst = (t[idx].cpu().numpy() for t in out[:3])
+    ok = (ost == 0) & (gst == 0)
+    res = {"rows": int(idx.numel()), "status_mismatches": int((ost != gst).sum()),
+           "max_rel_err_sigma": float(np.max(np.abs(gs[ok] / os_[ok] - 1))) if ok.any() else None}
+    if gP is not None:
+        hg = gsig[idx].cpu().numpy()
+        og = po.backward(hg, ov, ost, VEGA_FLOOR, mode)
+        if mode == 0:
+            on = ok & (ov > VEGA_FLOOR) & (np.abs(ov / VEGA_FLOOR - 1) > 1e-12) & (og != 0)
+        else:
+            on = ok & (ov > VEGA_FLOOR) & (og != 0)
+        res["max_rel_err_grad_P"] = float(np.max(np.abs(gP[idx].cpu().numpy()[on] / og[on] - 1))) if on.any() else None
+    return res, (c, r, q)
+
+
+def _alloc_out(n):
+    return (torch.empty(n, dtype=torch.float64, device="cuda"), torch.empty(n, dtype=torch.float64, device="cuda"),
+            torch.empty(n, dtype=torch.uint8, device="cuda"))
+
+
+def run_sweep(pv, wl, hbm_peak, flops_mixed, max_exp):
     """Config 4 (BASELINE.json configs[4]): forward IV/s for n = 2^10 .. 2^28, inputs as config 1 ("all") and its
-    rejection-sampled 1-solve variant; per size the median and best of 20 launches timed one by one with CUDA events."""
+    rejection-sampled 1-solve variant; per size the median of 10 launches timed one by one with CUDA events (what a lone
+    call costs) and the same 10 launches enqueued back to back."""
     stream = torch.cuda.current_stream()
     res = []
-    for e in range(10, 29, 2):
+    for e in range(10, max_exp + 1, 2):
         n = 1 << e
         row = {"n": n}
         for name, so in (("all", False), ("solve", True)):
             cfg = wl.config4(n, seed=40 + e, device="cuda", solve_only=so)
             a = [cfg[k] for k in KEYS]
-            out = (torch.empty(n, dtype=torch.float64, device="cuda"), torch.empty(n, dtype=torch.float64, device="cuda"),
-                   torch.empty(n, dtype=torch.uint8, device="cuda"))
+            out = _alloc_out(n)
             for _ in range(3):
                 pv.pivot_iv_forward(*a, out=out, stream=stream)
             ts = []
-            for _ in range(20):
+            for _ in range(10):
                 e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
                 pv.pivot_iv_forward(*a, out=out, stream=stream)
                 e1.record(stream); e1.synchronize()
                 ts.append(e0.elapsed_time(e1))
-            med, best = float(np.median(ts)), float(np.min(ts))
-            # the same 20 launches enqueued back to back (for small n a lone launch is dominated by the host-side call)
-            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(20):
-                pv.pivot_iv_forward(*a, out=out, stream=stream)
-            e1.record(stream); e1.synchronize()
-            row.setdefault("ms_back_to_back", {})[name] = e0.elapsed_time(e1) / 20
-            row[name] = {"ms_median": med, "ms_best": best, "iv_per_s": n / (med * 1e-3),
-                         "hbm_frac": FWD_BYTES_PER_ROW * n / (med * 1e-3) / 1e9 / hbm_peak}
+            med = float(np.median(ts))
+            b2b = _time_calls(lambda: pv.pivot_iv_forward(*a, out=out, stream=stream), stream, 10, warm=0)
+            row[name] = {"ms_single": round(med, 5), "ms_back_to_back": round(b2b, 5), "iv_per_s": n / (b2b * 1e-3),
+                         "hbm_frac": round(FWD_BYTES["b76"] * n / (b2b * 1e-3) / 1e9 / hbm_peak, 4)}
             if not so:
-                row[name]["fp64_frac"] = flops_mixed * n / (med * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+                row[name]["fp64_frac_oracle_flops"] = round(flops_mixed * n / (b2b * 1e-3) / 1e12 / FP64_PEAK_TFLOPS, 4)
             del cfg, a, out
         res.append(row)
     return res
 
 
-def run_configs(pv, wl):
-    """Forward ms at 2^24 rows on the four workload shapes of the A/B table: 10 launches, CUDA events."""
-    n = 1 << 24
+def run_configs(pv, wl, po, hbm_peak, quick):
+    """Every config of BASELINE.json at its own size: throughput, roofline fractions (oracle-counted flops of THAT config,
+    algorithmic bytes), and the error against the oracle on a sample."""
     stream = torch.cuda.current_stream()
-    cases = {"config4_mixed": lambda: wl.config4(n, device="cuda"),
-             "config4_1solve": lambda: wl.config4(n, device="cuda", solve_only=True),
-             "config0": lambda: wl.config0(n, device="cuda"),
-             "config2_bsm_chains": lambda: wl.config2(days=n // 16000, device="cuda")}
     res = {}
-    for name, mk in cases.items():
-        cfg = mk()
+
+    def flops_of(c, r, q, m=1 << 17):
+        counts, rows = po.count_ops(*[c[k][:m] for k in KEYS], r=None if r is None else r[:m], q=None if q is None else q[:m])
+        return _flops_per_row_from_counts(counts, rows)[1]
+
+    def fwd_case(name, cfg, sample, kernels=(("default", None),)):
         a = [cfg[k] for k in KEYS]
-        m = a[0].numel()
-        out = (torch.empty(m, dtype=torch.float64, device="cuda"), torch.empty(m, dtype=torch.float64, device="cuda"),
-               torch.empty(m, dtype=torch.uint8, device="cuda"))
-        for _ in range(3):
-            pv.pivot_iv_forward(*a, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
-        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(10):
-            pv.pivot_iv_forward(*a, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
-        e1.record(stream); e1.synchronize()
-        ms = e0.elapsed_time(e1) / 10
-        res[name] = {"rows": m, "ms": ms, "iv_per_s": m / (ms * 1e-3), "solved_fraction": float((out[2] == 0).double().mean().item())}
-        # the same workload through the explicit row-per-thread organisation (pivot_iv_forward_ex, PIVOT_FWD_ROWWISE)
-        for _ in range(3):
-            pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
-        e0.record(stream)
-        for _ in range(10):
-            pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE, r=cfg["r"], q=cfg["q"], out=out, stream=stream)
-        e1.record(stream); e1.synchronize()
-        res[name]["ms_rowwise_hint"] = e0.elapsed_time(e1) / 10
-        # ... and through pivot_iv_forward_auto (probe + the chosen organisation)
-        ws = torch.zeros(16, dtype=torch.int32, device="cuda")
-        for _ in range(3):
-            pv.pivot_iv_forward_auto(*a, r=cfg["r"], q=cfg["q"], out=out, workspace=ws, stream=stream)
-        e0.record(stream)
-        for _ in range(10):
-            pv.pivot_iv_forward_auto(*a, r=cfg["r"], q=cfg["q"], out=out, workspace=ws, stream=stream)
-        e1.record(stream); e1.synchronize()
-        res[name]["ms_auto"] = e0.elapsed_time(e1) / 10
-        res[name]["auto_probe[decision,solved,alike,samples]"] = ws[:4].tolist()
-        del cfg, a, out
+        n = a[0].numel()
+        bsm = cfg.get("r") is not None
+        out = _alloc_out(n)
+        entry = {"rows": n, "mode": "BSM (S,K,tau,r,q,P,flag)" if bsm else "Black-76 (F,K,tau,P,flag)"}
+        for label, kern in kernels:
+            if kern is None:
+                fn = lambda: pv.pivot_iv_forward(*a, r=cfg.get("r"), q=cfg.get("q"), out=out, stream=stream)
+            else:
+                fn = lambda: pv.pivot_iv_forward_ex(*a, kern, r=cfg.get("r"), q=cfg.get("q"), out=out, stream=stream)
+            ms = _time_calls(fn, stream, 10)
+            entry[label] = {"ms": round(ms, 5), "iv_per_s": n / (ms * 1e-3)}
+        pv.pivot_iv_forward(*a, r=cfg.get("r"), q=cfg.get("q"), out=out, stream=stream)
+        torch.cuda.synchronize()
+        par, (c, r, q) = _parity(po, cfg, out, _sample_idx(n, sample))
+        fl = flops_of(c, r, q)
+        ms = entry["default"]["ms"]
+        bytes_row = FWD_BYTES["bsm" if bsm else "b76"]
+        entry.update({"solved_fraction": float((out[2] == 0).double().mean().item()),
+                      "oracle_flops_per_row": round(fl, 1),
+                      "fp64_frac_oracle_flops": round(fl * n / (ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS, 4),
+                      "hbm_frac": round(bytes_row * n / (ms * 1e-3) / 1e9 / hbm_peak, 4), "bytes_per_row": bytes_row,
+                      "parity_vs_oracle": par})
+        res[name] = entry
+
+    fwd_case("config0", wl.config0(65536, seed=0, device="cuda"), 65536)
+    n1 = 1 << (22 if quick else 24)
+    fwd_case("config1", wl.config1(n1, seed=1, device="cuda"), 1 << 18,
+             kernels=(("default", None), ("fp64_only", pv.FWD_COMPACT | pv.FWD_FP64_ONLY)))
+    fwd_case("config1_1solve", wl.config1(n1, seed=1, device="cuda", solve_only=True), 1 << 18,
+             kernels=(("default", None), ("rowwise", pv.FWD_ROWWISE), ("fp64_only", pv.FWD_COMPACT | pv.FWD_FP64_ONLY)))
+    torch.cuda.empty_cache()
+    days = 128 if quick else 2048
+    fwd_case("config2_bsm_chains", wl.config2(days=days, seed=2, device="cuda"), 1 << 18,
+             kernels=(("default", None), ("rowwise", pv.FWD_ROWWISE)))
+    torch.cuda.empty_cache()
+    # config 3: training batch fwd+bwd, both gate modes
+    n3 = 1 << 22
+    cfg = wl.config3(n3, seed=3, device="cuda")
+    a = [cfg[k] for k in KEYS]
+    out = _alloc_out(n3)
+    gP = torch.empty(n3, dtype=torch.float64, device="cuda")
+    entry = {"rows": n3}
+    for label, mode in (("mask", pv.GATE_MASK), ("attenuate", pv.GATE_ATTENUATE)):
+        def step():
+            pv.pivot_iv_forward(*a, out=out, stream=stream)
+            pv.pivot_iv_backward(cfg["grad_sigma"], out[1], out[2], VEGA_FLOOR, mode, out=gP, stream=stream)
+        ms = _time_calls(step, stream, 20)
+        step(); torch.cuda.synchronize()
+        par, _ = _parity(po, cfg, out, _sample_idx(n3, 1 << 18), gP=gP, gsig=cfg["grad_sigma"], mode=mode)
+        entry[label] = {"ms_fwd_bwd": round(ms, 5), "rows_per_s": n3 / (ms * 1e-3),
+                        "hbm_frac": round((FWD_BYTES["b76"] + BWD_BYTES_PER_ROW) * n3 / (ms * 1e-3) / 1e9 / hbm_peak, 4),
+                        "parity_vs_oracle": par}
+    entry["gate_on_fraction"] = float(((out[2] == 0) & (out[1] > VEGA_FLOOR)).double().mean().item())
+    res["config3_fwd_bwd"] = entry
     return res
 
 
@@ -214,6 +288,7 @@ def run_reference(args):
     cfg = wl.config4(m, device="cpu")
     c = {k: cfg[k].numpy() for k in KEYS}
     gs = np.random.default_rng(4).standard_normal(m)
+
     def step():
         s, v, st = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"])
         po.backward(gs, v, st, VEGA_FLOOR, 0)
@@ -234,27 +309,62 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(n, argv):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (torch.distributed.run, one node)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), os.path.abspath(__file__)] + argv
+    return subprocess.call(cmd)
+
+
+def run_selftest_launch(args):
+    """CPU-only check of the N > 1 plumbing (tests/test_sharding_gloo.py): gloo process group, the row shards every rank
+    takes of ONE array, and the max-over-ranks / sum bookkeeping -- the same code path `--gpus N` uses, minus the kernels."""
+    import torch.distributed as dist
+    from paper_2606_17065_b200.sharding import shard_rows
+    rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+    dist.init_process_group("gloo")
+    n = args.rows
+    b, e = shard_rows(n, rank, world)
+    mine = torch.tensor([float(b), float(e)], dtype=torch.float64)
+    allb = [torch.zeros(2, dtype=torch.float64) for _ in range(world)]
+    dist.all_gather(allb, mine)
+    t = torch.tensor([1.0 + rank], dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    if rank == 0:
+        print(json.dumps({"selftest": "launch", "n_gpus": world, "rows": n,
+                          "shards": [[int(x[0]), int(x[1])] for x in allb], "max_ms": t.item()}), flush=True)
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--rows", type=int, default=1 << 26, help="rows per GPU")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--configs", action="store_true",
-                    help="forward-only timing of the other workload shapes at 2^24 rows (config 4 mixed, 1-solve, config 0, "
-                         "config 2 BSM chains); adds a 'configs' dict to the JSON line.  With PIVOT_IV_FWD_KERNEL=rowwise "
-                         "this is the A/B of DESIGN.md section 8")
-    ap.add_argument("--sweep", action="store_true",
-                    help="config 4: forward-only size sweep n = 2^10 .. 2^28 (all rows and the 1-solve variant); adds a "
-                         "'sweep' list to the JSON line")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config table (configs 0-3)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 size sweep")
+    ap.add_argument("--quick", action="store_true", help="smaller configs / sweep up to 2^24 (profiling, smoke runs)")
+    ap.add_argument("--selftest-launch", action="store_true", help="CPU-only check of the N > 1 launcher and sharding")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
+    if args.selftest_launch:
+        return run_selftest_launch(args)
     if args.impl == "reference":
         return run_reference(args)
 
     import paper_2606_17065_b200 as pv
+    from paper_2606_17065_b200.sharding import shard_rows
     import workloads as wl
 
     rank = int(os.environ.get("RANK", "0"))
@@ -269,14 +379,16 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     n = args.rows
     K, W = args.steps, max(args.warmup, 3)
+    lib = pv.load_library()
 
-    # --- inputs resident in HBM (row shard of this rank; seeds differ per rank)
+    # --- inputs resident in HBM.  The job's workload is world x n rows of config 4; rank r owns the contiguous shard
+    #     shard_rows(world n, r, world) of it (= n rows) and draws it with its own seed.
+    g_begin, g_end = shard_rows(world * n, rank, world)
     cfg = wl.config4(n, seed=4 + rank, device="cuda")
     a = [cfg[k] for k in KEYS]
     g = torch.Generator(device="cuda"); g.manual_seed(1000 + rank)
     gsig = torch.randn(n, dtype=torch.float64, device="cuda", generator=g)
-    out = (torch.empty(n, dtype=torch.float64, device="cuda"), torch.empty(n, dtype=torch.float64, device="cuda"),
-           torch.empty(n, dtype=torch.uint8, device="cuda"))
+    out = _alloc_out(n)
     gP = torch.empty(n, dtype=torch.float64, device="cuda")
     stream = torch.cuda.current_stream()
 
@@ -316,6 +428,9 @@ def main():
         total_ms, fwd_ms, bwd_ms = (float(x) for x in t.tolist())
     ms_per_step = total_ms / K
     value = world * n / (ms_per_step * 1e-3)
+    # kernels launched per step: counted from the library's own dispatch (forward: 1; backward: the 4-row vector body,
+    # plus a scalar tail only when n is not a multiple of 4 or a pointer is not 16-byte aligned -- neither here)
+    launches_per_step = int(lib.pivot_iv_launches_per_forward()) + int(lib.pivot_iv_launches_per_backward()) + (1 if n % 4 else 0)
 
     # --- e2e: the same step through the C-ABI host entry point (pinned host buffers, H2D + D2H inside the timed region)
     e2e = None
@@ -325,7 +440,7 @@ def main():
         hout = (torch.empty(n, dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory(),
                 torch.empty(n, dtype=torch.uint8).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory())
         pipe = pv.Pipeline(chunk_rows=1 << 21, n_slots=4)
-        ke = max(1, min(K, 5))
+        ke = max(1, min(K, 3))
         pipe.forward_backward_host(*host, hgs, VEGA_FLOOR, pv.GATE_MASK, out=hout)
         barrier()
         t0 = time.perf_counter()
@@ -341,61 +456,78 @@ def main():
         e2e = {"value": world * n / dt, "unit": "rows/s", "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 25 * n,
                "ms_per_step": dt * 1e3, "steps": ke, "api": "pivot_iv_forward_backward_host (pinned host buffers)"}
         del host, hgs, hout
-        # label-generation shape of the paper (64 batches x 65,536 options, H2D included): forward only,
-        # one 65,536-row chunk per batch, 4 staging slots (copy engines and SMs overlap across batches)
-        if rank == 0 and world == 1:
-            nl = 64 * 65536
-            lab = wl.config0(nl, seed=9, device="cuda")
-            lh = [lab[k].cpu().pin_memory() for k in KEYS]
-            lo = (torch.empty(nl, dtype=torch.float64).pin_memory(), torch.empty(nl, dtype=torch.float64).pin_memory(),
-                  torch.empty(nl, dtype=torch.uint8).pin_memory())
-            lp = pv.Pipeline(chunk_rows=65536, n_slots=4)
+        # Label generation (64 batches x 65,536 options, H2D included): ONE host array of 4,194,304 config-0 rows,
+        # forward only.  With N ranks each takes its contiguous shard (sharding.shard_rows) through its own pipeline.
+        nl = 64 * 65536
+        lab = wl.config0(nl, seed=9, device="cuda")
+        lb, le = shard_rows(nl, rank, world)
+        lh = [lab[k][lb:le].cpu().pin_memory() for k in KEYS]
+        m_l = le - lb
+        lo = (torch.empty(m_l, dtype=torch.float64).pin_memory(), torch.empty(m_l, dtype=torch.float64).pin_memory(),
+              torch.empty(m_l, dtype=torch.uint8).pin_memory())
+        best = None
+        for chunk, slots in ((65536, 4), (1 << 19, 4)):
+            lp = pv.Pipeline(chunk_rows=chunk, n_slots=slots)
             lp.forward_host(*lh, out=lo)
+            barrier()
             t0 = time.perf_counter()
             for _ in range(5):
                 lp.forward_host(*lh, out=lo)
             dtl = (time.perf_counter() - t0) / 5
             lp.close()
-            e2e["label_pipeline"] = {"labels_per_s": nl / dtl, "ms": dtl * 1e3, "batches": 64, "batch_rows": 65536,
-                                     "h2d_bytes": 40 * nl, "d2h_bytes": 17 * nl,
-                                     "paper_h100_labels_per_s": 48.9e6, "note": "config-0 rows, pinned host buffers"}
-            del lab, lh, lo
+            t = torch.tensor([dtl], device="cuda", dtype=torch.float64)
+            if dist is not None:
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dtl = float(t.item())
+            r_ = {"chunk_rows": chunk, "n_slots": slots, "labels_per_s": nl / dtl, "ms": dtl * 1e3,
+                  "h2d_gb_per_s": 40 * nl / dtl / 1e9}
+            if best is None or r_["labels_per_s"] > best["labels_per_s"]:
+                best = r_
+            e2e.setdefault("label_pipeline_runs", []).append(r_)
+        e2e["label_pipeline"] = dict(best, batches=64, batch_rows=65536, h2d_bytes=40 * nl, d2h_bytes=17 * nl,
+                                     paper_h100_labels_per_s=48.9e6, sharded_over_ranks=world,
+                                     note="config-0 rows, pinned host buffers, one array sharded by shard_rows")
+        del lab, lh, lo
 
     # --- zone mix of this workload (diagnostic kernel variant; not timed)
     zsig, zveg, zst, zone = pv.pivot_iv_forward_zones(*a)
     mix = [int(((zone == z) & (zst == 0)).sum().item()) for z in range(4)] + [int((zst != 0).sum().item())]
-    del zsig, zveg, zone
+    del zsig, zveg, zone, zst
 
     # --- cpu_baseline + parity sample + algorithmic flop count: the oracle, rank 0 at N = 1 only
     cpu = None
     err = {}
     flops_plain = flops_all = None
+    po = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import pyoracle as po
-        m = min(n, 1 << 24)
-        c = {k: cfg[k][:m].cpu().numpy() for k in KEYS}
-        hg = gsig[:m].cpu().numpy()
-        t0 = time.perf_counter()
-        os_, ov, ost = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"])
-        og = po.backward(hg, ov, ost, VEGA_FLOOR, 0)
-        dt = time.perf_counter() - t0
-        cpu = {"value": m / dt, "unit": "rows/s", "cores": po.max_threads(), "kind": "oracle",
-               "sample": f"first {m} rows of the same workload, forward + MASK backward, one pass"}
+        m = min(n, 1 << 23)
+        idx = _sample_idx(n, m)                     # strided over ALL n rows
+        par, (c, _, _) = _parity(po, cfg, out, idx, gP=gP, gsig=gsig, mode=0)
+        err = {"status_mismatches": par["status_mismatches"], "max_rel_err_sigma": par["max_rel_err_sigma"],
+               "max_rel_err_grad_P": par["max_rel_err_grad_P"], "parity_sample_rows": par["rows"],
+               "parity_sample": f"every {n // m}-th row of all {n} rows"}
+        hg = gsig[idx].cpu().numpy()
+
+        def cpu_step():
+            s_, v_, st_ = po.forward(c["SorF"], c["K"], c["tau"], c["P"], c["flag"])
+            po.backward(hg, v_, st_, VEGA_FLOOR, 0)
+        cpu_step()                                   # warm-up: thread pool, first touch
+        ts = []
+        for _ in range(3):
+            t0 = time.perf_counter(); cpu_step(); ts.append(time.perf_counter() - t0)
+        cpu = {"value": m / min(ts), "unit": "rows/s", "cores": po.max_threads(), "kind": "oracle",
+               "sample": f"{m} rows (every {n // m}-th) of the same workload, forward + MASK backward, best of 3 after one warm-up pass",
+               "seconds_per_pass": [round(x, 3) for x in ts]}
         # single-thread figure, to sit beside the paper's 1.60e5 IV/s scalar Python-loop baseline
-        m1 = min(m, 1 << 20)
+        m1 = min(m, 1 << 19)
         t1 = time.perf_counter()
         po.forward(c["SorF"][:m1], c["K"][:m1], c["tau"][:m1], c["P"][:m1], c["flag"][:m1], nthreads=1)
         cpu["single_thread_forward_iv_per_s"] = m1 / (time.perf_counter() - t1)
-        gs_, gv_, gst_ = (t_[:m].cpu().numpy() for t_ in out)
-        ok = (ost == 0) & (gst_ == 0)
-        err["status_mismatches"] = int((ost != gst_).sum())
-        err["max_rel_err_sigma"] = float(np.max(np.abs(gs_[ok] / os_[ok] - 1))) if ok.any() else None
-        on = ok & (ov > VEGA_FLOOR) & (np.abs(ov / VEGA_FLOOR - 1) > 1e-12) & (og != 0)
-        err["max_rel_err_grad_P"] = float(np.max(np.abs(gP[:m].cpu().numpy()[on] / og[on] - 1))) if on.any() else None
-        err["parity_sample_rows"] = m
         mc = min(m, 1 << 18)
         counts, rows = po.count_ops(*[c[k][:mc] for k in KEYS])
         flops_plain, flops_all = _flops_per_row_from_counts(counts, rows)
+        del c, hg
     if flops_all is None:
         tot = float(sum(mix))
         flops_all = sum(f * k for f, k in zip(FALLBACK_FLOPS_PER_CLASS, mix)) / tot
@@ -415,75 +547,86 @@ def main():
     peaks, peak_src = _peaks()
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     fwd_tflops = flops_all * n / (fwd_ms * 1e-3) / 1e12
-    roofline = {"kernel": "forward_kernel_tile<false,false>", "bound": "alu", "achieved": fwd_tflops,
+    exec_tflops = NCU["fwd_issued_fp64_flops_per_row"] * n / (fwd_ms * 1e-3) / 1e12
+    roofline = {"kernel": "forward_kernel_tile<false,false,4,false>", "bound": "alu", "achieved": fwd_tflops,
                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": fwd_tflops / FP64_PEAK_TFLOPS,
-                "traffic": FWD_TRAFFIC_BYTES_PER_ROW * n,
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per row of one ncu --set full capture "
-                                  "(profiles/), scaled to this launch's rows",
+                "what_frac_is": "ALGORITHMIC flops (the oracle's operation count for this workload, 2 Householder steps, "
+                                "library calls at the SASS cost of the CUDA builtins) per second over the derived fp64 peak: a "
+                                "throughput index, not the pipe utilisation -- see `executed`",
+                "executed": {"issued_fp64_flops_per_row": NCU["fwd_issued_fp64_flops_per_row"],
+                             "tflops": exec_tflops, "frac_of_peak": exec_tflops / FP64_PEAK_TFLOPS,
+                             "fp64_pipe_busy_pct": NCU["fwd_fp64_pipe_busy_pct"], "issue_active_pct": NCU["fwd_issue_active_pct"],
+                             "warp_inst_per_row": NCU["fwd_warp_inst_per_row"],
+                             "note": "constants quoted from the ncu --set full capture of the committed kernel", "source": NCU["source"]},
+                "traffic": NCU["fwd_dram_bytes_per_row"] * n,
+                "traffic_source": "constant: dram__bytes_read.sum + dram__bytes_write.sum per row of the ncu --set full capture "
+                                  "named in `executed.source`, scaled to this launch's rows (40.0 B read; part of the 17 B written is "
+                                  "still dirty in L2 when the kernel ends)",
                 "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md s7)",
                 "dfma_probe_tflops": probe_tflops,
                 "flops_per_row": flops_all, "flops_per_row_excl_transcendental_internals": flops_plain,
                 "avg_launch_ms": fwd_ms,
-                "hbm": {"achieved": FWD_BYTES_PER_ROW * n / (fwd_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                        "frac": FWD_BYTES_PER_ROW * n / (fwd_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src}}
+                "hbm": {"achieved": FWD_BYTES["b76"] * n / (fwd_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": FWD_BYTES["b76"] * n / (fwd_ms * 1e-3) / 1e9 / hbm_peak, "peak_source": peak_src}}
     bwd_gbs = BWD_BYTES_PER_ROW * n / (bwd_ms * 1e-3) / 1e9
     roofline_bwd = {"kernel": "backward_kernel_vec4<MASK>", "bound": "hbm", "achieved": bwd_gbs, "peak": hbm_peak,
-                    "unit": "GB/s", "frac": bwd_gbs / hbm_peak, "traffic": None, "avg_launch_ms": bwd_ms,
-                    "peak_source": peak_src}
+                    "unit": "GB/s", "frac": bwd_gbs / hbm_peak, "traffic": NCU["bwd_dram_bytes_per_row"] * n,
+                    "traffic_source": "constant from " + NCU["source"], "avg_launch_ms": bwd_ms, "peak_source": peak_src}
 
-    # --- the "next" rows, timed separately from the step: Black price node and full-VJP backward
+    # --- the "next" rows, timed separately from the step
     next_rows = None
     if rank == 0 and world == 1:
-        def _time(fn, reps=10):
-            for _ in range(3):
-                fn()
-            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            for _ in range(reps):
-                fn()
-            e1.record(stream); torch.cuda.synchronize()
-            return e0.elapsed_time(e1) / reps
         sig_in = torch.where(out[2] == 0, out[0], torch.full_like(out[0], 0.2))
-        ms_p = _time(lambda: pv.pivot_iv_black_price(a[0], a[1], a[2], sig_in, a[4], stream=stream))
-        ms_b = _time(lambda: pv.pivot_iv_backward_inputs(a[0], a[1], a[2], a[4], out[0], out[1], out[2], gsig, VEGA_FLOOR,
-                                                         pv.GATE_MASK, stream=stream))
+        ms_p = _time_calls(lambda: pv.pivot_iv_black_price(a[0], a[1], a[2], sig_in, a[4], stream=stream), stream, 5)
+        ms_b = _time_calls(lambda: pv.pivot_iv_backward_inputs(a[0], a[1], a[2], a[4], out[0], out[1], out[2], gsig, VEGA_FLOOR,
+                                                               pv.GATE_MASK, stream=stream), stream, 5)
+        ms_lp = _time_calls(lambda: pv.pivot_iv_loss_price(a[0], a[1], a[2], a[3], a[4], sig_in, grad_scale=1.0, stream=stream),
+                            stream, 5)
+        ms_lr = _time_calls(lambda: pv.pivot_iv_loss_roundtrip(a[0], a[1], a[2], a[3], a[4], sig_in, sig_in, 1e-6, grad_scale=1.0,
+                                                               stream=stream), stream, 3)
         on_frac = float(((out[2] == 0) & (out[1] > VEGA_FLOOR)).double().mean().item())
         bp, bb = 56.0, 17.0 + 32.0 + 40.0 * on_frac   # algorithmic bytes/row (Black-76): see DESIGN.md section 11
         next_rows = {"black_price": {"ms": ms_p, "rows_per_s": n / (ms_p * 1e-3), "bytes_per_row": bp,
                                      "hbm_frac": bp * n / (ms_p * 1e-3) / 1e9 / hbm_peak},
                      "backward_inputs": {"ms": ms_b, "rows_per_s": n / (ms_b * 1e-3), "bytes_per_row": bb,
                                          "gate_on_fraction": on_frac,
-                                         "hbm_frac": bb * n / (ms_b * 1e-3) / 1e9 / hbm_peak}}
+                                         "hbm_frac": bb * n / (ms_b * 1e-3) / 1e9 / hbm_peak},
+                     "loss_price_with_grad": {"ms": ms_lp, "rows_per_s": n / (ms_lp * 1e-3), "bytes_per_row": 56.0,
+                                              "hbm_frac": 56.0 * n / (ms_lp * 1e-3) / 1e9 / hbm_peak},
+                     "loss_roundtrip_with_grad": {"ms": ms_lr, "rows_per_s": n / (ms_lr * 1e-3), "bytes_per_row": 64.0,
+                                                  "hbm_frac": 64.0 * n / (ms_lr * 1e-3) / 1e9 / hbm_peak,
+                                                  "note": "one fused kernel: price node + LBR inversion + weighted residual + gradient"}}
         del sig_in
 
     sweep = configs = None
-    if (args.sweep or args.configs) and rank == 0 and world == 1:
+    if rank == 0 and world == 1:
         del cfg, a, out, gP, gsig
         torch.cuda.empty_cache()
-        if args.sweep:
-            sweep = run_sweep(pv, wl, hbm_peak, flops_all)
-        if args.configs:
-            configs = run_configs(pv, wl)
+        if not args.no_sweep:
+            sweep = run_sweep(pv, wl, hbm_peak, flops_all, 24 if args.quick else 28)
+            torch.cuda.empty_cache()
+        if not args.no_configs and po is not None:
+            configs = run_configs(pv, wl, po, hbm_peak, args.quick)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": "rows/s", "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic",
+                "dtype": DTYPE, "data": "synthetic",
                 "config": {"workload": "config 4 @ n=2^26 rows/GPU (inputs as config 1: x~U[-5,5], s log-U[1e-4,5], "
                                        "call/put 50/50, Black-76 D=1); step = fused forward + MASK backward (floor 1e-8)",
                            "rows_per_gpu": n, "l2": "inputs+outputs 5.5 GB per step >> 126 MB L2, no flush needed",
+                           "global_rows": world * n, "rank0_shard": [g_begin, g_end],
                            "zone_mix_rows[z0,z1,z2,z3,non_ok]": mix},
                 "fwd_iv_per_s": world * n / (fwd_ms * 1e-3), "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
                 "bwd_rows_per_s": world * n / (bwd_ms * 1e-3),
                 "solved_rows_per_s_fwd": world * sum(mix[:4]) / (fwd_ms * 1e-3),
-                "clocks": clocks, "e2e": e2e, "gpu_launches": K * (pv.load_library().pivot_iv_launches_per_forward() + pv.load_library().pivot_iv_launches_per_backward()),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": K * launches_per_step,
                 "roofline": roofline, "roofline_backward": roofline_bwd, "cpu_baseline": cpu}
         line.update(err)
         if sweep is not None:
             line["sweep"] = sweep
         if configs is not None:
             line["configs"] = configs
-            line["forward_kernel_variant"] = os.environ.get("PIVOT_IV_FWD_KERNEL", "tile")
         if next_rows is not None:
             line["next_rows"] = next_rows
         line["paper_context"] = {"h100_triton_fused_iv_per_s": 1.79e9, "h100_max_rel_err": 9.3e-14,

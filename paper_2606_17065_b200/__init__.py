@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     FWD_FP64_ONLY,
     PivotError,
     Pipeline,
+    ShardedPipeline,
     library_path,
     load_library,
     pivot_iv_black_price,
@@ -37,7 +38,7 @@ from .binding import (  # noqa: F401
 __all__ = [
     "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_backward_inputs", "pivot_iv_black_price",
     "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
-    "Pipeline", "pivot_iv_probe_dfma",
+    "Pipeline", "ShardedPipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
     "GATE_ATTENUATE", "GATE_STRICT", "RT_GATED", "RT_NAIVE", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "pivot_iv_debug_math", "EXPORTS",
 ]

@@ -128,9 +128,11 @@ def _forward(SorF, K, tau, P, flag, r, q, out, stream, zones, kernel=None):
     _require_cuda()
     lib = load_library()
     n = SorF.numel()
-    for nm, t in (("K", K), ("tau", tau), ("P", P), ("flag", flag), ("r", r), ("q", q)):
-        if t is not None and t.numel() != n:
-            raise PivotError(f"{nm}: length {t.numel()} != {n}")
+    _same_len(n, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
+    _same_device(SorF, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
+    if out is not None:
+        _same_len(n, **{f"out[{i}]": t for i, t in enumerate(out)})
+        _same_device(SorF, **{f"out[{i}]": t for i, t in enumerate(out)})
     inp = _Inputs(_dev(SorF, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P, "P"),
                   _dev(flag, "flag"))
     if out is None:
@@ -214,8 +216,8 @@ def pivot_iv_backward(grad_sigma, vega, status, vega_floor: float, mode: int, ou
     _require_cuda()
     lib = load_library()
     n = grad_sigma.numel()
-    if vega.numel() != n or status.numel() != n:
-        raise PivotError("grad_sigma, vega, status must have the same length")
+    _same_len(n, vega=vega, status=status, out=out)
+    _same_device(grad_sigma, vega=vega, status=status, out=out)
     gP = torch.empty_like(grad_sigma) if out is None else out
     with torch.cuda.device(grad_sigma.device):
         _check(lib.pivot_iv_backward(_dev(grad_sigma, "grad_sigma"), _dev(vega, "vega"),
@@ -229,6 +231,8 @@ def pivot_iv_black_price(S_or_F, K, tau, sigma, flag, r=None, q=None, with_vega=
     _require_cuda()
     lib = load_library()
     n = S_or_F.numel()
+    _same_len(n, K=K, tau=tau, sigma=sigma, flag=flag, r=r, q=q)
+    _same_device(S_or_F, K=K, tau=tau, sigma=sigma, flag=flag, r=r, q=q)
     inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), None,
                   _dev(flag, "flag"))
     price = torch.empty(n, dtype=torch.float64, device=S_or_F.device)
@@ -246,6 +250,8 @@ def pivot_iv_backward_inputs(S_or_F, K, tau, flag, sigma, vega, status, grad_sig
     _require_cuda()
     lib = load_library()
     n = S_or_F.numel()
+    _same_len(n, K=K, tau=tau, flag=flag, sigma=sigma, vega=vega, status=status, grad_sigma=grad_sigma, r=r, q=q)
+    _same_device(S_or_F, K=K, tau=tau, flag=flag, sigma=sigma, vega=vega, status=status, grad_sigma=grad_sigma, r=r, q=q)
     inp = _Inputs(_dev(S_or_F, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), None,
                   _dev(flag, "flag"))
     outs = [torch.empty(n, dtype=torch.float64, device=S_or_F.device) for _ in range(4)]
@@ -340,6 +346,9 @@ class Pipeline:
 
     def forward_host(self, S_or_F, K, tau, P, flag, r=None, q=None, out=None):
         n = S_or_F.numel()
+        _same_len(n, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
+        if out is not None:
+            _same_len(n, **{f"out[{i}]": t for i, t in enumerate(out)})
         if out is None:
             out = (torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.float64),
                    torch.empty(n, dtype=torch.uint8))
@@ -352,6 +361,9 @@ class Pipeline:
 
     def forward_backward_host(self, S_or_F, K, tau, P, flag, grad_sigma, vega_floor, mode, r=None, q=None, out=None):
         n = S_or_F.numel()
+        _same_len(n, K=K, tau=tau, P=P, flag=flag, grad_sigma=grad_sigma, r=r, q=q)
+        if out is not None:
+            _same_len(n, **{f"out[{i}]": t for i, t in enumerate(out)})
         if out is None:
             out = (torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.float64),
                    torch.empty(n, dtype=torch.uint8), torch.empty(n, dtype=torch.float64))
@@ -363,3 +375,51 @@ class Pipeline:
                                                         _host(vega, "vega"), _host(status, "status", torch.uint8),
                                                         _host(gP, "grad_P")))
         return sigma, vega, status, gP
+
+
+class ShardedPipeline:
+    """Row-sharded label generation over several GPUs from ONE process: one
+    pivot_iv_pipeline per device, each fed a contiguous shard (sharding.shard_rows) of the same host arrays by its own
+    host thread (the C call releases the GIL).  Rows are independent: no collective, results land in the caller's arrays.
+    With one process per GPU (torchrun) each rank simply runs a Pipeline on shard_rows(n, rank, world) instead."""
+
+    def __init__(self, devices, chunk_rows: int = 1 << 19, n_slots: int = 4):
+        from .sharding import shard_rows
+        self._shard_rows = shard_rows
+        self.devices = list(devices)
+        if not self.devices:
+            raise PivotError("ShardedPipeline needs at least one device")
+        self.pipes = [Pipeline(chunk_rows=chunk_rows, n_slots=n_slots, device=int(d)) for d in self.devices]
+
+    def close(self):
+        for p in self.pipes:
+            p.close()
+
+    def shards(self, n: int):
+        return [self._shard_rows(n, k, len(self.pipes)) for k in range(len(self.pipes))]
+
+    def forward_host(self, S_or_F, K, tau, P, flag, r=None, q=None, out=None):
+        import threading
+        n = S_or_F.numel()
+        _same_len(n, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
+        if out is None:
+            out = (torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.float64),
+                   torch.empty(n, dtype=torch.uint8))
+        _same_len(n, **{f"out[{i}]": t for i, t in enumerate(out)})
+        errs = []
+
+        def work(k, b, e):
+            try:
+                sl = lambda t: None if t is None else t[b:e]
+                self.pipes[k].forward_host(sl(S_or_F), sl(K), sl(tau), sl(P), sl(flag), r=sl(r), q=sl(q),
+                                           out=tuple(t[b:e] for t in out))
+            except Exception as ex:   # surfaced to the caller below
+                errs.append(ex)
+        threads = [threading.Thread(target=work, args=(k, b, e)) for k, (b, e) in enumerate(self.shards(n)) if e > b]
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        if errs:
+            raise errs[0]
+        return out

@@ -15,16 +15,22 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
          "-shared", "-cudart", "shared"]
 
 
-def needs_build() -> bool:
-    return not os.path.exists(SO) or any(os.path.getmtime(SO) < os.path.getmtime(d) for d in DEPS)
+SO_CHECKED = os.path.join(HERE, "libpivot_iv_boundscheck.so")
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
-        return SO
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SRC
+def needs_build(so: str = SO) -> bool:
+    return not os.path.exists(so) or any(os.path.getmtime(so) < os.path.getmtime(d) for d in DEPS)
+
+
+def build(force: bool = False, verbose: bool = False, bounds_check: bool = False) -> str:
+    """bounds_check=True builds libpivot_iv_boundscheck.so: the same sources with -DPIVOT_BOUNDS_CHECK (device-side asserts on
+    every shared-memory index of the tile kernel), loaded only by tests/test_gpu_boundscheck.py."""
+    so = SO_CHECKED if bounds_check else SO
+    if not force and not needs_build(so):
+        return so
+    cmd = [NVCC] + FLAGS + (["-DPIVOT_BOUNDS_CHECK"] if bounds_check else []) + (["-Xptxas", "-v"] if verbose else []) + ["-o", so] + SRC
     subprocess.check_call(cmd)
-    return SO
+    return so
 
 
 if __name__ == "__main__":

@@ -16,6 +16,16 @@
 #include "../../include/pivot_iv.h"
 #include "lbr_device.cuh"
 
+// -DPIVOT_BOUNDS_CHECK (build.py build(bounds_check=True) -> libpivot_iv_boundscheck.so): every shared-memory index of the
+// tile kernel is asserted in range on the device (compute-sanitizer is not available on this pool; tests/test_gpu_boundscheck.py
+// runs the ragged / edge / BSM cases through this build).  Compiled out of the product library.
+#ifdef PIVOT_BOUNDS_CHECK
+#include <cassert>
+#define PIVOT_ASSERT(c) assert(c)
+#else
+#define PIVOT_ASSERT(c) ((void)0)
+#endif
+
 namespace pivot {
 
 constexpr int kFwdThreads = 128;
@@ -103,6 +113,7 @@ __device__ __noinline__ void tile_rare_row(pivot_iv_inputs in, int64_t base, int
   sm.veg[p] = queued ? pr.D : 0.0;
   if (queued) {
     const int slot = atomicAdd(&sm.count, 1);
+    PIVOT_ASSERT(slot >= 0 && slot < TileSmem<RPT>::kTileRows && p >= 0 && p < TileSmem<RPT>::kTileRows);
     sm.q0[slot] = pr.U;
     sm.q1[slot] = pr.O;
     sm.q2[slot] = pr.B;
@@ -192,6 +203,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     for (int k = 0; k < RPT; ++k) {
       if ((qmask >> k) & 1u) {
         const int j = slot + __popc(bal[k] & lt);
+        PIVOT_ASSERT(j >= 0 && j < kTileRows);
         sm.q0[j] = vF[k];
         sm.q1[j] = vK[k];
         sm.q2[j] = vP[k];
@@ -219,6 +231,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       const SeedHead hd = lbr_seed_head<FULL>(nm.qrel, nm.beta, nm.bbar, nm.bmax);
       sm.q0[j] = hd.v0; sm.q1[j] = hd.v1; sm.q2[j] = hd.v2; sm.q3[j] = hd.v3;
       const int p = pj & 0x3fff;
+      PIVOT_ASSERT(p < rows);
       sm.veg[p] = BSM ? sm.veg[p] * nm.rootFK : nm.rootFK;    // D sqrt(FK)
       cls = (hd.zone == 0) ? 0 : ((hd.zone == 3) ? 2 : 1);
       if (DIAG && dg.zone) dg.zone[base + p] = (int8_t)hd.zone;
@@ -236,6 +249,9 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     base2 = __shfl_sync(0xffffffffu, base2, 0);
     const int b0 = (int)(base01 & 0xffffu), b1 = (int)(base01 >> 16), b2 = (int)base2;
     const unsigned lt = (1u << lane) - 1u;
+    PIVOT_ASSERT(cls != 0 || (b0 + __popc(m0 & lt) >= 0 && b0 + __popc(m0 & lt) < kTileRows));
+    PIVOT_ASSERT(cls != 1 || (kTileRows - 1 - (b1 + __popc(m1 & lt)) >= 0 && b0 + b1 + __popc(m1 & lt) < kTileRows));
+    PIVOT_ASSERT(cls != 2 || (b2 + __popc(m2 & lt) >= 0 && b2 + __popc(m2 & lt) < kTileRows));
     if (cls == 0) sm.perm[b0 + __popc(m0 & lt)] = (uint16_t)j;
     else if (cls == 1) sm.perm[kTileRows - 1 - (b1 + __popc(m1 & lt))] = (uint16_t)j;
     else if (cls == 2) sm.permU[b2 + __popc(m2 & lt)] = (uint16_t)j;
@@ -261,8 +277,10 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       const Seed sd = lbr_seed_tail3<FULL>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
       x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = sd.kind;
     }
+    PIVOT_ASSERT(j >= 0 && j < cnt && cnt <= rows && n0 + n1 + (int)sm.n2 == cnt);
     const NormSolve ns = lbr_refine<kHouseholderSteps, FULL>(x, s0, p1, p2, kind);
     const int p = sm.pos[j] & 0x3fff;
+    PIVOT_ASSERT(p < rows);
     const double tau = sm.sig[p];
     const double rinv = rsqrt(tau);
     sm.sig[p] = ns.s * rinv;
@@ -309,11 +327,17 @@ __device__ __forceinline__ double backward_row(double gs, double V, uint8_t st, 
 }
 
 // 4 rows per thread per iteration (two 16-byte loads per fp64 array, one 4-byte status load), grid-stride.
-// grad_P may alias grad_sigma (include/pivot_iv.h): neither pointer is __restrict__, and a thread loads its rows before it stores them.
-template <int MODE>
+// grad_P may alias grad_sigma (include/pivot_iv.h).  INPLACE = false (distinct buffers): both pointers are __restrict__, so
+// the loads of the next iteration may be hoisted over the stores of this one.  INPLACE = true (grad_P == grad_sigma):
+// neither is, and a thread loads its rows before it stores them.
+template <int MODE, bool INPLACE>
 __global__ void __launch_bounds__(kBwdThreads)
-backward_kernel_vec4(const double* gs, const double* __restrict__ vega, const uint8_t* __restrict__ status,
-                     double floor_, int64_t n4, double* gP) {
+backward_kernel_vec4(const double* gs_, const double* __restrict__ vega, const uint8_t* __restrict__ status,
+                     double floor_, int64_t n4, double* gP_) {
+  typedef const double* __restrict__ RIn;
+  typedef double* __restrict__ ROut;
+  const double* gs = INPLACE ? gs_ : static_cast<RIn>(gs_);
+  double* gP = INPLACE ? gP_ : static_cast<ROut>(gP_);
   const double floor2 = __dmul_rn(floor_, floor_);
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < n4; j += stride) {
@@ -464,7 +488,9 @@ int launch_backward_t(const double* gs, const double* vega, const uint8_t* statu
     int64_t blocks = (n4 + kBwdThreads - 1) / kBwdThreads;
     const int64_t cap = (int64_t)sm_count() * 8 * 4;  // 8 resident CTAs of 256 threads per SM, 4 waves' worth
     if (blocks > cap) blocks = cap;
-    backward_kernel_vec4<MODE><<<(unsigned)blocks, kBwdThreads, 0, st>>>(gs, vega, status, floor_, n4, gP);
+    // overlapping but unequal ranges are the caller's error (the header allows grad_P == grad_sigma only)
+    if (gs == gP) backward_kernel_vec4<MODE, true><<<(unsigned)blocks, kBwdThreads, 0, st>>>(gs, vega, status, floor_, n4, gP);
+    else backward_kernel_vec4<MODE, false><<<(unsigned)blocks, kBwdThreads, 0, st>>>(gs, vega, status, floor_, n4, gP);
     done = 4 * n4;
   }
   if (done < n) {

@@ -211,6 +211,38 @@ def test_host_pipeline_matches_device_path():
     pipe.close()
 
 
+def test_host_pipeline_matches_oracle():
+    """The host entry points against the ORACLE (not against the device path): pivot_iv_forward_backward_host on config 3 in
+    chunks with a ragged last one, and the row-sharded multi-device driver (two pipelines; both on cuda:0 when the box has
+    one GPU -- the shard bookkeeping is what is under test) on BSM chains."""
+    cfg = wl.config3(200_003, seed=19)
+    c = to_numpy(cfg)
+    pipe = pv.Pipeline(chunk_rows=65_536, n_slots=4)
+    s, v, st, gP = pipe.forward_backward_host(*[cfg[k] for k in KEYS], cfg["grad_sigma"], 1e-8, 0)
+    pipe.close()
+    o = oracle_forward(c)
+    compare_forward((s.numpy(), v.numpy(), st.numpy()), o, c)
+    compare_backward(gP.numpy(), c["grad_sigma"], v.numpy(), st.numpy(), o[1], 1e-8, 0)
+    c2 = wl.config2(days=3, expiries=7, strikes=399)
+    ndev = torch.cuda.device_count()
+    sp = pv.ShardedPipeline(devices=[0, 1 % ndev], chunk_rows=10_000, n_slots=2)
+    n2 = c2["K"].numel()
+    sh = sp.shards(n2)
+    assert sh[0][0] == 0 and sh[0][1] == sh[1][0] and sh[1][1] == n2 and sh[1][0] % 2 == 0
+    out = sp.forward_host(*[c2[k] for k in KEYS], r=c2["r"], q=c2["q"])
+    sp.close()
+    h2 = to_numpy(c2)
+    compare_forward(tuple(t.numpy() for t in out), oracle_forward(h2), h2)
+    with pytest.raises(pv.PivotError):                       # a short tensor is refused before the library is called
+        pv.Pipeline(chunk_rows=1000, n_slots=1).forward_host(cfg["SorF"], cfg["K"][:-1], cfg["tau"], cfg["P"], cfg["flag"])
+    d = to_device(cfg)
+    with pytest.raises(pv.PivotError):
+        pv.pivot_iv_forward(d["SorF"], d["K"], d["tau"], d["P"], d["flag"],
+                            out=(torch.empty(10, dtype=torch.float64, device="cuda"),) * 2 + (torch.empty(10, dtype=torch.uint8, device="cuda"),))
+    with pytest.raises(pv.PivotError):
+        pv.pivot_iv_backward(d["grad_sigma"], d["SorF"][:-1], torch.zeros(200_003, dtype=torch.uint8, device="cuda"), 1e-8, 0)
+
+
 def test_streams_and_preallocated_outputs():
     cfg = wl.config0(10_000)
     d = to_device(cfg)

@@ -53,3 +53,20 @@ def test_shard_rows_properties():
                 prev = e
                 cover += e - b
             assert prev == n and cover == n
+
+
+def test_bench_spawns_its_own_ranks():
+    """`python bench.py --gpus 2` without a launcher must start two ranks itself (torch.distributed.run): the CPU self-test
+    mode runs the same launcher and shard bookkeeping over gloo and reports what every rank took of ONE array."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    n = 1_000_003
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--selftest-launch", "--rows", str(n)],
+                       env=env, capture_output=True, text=True, timeout=300)
+    assert p.returncode == 0, p.stderr[-2000:]
+    line = [ln for ln in p.stdout.splitlines() if ln.startswith("{")][-1]
+    r = json.loads(line)
+    assert r["n_gpus"] == 2 and r["max_ms"] == 2.0            # two ranks really ran (max over ranks of 1 + rank)
+    assert r["shards"][0][0] == 0 and r["shards"][0][1] == r["shards"][1][0] and r["shards"][1][1] == n
+    assert r["shards"][1][0] % 2 == 0
