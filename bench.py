@@ -46,12 +46,12 @@ BWD_BYTES_PER_ROW = 25
 # Constants QUOTED from the ncu --set full captures of the committed kernels (profiles/r2*_ncu_full.md; config 4 mixed rows):
 NCU = {
     "source": "profiles/r2c_forward_tile_ncu_full.md, profiles/r2c_backward_ncu_full.md (ncu --set full of this kernel, config 4)",
-    "fwd_dram_bytes_per_row": 54.7,          # dram__bytes_read.sum + dram__bytes_write.sum per row (40.0 read + 14.7 written)
-    "fwd_issued_fp64_flops_per_row": 229.0,  # 2 DFMA + DADD + DMUL thread instructions per row
-    "fwd_fp64_pipe_busy_pct": 43.7,
-    "fwd_issue_active_pct": 68.0,
-    "fwd_warp_inst_per_row": 20.9,
-    "bwd_dram_bytes_per_row": 25.0,
+    "fwd_dram_bytes_per_row": 56.5,          # dram__bytes_read.sum + dram__bytes_write.sum per row (40.0 read + 16.5 written)
+    "fwd_issued_fp64_flops_per_row": 229.7,  # 2 DFMA + DADD + DMUL thread instructions per row
+    "fwd_fp64_pipe_busy_pct": 44.3,
+    "fwd_issue_active_pct": 69.8,
+    "fwd_warp_inst_per_row": 20.96,
+    "bwd_dram_bytes_per_row": 24.5,          # 17.0 read + 7.5 written
 }
 # per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
 # CUDA 12.9 builtins); "/" and sqrt count 1 flop each
@@ -560,8 +560,8 @@ def main():
                              "note": "constants quoted from the ncu --set full capture of the committed kernel", "source": NCU["source"]},
                 "traffic": NCU["fwd_dram_bytes_per_row"] * n,
                 "traffic_source": "constant: dram__bytes_read.sum + dram__bytes_write.sum per row of the ncu --set full capture "
-                                  "named in `executed.source`, scaled to this launch's rows (40.0 B read; part of the 17 B written is "
-                                  "still dirty in L2 when the kernel ends)",
+                                  "named in `executed.source`, scaled to this launch's rows (40.0 B read + 16.5 B written per row; part of "
+                                  "the 17 B written is still dirty in L2 when the kernel ends)",
                 "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md s7)",
                 "dfma_probe_tflops": probe_tflops,
                 "flops_per_row": flops_all, "flops_per_row_excl_transcendental_internals": flops_plain,
