@@ -78,6 +78,9 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma,
 // Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); both partitions cost shared-memory traffic only.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kTileThreads = 256;
+#ifndef PIVOT_PREFETCH_DIST
+#define PIVOT_PREFETCH_DIST 592
+#endif
 // RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers, both modes) for large n;
 // 1 (256-row tiles) for small n, so that a launch of 65,536 rows still spreads over every SM.
 
@@ -137,6 +140,24 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
   const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
   if (tid == 0) { sm.count = 0; sm.n01 = 0u; sm.n2 = 0u; }
+  {
+    // L2 prefetch for the CTA that will run about one residency later on this SM slot (blockIdx.x + kPrefetchDist): its phase A
+    // then finds its 40 (56) KB of inputs in L2 instead of waiting for HBM while nothing else of that CTA can run
+    const int64_t pbase = base + (int64_t)PIVOT_PREFETCH_DIST * kTileRows;
+    constexpr int kLines = kTileRows * 8 / 128;   // 128-byte lines per input array of a tile
+    if (tid < kLines && pbase + kTileRows <= n) {
+      const int64_t o = pbase + (int64_t)tid * 16;
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(in.S_or_F + o));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(in.K + o));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(in.tau + o));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(in.P + o));
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(in.flag + o));
+      if (BSM) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(in.r + o));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(in.q + o));
+      }
+    }
+  }
   __syncthreads();
 
   // ---- phase A: all rows of the tile; every load of the thread's rows is issued before the first use
