@@ -217,9 +217,9 @@ int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivo
 /* Test-only: evaluates ONE function of the device math library elementwise, out[i] = fn(a[i] [, b[i]]), so that its error
  * can be measured on the device against a multiprecision reference (tests/test_gpu_mathlib.py; DESIGN.md section 5 lists
  * the measured bounds).  a, b, out: device, n doubles; b is read only by the two-argument functions (erfcx pair: the pair
- * is erfcx(a), erfcx(b); div_fast: a / b).  fp32-grade functions take and return doubles (converted inside).
+ * is erfcx(a), erfcx(b); div_fast: a / b; erfcx_dd: z1 = a, gap b; W: x = a, s = b).  fp32-grade functions take and return doubles (converted inside).
  * Returns PIVOT_ERR_BAD_ARG for an unknown fn, PIVOT_ERR_NULL / _BAD_N / _CUDA as usual. */
-#define PIVOT_DBG_ERFCX_ONE 0      /* erfcx(a), a >= 0, fp64 (degree-22 form) */
+#define PIVOT_DBG_ERFCX_ONE 0      /* erfcx(a), a >= -0.0708, fp64 (degree-24 form) */
 #define PIVOT_DBG_ERFCX_PAIR_1 1   /* first of erfcx_pair(a, b) */
 #define PIVOT_DBG_ERFCX_PAIR_2 2   /* second of erfcx_pair(a, b) */
 #define PIVOT_DBG_ERFCX_SEED 3     /* erfcx(a), fp32 seed grade */
@@ -238,7 +238,13 @@ int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivo
 #define PIVOT_DBG_NINV_TAIL_FULL 16 /* ... refined by two Newton steps at fp64 */
 #define PIVOT_DBG_EXPF_SEED 17     /* exp(a) in fp32 (MUFU.EX2), |a| <= 87 */
 #define PIVOT_DBG_LOGF_SEED 18     /* ln(a) in fp32 (MUFU.LG2) */
-#define PIVOT_DBG_COUNT 19
+#define PIVOT_DBG_ERFCX_DD_DIFF 19 /* erfcx(a) - erfcx(a + b), a >= -0.0708, b >= 0: divided-difference form, fp64 */
+#define PIVOT_DBG_ERFCX_DD_SUM 20  /* erfcx(a) + erfcx(a + b), same evaluation */
+#define PIVOT_DBG_ERFCX_DD_SEED_DIFF 21 /* ... fp32 seed grade */
+#define PIVOT_DBG_ERFCX_DD_SEED_SUM 22
+#define PIVOT_DBG_W_FULL 23        /* eval_W at x = a <= 0, s = b > 0: W = b/b' if the difference form was taken, else -Wbar */
+#define PIVOT_DBG_W_SEED 24        /* ... at seed grade */
+#define PIVOT_DBG_COUNT 25
 int pivot_iv_debug_math(int fn, const double* a, const double* b, int64_t n, double* out, pivot_iv_stream stream);
 
 /* Number of kernels a call launches (for bench.py's `gpu_launches` bookkeeping). */

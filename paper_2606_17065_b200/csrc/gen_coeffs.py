@@ -4,10 +4,13 @@ Build-step script (run by hand when an approximation changes; the generated head
 the library needs only nvcc).  Everything is derived here from mpmath at 40 digits -- no published coefficient table
 is used, and nothing is shared with oracle/ (which uses libm in long double).
 
-  erfcx(z), z >= 0 (fp64):  y = (z - C)/(z + C),  erfcx(z) = (1 - y) Q(y),  Q = degree-N polynomial in y on [-1,1]
-                            (Chebyshev interpolant converted to the monomial basis; (1-y) = 2C/(z+C) keeps the
-                            1/z decay exact, so Q is smooth up to y = 1 <=> z = infinity)
-  erfcx(z), z >= 0 (fp32):  same form, lower degree, for the seed (needs ~1e-6)
+  erfcx(z), z >= ZMIN (fp64):  y = (z - C)/(z + C),  erfcx(z) = (1 - y) Q(y),  Q = degree-N polynomial in y on
+                            [y(ZMIN), 1] (Chebyshev interpolant converted to the monomial basis; (1-y) = 2C/(z+C) keeps the
+                            1/z decay exact, so Q is smooth up to y = 1 <=> z = infinity).  ZMIN = -0.0708 is slightly
+                            negative and the degree is chosen for the DERIVATIVE of Q as well: the solver forms
+                            erfcx(z1) - erfcx(z2) from the divided difference Q[y1, y2] (lbr_device.cuh, erfcx_dd), whose
+                            error is that of Q' (Markov: up to N^2 times the error of Q near the ends of the interval)
+  erfcx(z), z >= ZMIN (fp32):  same form, lower degree, for the seed (needs ~1e-6)
   Phi^-1 tail (fp32):       for p <= 1/2 with u = sqrt(-2 ln p):  -Phi^-1(p) = u - R(u), R = polynomial in w = 1/(1+u)
                             ... fitted by least squares on Chebyshev nodes (seed accuracy ~1e-5 relative)
 Prints the achieved accuracies; writes the header next to this file.
@@ -55,13 +58,43 @@ def cheb_to_monomial(c):
     return a
 
 
-def fit_erfcx(C, N):
-    def Q(y):
-        if y >= 1:
-            return 1 / (2 * C * mp.sqrt(mp.pi))
-        z = C * (1 + y) / (1 - y)
-        return erfcx(z) * (z + C) / (2 * C)
-    return cheb_to_monomial(cheb_coeffs(Q, N))
+ZMIN = -0.0708   # z1 = (|h| - t)/sqrt2 >= -0.1/sqrt2 wherever the difference form is used (lbr_device.cuh, eval_W)
+
+
+def erfcx_Q(y, C):
+    if y >= 1:
+        return 1 / (2 * C * mp.sqrt(mp.pi))
+    z = C * (1 + y) / (1 - y)
+    return erfcx(z) * (z + C) / (2 * C)
+
+
+def fit_erfcx(C, N, zmin=ZMIN):
+    """Q on y in [ymin, 1], ymin = y(zmin): Chebyshev interpolant in u = (y - mid)/half, converted to monomials in y."""
+    import math
+    ymin = (mp.mpf(zmin) - C) / (mp.mpf(zmin) + C)
+    half, mid = (1 - ymin) / 2, (1 + ymin) / 2
+    au = cheb_to_monomial(cheb_coeffs(lambda u: erfcx_Q(mid + half * u, C), N))
+    out = [mp.mpf(0)] * (N + 1)
+    for k, ck in enumerate(au):
+        for j in range(k + 1):
+            out[j] += ck * math.comb(k, j) * (1 / half) ** k * (-mid) ** (k - j)
+    return out
+
+
+def check_bracket(a, C, zmin=ZMIN):
+    """max relative truncation error of Q(y) - (1 - y) Q'(y) (= -erfcx'(z) (z + C)^2 / 2C: what the divided-difference form
+    of erfcx(z1) - erfcx(z2) multiplies) over z >= zmin, in mpmath (no rounding)."""
+    N = len(a) - 1
+    y0 = float((mp.mpf(zmin) - C) / (mp.mpf(zmin) + C))
+    worst = 0.0
+    for y in np.concatenate([np.linspace(y0, -0.9, 60), np.linspace(-0.9, 0.9995, 120)]):
+        ym = mp.mpf(float(y))
+        q = sum(a[k] * ym ** k for k in range(N + 1))
+        dq = sum(k * a[k] * ym ** (k - 1) for k in range(1, N + 1))
+        qt = erfcx_Q(ym, C)
+        dqt = mp.diff(lambda t: erfcx_Q(t, C), ym)
+        worst = max(worst, abs(float((q - (1 - ym) * dq) / (qt - (1 - ym) * dqt) - 1)))
+    return worst
 
 
 def horner(a, y, dtype):
@@ -72,7 +105,7 @@ def horner(a, y, dtype):
 
 
 def check_erfcx(a, C, dtype):
-    zs = np.concatenate([np.linspace(0, 1, 301), np.linspace(1, 12, 1101), np.linspace(12, 60, 200), [1e3, 1e6]])
+    zs = np.concatenate([np.linspace(ZMIN, 0, 30), np.linspace(0, 1, 301), np.linspace(1, 12, 1101), np.linspace(12, 60, 200), [1e3, 1e6]])
     worst = 0.0
     af = [dtype(float(v)) for v in a]
     for z in zs:
@@ -158,15 +191,17 @@ def fmt(vals, per_line=3, f32=False):
 
 
 def main():
-    C64, N64 = 4.0, 22
+    C64, N64 = 4.0, 24
     a64 = fit_erfcx(C64, N64)
     e64 = check_erfcx(a64, C64, np.float64)
+    b64 = check_bracket(a64, C64)
     C32, N32 = 2.0, 10
     a32 = fit_erfcx(C32, N32)
     e32 = check_erfcx(a32, C32, np.float32)
+    b32 = check_bracket(a32, C32)
     ninv, en = fit_ninv_tail(7)
-    print(f"erfcx fp64: C={C64} N={N64} max rel err (fp64 Horner, no FMA) = {e64:.3e}")
-    print(f"erfcx fp32: C={C32} N={N32} max rel err (fp32 Horner) = {e32:.3e}")
+    print(f"erfcx fp64: C={C64} N={N64} z >= {ZMIN}: max rel err (fp64 Horner, no FMA) = {e64:.3e}; Q - (1-y)Q' truncation = {b64:.3e}")
+    print(f"erfcx fp32: C={C32} N={N32} z >= {ZMIN}: max rel err (fp32 Horner) = {e32:.3e}; Q - (1-y)Q' truncation = {b32:.3e}")
     print(f"ninv tail : deg 7 in w=1/(1+u), max rel err = {en:.3e}")
     NEXP, NATH = 11, 8
     aexp, eexp = fit_exp(NEXP)
@@ -176,8 +211,9 @@ def main():
     print(f"atanh     : f(1 + w G(w)), G degree {NATH}, |f| <= {float(FMAX):.4f}, max rel err = {eath:.3e}")
     with open(os.path.join(HERE, "coeffs.cuh"), "w") as f:
         f.write("// coeffs.cuh -- GENERATED by gen_coeffs.py (mpmath, 40 digits); do not edit by hand.\n")
-        f.write(f"// erfcx fp64: erfcx(z) = (2C/(z+C)) Q((z-C)/(z+C)), C = {C64}, degree {N64}, max rel err {e64:.2e}\n")
-        f.write(f"// erfcx fp32: same form, C = {C32}, degree {N32}, max rel err {e32:.2e}\n")
+        f.write(f"// erfcx fp64: erfcx(z) = (2C/(z+C)) Q((z-C)/(z+C)), z >= {ZMIN}, C = {C64}, degree {N64}, max rel err {e64:.2e}; "
+                f"Q - (1-y)Q' (divided-difference form) {b64:.2e}\n")
+        f.write(f"// erfcx fp32: same form, C = {C32}, degree {N32}, max rel err {e32:.2e}; Q - (1-y)Q' {b32:.2e}\n")
         f.write(f"// ninv tail : -Phi^-1(p) = u - R(1/(1+u)), u = sqrt(-2 ln p), p <= 0.345 (z >= 0.4), degree 7, max rel err {en:.2e}\n")
         f.write(f"// exp       : degree {NEXP} polynomial on |r| <= ln2/2, max rel err {eexp:.2e}\n")
         f.write(f"// atanh     : atanh(f) = f (1 + w G(w)), w = f^2, G degree {NATH}, |f| <= {float(FMAX):.4f}, max rel err {eath:.2e}\n")
@@ -186,6 +222,7 @@ def main():
         f.write("__constant__ double kExpP[kExpN + 1] = {\n" + fmt(aexp) + "};\n")
         f.write(f"constexpr int kAtanhN = {NATH};\n")
         f.write("__constant__ double kAtanhG[kAtanhN + 1] = {\n" + fmt(aath) + "};\n")
+        f.write(f"constexpr double kErfcxZmin = {ZMIN};   // the erfcx forms are fitted for z >= kErfcxZmin\n")
         f.write(f"constexpr double kErfcxC = {C64};\nconstexpr int kErfcxN = {N64};\n")
         f.write("__constant__ double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
         f.write(f"constexpr float kErfcxCf = {C32}f;\nconstexpr int kErfcxNf = {N32};\n")

@@ -50,7 +50,8 @@ __constant__ double kInvSqrt3 = 0.57735026918962576451;        // 1/sqrt(3)
 __constant__ double kLog2e = 1.4426950408889634074;            // 1/ln 2
 __constant__ double kLn2 = 0.69314718055994530942;             // ln 2 (nearest double)
 __constant__ double kLn2Lo = 2.3190468138462995584e-17;        // ln 2 - (double)ln 2
-__constant__ double kSmallT = 0.1;                              // series / erfcx switch-over
+__constant__ double kSmallT = 0.1;                              // |h| - t below -kSmallT: sum form of eval_W; t_c below it: series for s_l
+__constant__ double kSqrt2 = 1.4142135623730950488;            // sqrt(2)
 __constant__ double kSqrt2m1 = 0.41421356237309504880;         // sqrt(2) - 1
 __constant__ double kSeriesC[5] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0};
 __constant__ double kNinvCut = -1.0651;                         // ln 0.345: domain of the Phi^-1 tail fit
@@ -264,18 +265,65 @@ template <bool FULL> __device__ __forceinline__ double g_erfcx(double z) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// erfcx(z1) - erfcx(z2) and erfcx(z1) + erfcx(z2) for z1 >= kErfcxZmin, z2 = z1 + delta, delta >= 0 handed in as formed by
+// the caller WITHOUT cancellation.  With r = 1/(z + C), y = 1 - 2C r, erfcx(z) = 2C r Q(y) and the divided difference
+// DQ = Q[y1, y2] (one Horner-type recurrence beside the one of Q(y1): c_k = b_{k+1} + y2 c_{k+1}; no division):
+//   y2 - y1 = 2C delta r1 r2,        Q(y2) = Q(y1) + (y2 - y1) DQ,
+//   erfcx(z1) - erfcx(z2) = 2C delta r1 r2 [Q(y1) - 2C r2 DQ]     a PRODUCT: full relative accuracy however small delta is
+//   erfcx(z1) + erfcx(z2) = 2C [r1 Q(y1) + r2 Q(y2)]
+// (Q - 2C r Q' = -erfcx'(z) (z + C)^2 / 2C runs from 2.26 at z = 0 to 1/(2C sqrt(pi)) at infinity with both terms positive:
+// no cancellation inside the bracket either.)  Same cost as two independent erfcx evaluations, and it replaces the
+// small-t Taylor series of W that round 1 needed where the plain difference cancels.
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double erfcx_dd(double z1, double z2, double delta, bool want_sum) {
+  const double d1 = z1 + kErfcxC, d2 = z2 + kErfcxC;
+  const double r12 = rcp_nr2(d1 * d2);            // = r1 r2
+  const double r1 = r12 * d2, r2 = r12 * d1;
+  const double y1 = fma(-2.0 * kErfcxC, r1, 1.0), y2 = fma(-2.0 * kErfcxC, r2, 1.0);
+  double b = kErfcxQ[kErfcxN], c = 0.0;
+#pragma unroll
+  for (int k = kErfcxN - 1; k >= 0; --k) {
+    c = fma(c, y2, b);
+    b = fma(b, y1, kErfcxQ[k]);
+  }
+  const double p = (2.0 * kErfcxC) * delta * r12;  // y2 - y1
+  const double diff = p * fma(-2.0 * kErfcxC, r2 * c, b);
+  const double sum = (2.0 * kErfcxC) * fma(r1, b, r2 * fma(p, c, b));
+  return want_sum ? sum : diff;
+}
+
+// ... at seed grade: fp32, on the FMA pipe (relative error ~2e-6 in either result)
+__device__ __forceinline__ float erfcx_dd_seed(float z1, float z2, float delta, bool want_sum) {
+  const float d1 = z1 + kErfcxCf, d2 = z2 + kErfcxCf;
+  const float r12 = rcpf(d1 * d2);
+  const float r1 = r12 * d2, r2 = r12 * d1;
+  const float y1 = fmaf(-2.0f * kErfcxCf, r1, 1.0f), y2 = fmaf(-2.0f * kErfcxCf, r2, 1.0f);
+  float b = kErfcxQf[kErfcxNf], c = 0.0f;
+#pragma unroll
+  for (int k = kErfcxNf - 1; k >= 0; --k) {
+    c = fmaf(c, y2, b);
+    b = fmaf(b, y1, kErfcxQf[k]);
+  }
+  const float p = (2.0f * kErfcxCf) * delta * r12;
+  const float diff = p * fmaf(-2.0f * kErfcxCf, r2 * c, b);
+  const float sum = (2.0f * kErfcxCf) * fmaf(r1, b, r2 * fmaf(p, c, b));
+  return want_sum ? sum : diff;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // W-evaluation shared by the node stage and the Householder stages: at the point s returns
-//   have_W = true : Wd = W = b/b'            (z1 >= 0, or the small-t series)
-//   have_W = false: Wd = Wbar = (b_max-b)/b' (z1 < 0)
-// together with h = x/s, 1/s and E = (h^2+t^2)/2.
+//   have_W = true : Wd = W = b/b'     = c [erfcx(z1) - erfcx(z2)]    (z1 >= -0.1/sqrt2: the difference form, by erfcx_dd)
+//   have_W = false: Wd = Wbar = (b_max-b)/b' = c [erfcx(-z1) + erfcx(z2)]   (z1 < -0.1/sqrt2, which implies t > 0.1)
+// together with h = x/s, 1/s and E = (h^2+t^2)/2.   z1 = (|h| - t)/sqrt2, z2 = (|h| + t)/sqrt2.
+// The gap delta of erfcx_dd is sqrt2 t (difference form) or sqrt2 |h| (sum form: z2 - (-z1)), both formed directly.
 // ---------------------------------------------------------------------------------------------------------------
 struct WEval {
   double Wd, E, h, rs;
   bool have_W;
 };
 
-// SEED = true: the erfcx pair in fp32 on the FMA pipe (2e-7): enough for the node of the seed interpolant, where
-// z1 = O(1) by construction (no cancellation in e1 - e2) and |h| ~ 0.8 whenever the small-t series is taken.
+// SEED = true: the erfcx pair in fp32 on the FMA pipe (~2e-6): enough for the node of the seed interpolant and for every
+// Householder step but the last.
 template <bool SEED = false>
 __device__ __forceinline__ WEval eval_W(double x, double s) {
   WEval w;
@@ -284,44 +332,16 @@ __device__ __forceinline__ WEval eval_W(double x, double s) {
   const double t = 0.5 * s;
   const double ah = -w.h;
   w.E = 0.5 * fma(w.h, w.h, t * t);
-  const bool small = t < kSmallT;
-  const double z1 = (ah - t) * kInvSqrt2;
-  const bool neg = z1 < 0.0;
-  double e1, e2;
+  const double dz = ah - t;            // sqrt2 z1
+  const bool sum = dz < -kSmallT;      // z1 < -0.0707 (> kErfcxZmin)
+  w.have_W = !sum;
   if (SEED) {
-    e1 = (double)erfcx_seed(__double2float_rn(small ? ah * kInvSqrt2 : fabs(z1)));
-    e2 = (double)erfcx_seed(__double2float_rn((ah + t) * kInvSqrt2));
+    const float ahf = __double2float_rn(ah), tf = __double2float_rn(t);
+    const float dzf = ahf - tf;
+    const float e = erfcx_dd_seed((sum ? -dzf : dzf) * 0.70710678f, (ahf + tf) * 0.70710678f, (sum ? ahf : tf) * 1.41421356f, sum);
+    w.Wd = (double)(1.2533141f * e);
   } else {
-    erfcx_pair(small ? ah * kInvSqrt2 : fabs(z1), (ah + t) * kInvSqrt2, e1, e2);
-  }
-  w.have_W = small || !neg;
-  if (small) {
-    const double h = w.h;
-    const double w0 = kSqrtPiOver2 * e1;
-    const double w1 = fma(h, w0, 1.0);
-    const double w2 = fma(h, w1, w0);
-    const double w3 = fma(h, w2, 2.0 * w1);
-    const double w4 = fma(h, w3, 3.0 * w2);
-    const double w5 = fma(h, w4, 4.0 * w3);
-    const double t2 = t * t;
-    double acc = w5 * kSeriesC[1];
-    if (!SEED) {   // seed grade stops at the t^5 term (t < 0.1: the next one is below 1e-8)
-      const double w6 = fma(h, w5, 5.0 * w4);
-      const double w7 = fma(h, w6, 6.0 * w5);
-      const double w8 = fma(h, w7, 7.0 * w6);
-      const double w9 = fma(h, w8, 8.0 * w7);
-      const double w10 = fma(h, w9, 9.0 * w8);
-      const double w11 = fma(h, w10, 10.0 * w9);
-      acc = w11 * kSeriesC[4];
-      acc = fma(acc, t2, w9 * kSeriesC[3]);
-      acc = fma(acc, t2, w7 * kSeriesC[2]);
-      acc = fma(acc, t2, w5 * kSeriesC[1]);
-    }
-    acc = fma(acc, t2, w3 * kSeriesC[0]);
-    acc = fma(acc, t2, w1);
-    w.Wd = s * acc;  // 2 t acc
-  } else {
-    w.Wd = kSqrtPiOver2 * (neg ? e1 + e2 : e1 - e2);
+    w.Wd = kSqrtPiOver2 * erfcx_dd((sum ? -dz : dz) * kInvSqrt2, (ah + t) * kInvSqrt2, (sum ? ah : t) * kSqrt2, sum);
   }
   return w;
 }

@@ -36,6 +36,16 @@ debug_math_kernel(int fn, const double* __restrict__ a, const double* __restrict
     case PIVOT_DBG_NINV_TAIL_FULL: r = ninv_tail_full(x); break;
     case PIVOT_DBG_EXPF_SEED: r = (double)expf_seed(__double2float_rn(x)); break;
     case PIVOT_DBG_LOGF_SEED: r = (double)logf_seed(__double2float_rn(x)); break;
+    case PIVOT_DBG_ERFCX_DD_DIFF: r = erfcx_dd(x, x + y, y, false); break;
+    case PIVOT_DBG_ERFCX_DD_SUM: r = erfcx_dd(x, x + y, y, true); break;
+    case PIVOT_DBG_ERFCX_DD_SEED_DIFF:
+    case PIVOT_DBG_ERFCX_DD_SEED_SUM: {
+      const float z1 = __double2float_rn(x), d = __double2float_rn(y);
+      r = (double)erfcx_dd_seed(z1, z1 + d, d, fn == PIVOT_DBG_ERFCX_DD_SEED_SUM);
+      break;
+    }
+    case PIVOT_DBG_W_FULL: { const WEval w = eval_W<false>(x, y); r = w.have_W ? w.Wd : -w.Wd; break; }
+    case PIVOT_DBG_W_SEED: { const WEval w = eval_W<true>(x, y); r = w.have_W ? w.Wd : -w.Wd; break; }
     default: r = canonical_nan(); break;
   }
   out[i] = r;
@@ -48,7 +58,8 @@ extern "C" int pivot_iv_debug_math(int fn, const double* a, const double* b, int
   if (fn < 0 || fn >= PIVOT_DBG_COUNT) return PIVOT_ERR_BAD_ARG;
   if (n == 0) return PIVOT_OK;
   if (!a || !out) return PIVOT_ERR_NULL;
-  const bool two = fn == PIVOT_DBG_ERFCX_PAIR_1 || fn == PIVOT_DBG_ERFCX_PAIR_2 || fn == PIVOT_DBG_DIV_FAST;
+  const bool two = fn == PIVOT_DBG_ERFCX_PAIR_1 || fn == PIVOT_DBG_ERFCX_PAIR_2 || fn == PIVOT_DBG_DIV_FAST ||
+                   (fn >= PIVOT_DBG_ERFCX_DD_DIFF && fn <= PIVOT_DBG_W_SEED);
   if (two && !b) return PIVOT_ERR_NULL;
   const int64_t blocks = (n + 255) / 256;
   if (blocks > 0x7fffffff) return PIVOT_ERR_BAD_N;

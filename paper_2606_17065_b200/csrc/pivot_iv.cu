@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cstddef>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
@@ -99,8 +100,16 @@ struct TileSmem {
   uint8_t status[kTileRows];
   unsigned n01;               // rows per class: zone 0 | zones 1-2 << 16  (one native 32-bit shared atomic per warp)
   unsigned n2;                // ... zone 3
-  int count;                  // queued rows
+  unsigned count;             // queued rows
 };
+
+// shared-memory atomic add issued by ONE lane: written as PTX so that the compiler does not wrap it in its warp-aggregation
+// sequence (vote / find-leader / popc / shuffle: ~25 instructions around an atomic that a single lane executes anyway)
+__device__ __forceinline__ unsigned smem_atomic_add(unsigned* addr, unsigned v) {
+  unsigned old;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"((unsigned)__cvta_generic_to_shared(addr)), "r"(v) : "memory");
+  return old;
+}
 
 // A row the fast prelude could not classify (status 5): lbr_prelude_exact on its inputs, staged outputs, and its own
 // queue slot (flagged: lbr_normalise then takes the IEEE square root).
@@ -115,7 +124,7 @@ __device__ __noinline__ void tile_rare_row(pivot_iv_inputs in, int64_t base, int
   sm.sig[p] = queued ? tau : (pr.status == 4 ? 0.0 : canonical_nan());
   sm.veg[p] = queued ? pr.D : 0.0;
   if (queued) {
-    const int slot = atomicAdd(&sm.count, 1);
+    const int slot = (int)atomicAdd(&sm.count, 1u);
     PIVOT_ASSERT(slot >= 0 && slot < TileSmem<RPT>::kTileRows && p >= 0 && p < TileSmem<RPT>::kTileRows);
     sm.q0[slot] = pr.U;
     sm.q1[slot] = pr.O;
@@ -139,7 +148,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const int lane = tid & 31;
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
   const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
-  if (tid == 0) { sm.count = 0; sm.n01 = 0u; sm.n2 = 0u; }
+  if (tid == 0) { sm.count = 0u; sm.n01 = 0u; sm.n2 = 0u; }
   {
     // L2 prefetch for the CTA that will run about one residency later on this SM slot (blockIdx.x + kPrefetchDist): its phase A
     // then finds its 40 (56) KB of inputs in L2 instead of waiting for HBM while nothing else of that CTA can run
@@ -216,9 +225,9 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       bal[k] = __ballot_sync(0xffffffffu, (qmask >> k) & 1u);
       total += __popc(bal[k]);
     }
-    int wbase = 0;
-    if (lane == 0 && total > 0) wbase = atomicAdd(&sm.count, total);
-    int slot = __shfl_sync(0xffffffffu, wbase, 0);
+    unsigned wbase = 0u;
+    if (lane == 0 && total > 0) wbase = smem_atomic_add(&sm.count, (unsigned)total);
+    int slot = (int)__shfl_sync(0xffffffffu, wbase, 0);
     const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
     for (int k = 0; k < RPT; ++k) {
@@ -242,7 +251,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
 
   // ---- phase B1: normalisation, x, boundary point, node, zone; middle zones (1, 2) finished; rows regrouped by zone class
   //      lists: zone 0 (-> LOWER) from the front of perm, finished LINEAR rows from the back, zone 3 in permU
-  const int cnt = sm.count;
+  const int cnt = (int)sm.count;
   for (int j0 = 0; j0 < cnt; j0 += kTileThreads) {   // j0 is CTA-uniform: every lane reaches the ballots
     const int j = j0 + tid;
     int cls = -1;  // 0: zone 0, 1: finished (zones 1, 2), 2: zone 3
@@ -263,8 +272,8 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     // native 32-bit shared atomics hand out the list offsets: one for zone 0 / middle, one for zone 3 (if any)
     unsigned base01 = 0u, base2 = 0u;
     if (lane == 0) {
-      base01 = atomicAdd(&sm.n01, (unsigned)__popc(m0) | ((unsigned)__popc(m1) << 16));
-      if (m2) base2 = atomicAdd(&sm.n2, (unsigned)__popc(m2));
+      base01 = smem_atomic_add(&sm.n01, (unsigned)__popc(m0) | ((unsigned)__popc(m1) << 16));
+      if (m2) base2 = smem_atomic_add(&sm.n2, (unsigned)__popc(m2));
     }
     base01 = __shfl_sync(0xffffffffu, base01, 0);
     base2 = __shfl_sync(0xffffffffu, base2, 0);
@@ -273,9 +282,13 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     PIVOT_ASSERT(cls != 0 || (b0 + __popc(m0 & lt) >= 0 && b0 + __popc(m0 & lt) < kTileRows));
     PIVOT_ASSERT(cls != 1 || (kTileRows - 1 - (b1 + __popc(m1 & lt)) >= 0 && b0 + b1 + __popc(m1 & lt) < kTileRows));
     PIVOT_ASSERT(cls != 2 || (b2 + __popc(m2 & lt) >= 0 && b2 + __popc(m2 & lt) < kTileRows));
-    if (cls == 0) sm.perm[b0 + __popc(m0 & lt)] = (uint16_t)j;
-    else if (cls == 1) sm.perm[kTileRows - 1 - (b1 + __popc(m1 & lt))] = (uint16_t)j;
-    else if (cls == 2) sm.permU[b2 + __popc(m2 & lt)] = (uint16_t)j;
+    {
+      // one store: perm and permU are adjacent (permU[i] = perm[kTileRows + i])
+      static_assert(offsetof(TileSmem<RPT>, permU) == offsetof(TileSmem<RPT>, perm) + sizeof(uint16_t) * kTileRows, "perm | permU");
+      const int r = __popc((cls == 0 ? m0 : (cls == 1 ? m1 : m2)) & lt);
+      const int idx = (cls == 0) ? b0 + r : ((cls == 1) ? kTileRows - 1 - b1 - r : kTileRows + b2 + r);
+      if (cls >= 0) sm.perm[idx] = (uint16_t)j;
+    }
   }
   __syncthreads();
 

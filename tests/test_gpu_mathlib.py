@@ -42,7 +42,8 @@ def _lu(rng, lo, hi, n):
 
 def test_erfcx_fp64_and_seed():
     rng = np.random.default_rng(1)
-    z = np.concatenate([[0.0, 1e-300, 1e-17, 0.5, 1.0, 4.0, 26.0, 1e3, 1e8], rng.uniform(0, 8, 1500), _lu(rng, 1e-6, 1e3, 1500)])
+    z = np.concatenate([[0.0, 1e-300, 1e-17, 0.5, 1.0, 4.0, 26.0, 1e3, 1e8, -0.0708, -0.05, -1e-9], rng.uniform(0, 8, 1500),
+                        _lu(rng, 1e-6, 1e3, 1500), rng.uniform(-0.0708, 0, 200)])
     ref = [_erfcx(v) for v in z]
     e_one = _relerr(_run("erfcx_one", z), ref)
     z2 = z[::-1].copy()
@@ -50,8 +51,72 @@ def test_erfcx_fp64_and_seed():
     e_p2 = _relerr(_run("erfcx_pair_2", z2, z), ref)
     e_seed = _relerr(_run("erfcx_seed", z), ref)
     print(f"erfcx_one {e_one:.2e}  pair {max(e_p1, e_p2):.2e}  seed {e_seed:.2e}")
-    assert e_one <= 8 * EPS and e_p1 <= 8 * EPS and e_p2 <= 8 * EPS      # fit error 4.8e-16 + evaluation rounding
+    assert e_one <= 8 * EPS and e_p1 <= 8 * EPS and e_p2 <= 8 * EPS      # fit error 5.7e-16 + evaluation rounding
     assert e_seed <= 6e-7
+
+
+def test_erfcx_divided_difference_forms():
+    """erfcx(z1) -/+ erfcx(z1 + d) from the divided difference of the fitted polynomial (lbr_device.cuh: erfcx_dd): the
+    difference keeps its RELATIVE accuracy however small the gap d is (it replaced the small-t Taylor series of W)."""
+    rng = np.random.default_rng(11)
+    n = 4000
+    z1 = np.concatenate([rng.uniform(-0.0708, 1, n // 4), rng.uniform(0, 30, n // 4), _lu(rng, 1e-8, 50, n // 4),
+                         rng.uniform(-0.0708, 0.0, n // 4)])
+    d = _lu(rng, 1e-12, 60, n)
+    d[:50] = 0.0
+    z2 = z1 + d
+    d = z2 - z1                                   # the gap the device sees (exact)
+    ref_d = [_erfcx(a) - _erfcx(b) for a, b in zip(z1, z2)]
+    ref_s = [_erfcx(a) + _erfcx(b) for a, b in zip(z1, z2)]
+    e_d = _relerr(_run("erfcx_dd_diff", z1, d), ref_d)
+    e_s = _relerr(_run("erfcx_dd_sum", z1, d), ref_s)
+    # the seed-grade form sees float-rounded arguments
+    z1f, df = z1.astype(np.float32).astype(np.float64), d.astype(np.float32).astype(np.float64)
+    z1f = np.maximum(z1f, -0.0708)
+    ref_df = [_erfcx(a) - _erfcx(mp.mpf(float(a)) + mp.mpf(float(g))) for a, g in zip(z1f, df)]
+    ref_sf = [_erfcx(a) + _erfcx(mp.mpf(float(a)) + mp.mpf(float(g))) for a, g in zip(z1f, df)]
+    e_df = _relerr(_run("erfcx_dd_seed_diff", z1f, df), ref_df)
+    e_sf = _relerr(_run("erfcx_dd_seed_sum", z1f, df), ref_sf)
+    print(f"erfcx_dd diff {e_d:.2e} sum {e_s:.2e}  seed diff {e_df:.2e} seed sum {e_sf:.2e}")
+    assert e_d <= 16 * EPS and e_s <= 8 * EPS
+    assert e_df <= 2e-5 and e_sf <= 2e-6
+
+
+def test_eval_W_against_the_definition():
+    """eval_W (the ratio every Householder step is built on) against W = b/b', Wbar = (b_max - b)/b' from the literal
+    eq.(4) in mpmath, over small and large t, |h| from 0 to 36, both sides of the difference / sum switch."""
+    rng = np.random.default_rng(12)
+    n = 3000
+    s = _lu(rng, 1e-6, 40, n)
+    h = -np.concatenate([rng.uniform(0, 36, n // 2), _lu(rng, 1e-8, 5, n // 2)])
+    x = h * s
+    x[:20] = 0.0
+    keep = (np.abs(x) < 600)
+    x, s = x[keep], s[keep]
+
+    def W_ref(xv, sv):
+        xv, sv = mp.mpf(float(xv)), mp.mpf(float(sv))
+        hh, t = xv / sv, sv / 2
+        Phi = lambda z: mp.erfc(-z / mp.sqrt(2)) / 2
+        bmax = mp.exp(xv / 2)
+        b = bmax * Phi(hh + t) - Phi(hh - t) / bmax
+        bp = mp.exp(-(hh * hh + t * t) / 2) / mp.sqrt(2 * mp.pi)
+        return b / bp, (bmax - b) / bp
+
+    old = mp.mp.dps
+    mp.mp.dps = 400          # b underflows against b_max at 40 digits when |h| is large
+    try:
+        refs = [W_ref(a, b) for a, b in zip(x, s)]
+    finally:
+        mp.mp.dps = old
+    for name, tol in (("w_full", 3e-14), ("w_seed", 3e-5)):
+        got = _run(name, x, s)
+        worst = 0.0
+        for g, (W, Wb), xv, sv in zip(got, refs, x, s):
+            ref = W if g > 0 else -Wb
+            worst = max(worst, float(abs(mp.mpf(float(g)) / ref - 1)))
+        print(f"{name} max rel err {worst:.2e}")
+        assert worst <= tol, name
 
 
 def test_exp_fast_full_range_and_seed():
