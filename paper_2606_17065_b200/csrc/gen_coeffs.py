@@ -224,7 +224,7 @@ def main():
         f.write("__constant__ double kAtanhG[kAtanhN + 1] = {\n" + fmt(aath) + "};\n")
         f.write(f"constexpr double kErfcxZmin = {ZMIN};   // the erfcx forms are fitted for z >= kErfcxZmin\n")
         f.write(f"constexpr double kErfcxC = {C64};\nconstexpr int kErfcxN = {N64};\n")
-        f.write("__constant__ double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
+        f.write("__constant__ __align__(16) double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
         f.write(f"constexpr float kErfcxCf = {C32}f;\nconstexpr int kErfcxNf = {N32};\n")
         f.write("__device__ constexpr float kErfcxQf[kErfcxNf + 1] = {\n" + fmt(a32, 4, True) + "};\n")
         f.write("constexpr int kNinvN = 7;\n")

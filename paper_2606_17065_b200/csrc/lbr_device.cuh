@@ -275,16 +275,32 @@ template <bool FULL> __device__ __forceinline__ double g_erfcx(double z) {
 // no cancellation inside the bracket either.)  Same cost as two independent erfcx evaluations, and it replaces the
 // small-t Taylor series of W that round 1 needed where the plain difference cancels.
 // ---------------------------------------------------------------------------------------------------------------
+// Two adjacent doubles of a __constant__ table, loaded into ordinary registers where they are used.  sm_100a instructions
+// take no constant-bank operand: every constant passes through a register, the compiler hoists all such loads out of the pass
+// loops into UNIFORM registers, and once those run out (the fp64 erfcx table alone needs 50) it parks the overflow in vector
+// registers and swaps it in and out through MOV.SPILL / R2UR (3.7 % of the issued instructions, ~12 vector registers).
+// `vary` is a per-thread byte offset that is always 0 but that the compiler cannot prove uniform: the load then is a plain
+// LDC.128 into vector registers, outside the uniform register file.
+__device__ __forceinline__ void ldc_pair(const double* p, unsigned vary, double& lo, double& hi) {
+  asm volatile("ld.const.v2.f64 {%0, %1}, [%2];" : "=d"(lo), "=d"(hi) : "l"(__cvta_generic_to_constant(p) + vary));
+}
+
 __device__ __forceinline__ double erfcx_dd(double z1, double z2, double delta, bool want_sum) {
+  static_assert(kErfcxN % 2 == 0, "the pairs (k-2, k-1) start at even indices");
   const double d1 = z1 + kErfcxC, d2 = z2 + kErfcxC;
   const double r12 = rcp_nr2(d1 * d2);            // = r1 r2
   const double r1 = r12 * d2, r2 = r12 * d1;
   const double y1 = fma(-2.0 * kErfcxC, r1, 1.0), y2 = fma(-2.0 * kErfcxC, r2, 1.0);
+  const unsigned vary = (__double2hiint(delta) < 0) ? 16u : 0u;   // delta >= 0: always 0
   double b = kErfcxQ[kErfcxN], c = 0.0;
 #pragma unroll
-  for (int k = kErfcxN - 1; k >= 0; --k) {
+  for (int k = kErfcxN; k >= 2; k -= 2) {
+    double q0, q1;
+    ldc_pair(&kErfcxQ[k - 2], vary, q0, q1);
     c = fma(c, y2, b);
-    b = fma(b, y1, kErfcxQ[k]);
+    b = fma(b, y1, q1);
+    c = fma(c, y2, b);
+    b = fma(b, y1, q0);
   }
   const double p = (2.0 * kErfcxC) * delta * r12;  // y2 - y1
   const double diff = p * fma(-2.0 * kErfcxC, r2 * c, b);
@@ -394,7 +410,8 @@ __device__ __forceinline__ R rcn_G(R u, R omu, R Dl, R Dr, R r) {
 // ---------------------------------------------------------------------------------------------------------------
 struct SeedHead {
   int zone;        // 0: tail pending, v = (x, s_n, beta, pack(W_n, beta/b_n));  3: tail pending, v = (x, s_n, bbar,
-                   // pack(Wbar_n, bbar/bbar_n));  1, 2: finished, v = (x, s0, beta, bbar)
+                   // pack(Wbar_n, bbar/bbar_n));  1, 2: v = (x, pack(-+s_n, wq), beta, pack(Dr, Dl)) for lbr_seed_mid (sign
+                   // bit of the first float set: zone 1); FULL tier: finished, v = (x, s0, beta, bbar)
   double v0, v1, v2, v3;
 };
 
@@ -445,7 +462,13 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   o.v2 = beta; o.v3 = bbar;
   if (lower && !(sl > 1e-30)) {  // rounding / fp32-range guard, |x| below ~1e-30: linear seed
     o.zone = 1;
-    o.v1 = sc * beta * rcp_nr1(bc);
+    const double lin = beta * rcp_nr1(bc);
+    if (FULL) {
+      o.v1 = sc * lin;
+    } else {   // the same linear seed through lbr_seed_mid: node at s = 0, Dl = Dr = 1 (G = 1)
+      o.v1 = pack2f(-0.0f, __double2float_rn(lin));
+      o.v3 = pack2f(1.0f, 1.0f);
+    }
     return o;
   }
   const double sn = lower ? sl : sc + Wbc;    // s_l, or s_u where the tangent at the inflection point hits b_max
@@ -467,23 +490,30 @@ __device__ __forceinline__ SeedHead lbr_seed_head(double qrel, double beta, doub
   }
   // zones 1 and 2: s(beta) from the node (u = 0) to the inflection point (u = 1), s'' = 0 at the inflection point.
   // With kappa = b'(s_c)/b'(s_n) = exp(E_n - |x|/2) and rho = b_n/b_c (lower) or (b_max-b_n)/(b_max-b_c) (upper):
-  //   Dr = 1 - rho,  Dl = kappa (1 - rho),  DD = 0.
-  typedef typename std::conditional<FULL, double, float>::type R;
+  //   Dr = 1 - rho = |b_c - b_n| / (b_c or b_max - b_c),  Dl = kappa (1 - rho),  DD = 0.
+  // The interpolant is evaluated from the end with the SMALLER s (the node s_l below the inflection point, the inflection
+  // point itself above it), so that s keeps its relative accuracy when s_c -> 0 (|x| -> 0): wq is the abscissa measured from
+  // that end.  Default tier: only the three dimensionless parameters (wq, Dr, Dl) are formed here, where ~9 of 32 lanes are
+  // middle-zone rows; the fp32 rational cubic itself runs in lbr_seed_mid on warps that hold middle-zone rows only.
   o.zone = lower ? 1 : 2;
   const double bbc = vc * Wbc;
-  const double rho = (lower ? bn : bbn) * g_rcp<FULL>(lower ? bc : bbc);
+  const double H = bc - bn;                         // > 0 below the inflection point, < 0 above it
+  const double aH = fabs(H), den = lower ? bc : bbc;
+  const double rHD = g_rcp<FULL>(aH * den);
+  const double rH = rHD * den;                      // 1/|H|
+  const double Drd = aH * (rHD * aH);               // |H| / den
   const double kappa = vc * g_rcp<FULL>(vn);
-  const double H = bc - bn, rH = g_rcp<FULL>(H);
-  const R u = (R)((beta - bn) * rH), omu = (R)((bc - beta) * rH);
-  const R Dr = (R)(1.0 - rho);
-  const double Dld = kappa * (1.0 - rho);
-  const R Dl = (R)dmin_nn(Dld, 1e30);
-  const R r = rcn_control<R>(Dl, Dr, R(0));
-  // evaluated from the end with the SMALLER s (the node s_l below the inflection point, the inflection point itself
-  // above it), so that s keeps its relative accuracy when s_c -> 0 (|x| -> 0): the interpolant is reversal invariant
-  const R wq = lower ? u : omu, omw = lower ? omu : u;
-  const R Y = wq * rcn_G<R>(wq, omw, lower ? Dl : Dr, lower ? Dr : Dl, r);
-  const double s = fma(fabs(sc - sn), (double)Y, lower ? sn : sc);
+  const double wqd = (lower ? beta - bn : beta - bc) * rH;
+  const double Dld = dmin_nn(kappa * Drd, 1e30);
+  if (!FULL) {
+    const float snf = __double2float_rn(sn);
+    o.v1 = pack2f(lower ? -snf : snf, __double2float_rn(wqd));
+    o.v3 = pack2f(__double2float_rn(Drd), __double2float_rn(Dld));
+    return o;
+  }
+  const double r = rcn_control<double>(Dld, Drd, 0.0);
+  const double Y = wqd * rcn_G<double>(wqd, 1.0 - wqd, lower ? Dld : Drd, lower ? Drd : Dld, r);
+  const double s = fma(fabs(sc - sn), Y, lower ? sn : sc);
   o.v1 = (s > 0.0 && is_fin(s)) ? s : sc;   // a failed interpolant falls back to the inflection point
   return o;
 }
@@ -492,6 +522,28 @@ struct Seed {
   double x, s, p1, p2;
   int kind, zone;
 };
+
+// zones 1, 2 (default tier): the fp32 rational cubic on the parameters lbr_seed_head packed (header comment there).
+// The objective is LINEAR with p1 = beta; p2 = b_max - beta is rebuilt here (in these zones b_max - beta >= 0.1 b_max:
+// at s_u, Phi(-(h+t)) >= Phi(-1.3), so the subtraction costs at most 3 bits of a quantity that only enters where
+// Wbar is the ratio at hand).
+__device__ __forceinline__ Seed lbr_seed_mid(double x, double packed_sn_wq, double beta, double packed_D) {
+  Seed o;
+  o.x = x; o.kind = KIND_LINEAR; o.p1 = beta;
+  float sns, wq, Dr, Dl;
+  unpack2f(packed_sn_wq, sns, wq);
+  unpack2f(packed_D, Dr, Dl);
+  const bool lower = __float_as_int(sns) < 0;
+  o.zone = lower ? 1 : 2;
+  const double sn = (double)fabsf(sns);
+  const double sc = sqrt_nr1(-2.0 * x);
+  const float r = rcn_control<float>(Dl, Dr, 0.0f);
+  const float Y = wq * rcn_G<float>(wq, 1.0f - wq, lower ? Dl : Dr, lower ? Dr : Dl, r);
+  const double s = fma(fabs(sc - sn), (double)Y, lower ? sn : sc);
+  o.s = (s > 0.0 && is_fin(s)) ? s : sc;   // a failed interpolant falls back to the inflection point
+  o.p2 = exp_fast(0.5 * x) - beta;
+  return o;
+}
 
 // zone 0: f_low(s) = (2 pi |x| / 3 sqrt3) Phi(-z)^3, z = |x| / (sqrt3 s), as a function of beta on [0, b_l].
 // In normalised variables (u = beta/b_l, Y = f/f_low(s_l)) with q = |x|/s_l = sqrt3 z, omega = W_l/s_l,
@@ -589,6 +641,7 @@ __device__ __forceinline__ Seed lbr_seed(double qrel, double beta, double bbar, 
   const SeedHead hd = lbr_seed_head<FULL>(qrel, beta, bbar, bmax);
   if (hd.zone == 0) return lbr_seed_tail0<FULL>(hd.v0, hd.v1, hd.v2, hd.v3);
   if (hd.zone == 3) return lbr_seed_tail3<FULL>(hd.v0, hd.v1, hd.v2, hd.v3);
+  if (!FULL) return lbr_seed_mid(hd.v0, hd.v1, hd.v2, hd.v3);
   Seed o;
   o.x = hd.v0; o.s = hd.v1; o.p1 = hd.v2; o.p2 = hd.v3; o.kind = KIND_LINEAR; o.zone = hd.zone;
   return o;

@@ -305,7 +305,13 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = KIND_LOWER;
     } else if (k < n0 + n1) {
       j = sm.perm[kTileRows - 1 - (k - n0)];
-      x = sm.q0[j]; s0 = sm.q1[j]; p1 = sm.q2[j]; p2 = sm.q3[j]; kind = KIND_LINEAR;
+      if (FULL) {
+        x = sm.q0[j]; s0 = sm.q1[j]; p1 = sm.q2[j]; p2 = sm.q3[j];
+      } else {
+        const Seed sd = lbr_seed_mid(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
+        x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2;
+      }
+      kind = KIND_LINEAR;
     } else {
       j = sm.permU[k - n0 - n1];
       const Seed sd = lbr_seed_tail3<FULL>(sm.q0[j], sm.q1[j], sm.q2[j], sm.q3[j]);
