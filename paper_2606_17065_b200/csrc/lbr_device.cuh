@@ -291,7 +291,7 @@ __device__ __forceinline__ double erfcx_dd(double z1, double z2, double delta, b
   const double r12 = rcp_nr2(d1 * d2);            // = r1 r2
   const double r1 = r12 * d2, r2 = r12 * d1;
   const double y1 = fma(-2.0 * kErfcxC, r1, 1.0), y2 = fma(-2.0 * kErfcxC, r2, 1.0);
-  const unsigned vary = (__double2hiint(delta) < 0) ? 16u : 0u;   // delta >= 0: always 0
+  const unsigned vary = ((unsigned)__double2hiint(d2) >> 31) << 4;   // sign bit of d2 = z2 + C >= 3.9: always 0
   double b = kErfcxQ[kErfcxN], c = 0.0;
 #pragma unroll
   for (int k = kErfcxN; k >= 2; k -= 2) {

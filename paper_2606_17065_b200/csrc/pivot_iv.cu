@@ -45,7 +45,7 @@ struct DiagOut {
 // Best when nearly every row solves and neighbouring rows are alike (option chains in strike order).
 // ---------------------------------------------------------------------------------------------------------------
 template <bool BSM, bool DIAG, bool FULL>
-__global__ void __launch_bounds__(kFwdThreads)
+__global__ void __launch_bounds__(kFwdThreads, (FULL || DIAG) ? 1 : 7)
 forward_kernel_scalar(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                       uint8_t* __restrict__ status, DiagOut dg) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -103,11 +103,14 @@ struct TileSmem {
   unsigned count;             // queued rows
 };
 
-// shared-memory atomic add issued by ONE lane: written as PTX so that the compiler does not wrap it in its warp-aggregation
-// sequence (vote / find-leader / popc / shuffle: ~25 instructions around an atomic that a single lane executes anyway)
-__device__ __forceinline__ unsigned smem_atomic_add(unsigned* addr, unsigned v) {
+// Shared-memory atomic add issued by ONE lane.  For an atomic on a warp-uniform address ptxas emits its warp-aggregation
+// sequence (vote / find-leader / popc / multiply / shuffle: ~25 instructions) even when a single lane is active; `vary` is a
+// per-thread byte offset that is always 0 but that the compiler cannot prove uniform (a hash of tid x a bit of n that is never set), which
+// leaves the plain predicated ATOMS.ADD.
+__device__ __forceinline__ unsigned smem_atomic_add(unsigned* addr, unsigned vary, unsigned v) {
   unsigned old;
-  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"((unsigned)__cvta_generic_to_shared(addr)), "r"(v) : "memory");
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;"
+               : "=r"(old) : "r"((unsigned)__cvta_generic_to_shared(addr) + vary), "r"(v) : "memory");
   return old;
 }
 
@@ -146,6 +149,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   TileSmem<RPT>& sm = *reinterpret_cast<TileSmem<RPT>*>(smem_raw);
   const int tid = threadIdx.x;
   const int lane = tid & 31;
+  const unsigned vary = ((unsigned)tid * 40503u >> 3) * (unsigned)((uint64_t)n >> 62) * 4u;   // 0 (n < 2^38); see smem_atomic_add
   const int64_t base = (int64_t)blockIdx.x * kTileRows;
   const int rows = (int)((n - base < kTileRows) ? (n - base) : kTileRows);
   if (tid == 0) { sm.count = 0u; sm.n01 = 0u; sm.n2 = 0u; }
@@ -179,39 +183,51 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   const double* __restrict__ gq = BSM ? in.q + base : nullptr;
   double vF[RPT], vK[RPT], vT[RPT], vP[RPT],
       vf[RPT], vr[RPT], vq[RPT];
+  if (rows == kTileRows) {   // full tile (all but the last one): plain loads
 #pragma unroll
-  for (int k = 0; k < RPT; ++k) {
-    const int p = k * kTileThreads + tid;
-    const bool live = p < rows;
-    // dead rows read as flag = 0 -> BAD_INPUT, never stored
-    vF[k] = live ? __ldcs(gF + p) : 0.0;
-    vK[k] = live ? __ldcs(gK + p) : 0.0;
-    vT[k] = live ? __ldcs(gT + p) : 0.0;
-    vP[k] = live ? __ldcs(gP + p) : 0.0;
-    vf[k] = live ? __ldcs(gf + p) : 0.0;
-    vr[k] = (BSM && live) ? __ldcs(gr + p) : 0.0;
-    vq[k] = (BSM && live) ? __ldcs(gq + p) : 0.0;
+    for (int k = 0; k < RPT; ++k) {
+      const int p = k * kTileThreads + tid;
+      vF[k] = __ldcs(gF + p);
+      vK[k] = __ldcs(gK + p);
+      vT[k] = __ldcs(gT + p);
+      vP[k] = __ldcs(gP + p);
+      vf[k] = __ldcs(gf + p);
+      vr[k] = BSM ? __ldcs(gr + p) : 0.0;
+      vq[k] = BSM ? __ldcs(gq + p) : 0.0;
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      const int p = k * kTileThreads + tid;
+      const bool live = p < rows;
+      // dead rows read as flag = 0: "rare" by the fast prelude, dropped below (never stored to global memory)
+      vF[k] = live ? __ldcs(gF + p) : 0.0;
+      vK[k] = live ? __ldcs(gK + p) : 0.0;
+      vT[k] = live ? __ldcs(gT + p) : 0.0;
+      vP[k] = live ? __ldcs(gP + p) : 0.0;
+      vf[k] = live ? __ldcs(gf + p) : 0.0;
+      vr[k] = (BSM && live) ? __ldcs(gr + p) : 0.0;
+      vq[k] = (BSM && live) ? __ldcs(gq + p) : 0.0;
+    }
   }
   unsigned qmask = 0, rmask = 0;  // bit k: row k of this thread is queued / needs the exact prelude
 #pragma unroll
   for (int k = 0; k < RPT; ++k) {
     const int p = k * kTileThreads + tid;
-    const bool live = p < rows;
     const Prelude pr = lbr_prelude<BSM>(vF[k], vK[k], vT[k], vr[k], vq[k], vP[k], vf[k]);
     const bool queued = pr.status == 0;
-    if (live && pr.status != 5) {
-      sm.status[p] = (uint8_t)pr.status;
-      sm.sig[p] = queued ? vT[k] : (pr.status == 4 ? 0.0 : canonical_nan());
-      if (BSM) sm.veg[p] = queued ? pr.D : 0.0;
-      else if (!queued) sm.veg[p] = 0.0;
-      if (DIAG && !queued) {
-        if (dg.zone) dg.zone[base + p] = -1;
-        if (dg.s0) dg.s0[base + p] = 0.0;
-        if (dg.s1) dg.s1[base + p] = 0.0;
-      }
+    // staged unconditionally: the slots of dead rows (p >= rows) are never read, those of rare rows (status 5) are rewritten
+    // by tile_rare_row below, and the vega slot of a queued row is rewritten in phase B1
+    sm.status[p] = (uint8_t)pr.status;
+    sm.sig[p] = queued ? vT[k] : (pr.status == 4 ? 0.0 : canonical_nan());
+    sm.veg[p] = (BSM && queued) ? pr.D : 0.0;
+    if (DIAG && !queued && p < rows && pr.status != 5) {
+      if (dg.zone) dg.zone[base + p] = -1;
+      if (dg.s0) dg.s0[base + p] = 0.0;
+      if (dg.s1) dg.s1[base + p] = 0.0;
     }
     qmask |= queued ? (1u << k) : 0u;
-    rmask |= (live && pr.status == 5) ? (1u << k) : 0u;
+    rmask |= (pr.status == 5 && p < rows) ? (1u << k) : 0u;
     vF[k] = pr.U; vK[k] = pr.O; vP[k] = pr.B;   // what the solver pass needs
   }
   {
@@ -226,7 +242,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       total += __popc(bal[k]);
     }
     unsigned wbase = 0u;
-    if (lane == 0 && total > 0) wbase = smem_atomic_add(&sm.count, (unsigned)total);
+    if (lane == 0 && total > 0) wbase = smem_atomic_add(&sm.count, vary, (unsigned)total);
     int slot = (int)__shfl_sync(0xffffffffu, wbase, 0);
     const unsigned lt = (1u << lane) - 1u;
 #pragma unroll
@@ -272,8 +288,8 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     // native 32-bit shared atomics hand out the list offsets: one for zone 0 / middle, one for zone 3 (if any)
     unsigned base01 = 0u, base2 = 0u;
     if (lane == 0) {
-      base01 = smem_atomic_add(&sm.n01, (unsigned)__popc(m0) | ((unsigned)__popc(m1) << 16));
-      if (m2) base2 = smem_atomic_add(&sm.n2, (unsigned)__popc(m2));
+      base01 = smem_atomic_add(&sm.n01, vary, (unsigned)__popc(m0) | ((unsigned)__popc(m1) << 16));
+      if (m2) base2 = smem_atomic_add(&sm.n2, vary, (unsigned)__popc(m2));
     }
     base01 = __shfl_sync(0xffffffffu, base01, 0);
     base2 = __shfl_sync(0xffffffffu, base2, 0);

@@ -148,6 +148,33 @@ def test_edge_rows_match_oracle():
     assert set(np.unique(g[2])) == {0, 1, 2, 3, 4}
 
 
+@pytest.mark.parametrize("kernel", ["compact", "rowwise"])
+def test_exactly_at_the_money_rows(kernel):
+    """F == K exactly (x = 0, h = +-0 at every s): the closed form sigma = -2 Phi^-1((1 - beta)/2)/sqrt(T) applies, total
+    volatilities from 1e-5 to 30, so both the difference form (t <= 0.1) and the sum form of eval_W are taken with a zero
+    gap / zero |h|, in both organisations, against the oracle."""
+    rng = np.random.default_rng(77)
+    n = 20_000
+    F = 10.0 ** rng.uniform(-3, 4, n)
+    T = 10.0 ** rng.uniform(-3, 1, n)
+    s = 10.0 ** rng.uniform(-5, np.log10(30.0), n)
+    from scipy.special import ndtr
+    P = F * (2.0 * ndtr(0.5 * s) - 1.0)          # b(0, s) = 1 - 2 Phi(-s/2)
+    flag = np.where(rng.random(n) < 0.5, 1.0, -1.0)
+    cols = [F, F.copy(), T, P, flag]
+    o = po.forward(*cols)
+    kern = pv.FWD_COMPACT if kernel == "compact" else pv.FWD_ROWWISE
+    g = pv.pivot_iv_forward_ex(*[torch.from_numpy(np.ascontiguousarray(x)).cuda() for x in cols], kern)
+    g = tuple(t.cpu().numpy() for t in g)
+    c = dict(zip(KEYS, cols)); c["r"] = None; c["q"] = None
+    compare_forward(g, o, c)
+    ok = o[2] == 0
+    assert ok.sum() > 0.9 * n
+    sig_true = s / np.sqrt(T)
+    well = ok & (s > 1e-3) & (s < 8)              # where the price pins sigma to 1e-12 (time value not lost to rounding)
+    assert np.max(np.abs(g[0][well] / sig_true[well] - 1)) < 1e-8
+
+
 def test_bsm_bad_rates_and_mixed_rq_error():
     d = to_device(wl.config2(days=1, expiries=2, strikes=50))
     r = d["r"].clone(); r[3] = float("nan")
