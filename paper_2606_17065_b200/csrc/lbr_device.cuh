@@ -285,6 +285,9 @@ __device__ __forceinline__ void ldc_pair(const double* p, unsigned vary, double&
   asm volatile("ld.const.v2.f64 {%0, %1}, [%2];" : "=d"(lo), "=d"(hi) : "l"(__cvta_generic_to_constant(p) + vary));
 }
 
+// INPLACE = true: the table is read in place (ldc_pair: the tile kernel, whose pass loops overflow the uniform registers);
+// false: ordinary constant operands (the row-per-thread kernel and the single-use callers).  Same arithmetic, same bits.
+template <bool INPLACE = false>
 __device__ __forceinline__ double erfcx_dd(double z1, double z2, double delta, bool want_sum) {
   static_assert(kErfcxN % 2 == 0, "the pairs (k-2, k-1) start at even indices");
   const double d1 = z1 + kErfcxC, d2 = z2 + kErfcxC;
@@ -296,7 +299,7 @@ __device__ __forceinline__ double erfcx_dd(double z1, double z2, double delta, b
 #pragma unroll
   for (int k = kErfcxN; k >= 2; k -= 2) {
     double q0, q1;
-    ldc_pair(&kErfcxQ[k - 2], vary, q0, q1);
+    if (INPLACE) { ldc_pair(&kErfcxQ[k - 2], vary, q0, q1); } else { q0 = kErfcxQ[k - 2]; q1 = kErfcxQ[k - 1]; }
     c = fma(c, y2, b);
     b = fma(b, y1, q1);
     c = fma(c, y2, b);
@@ -340,7 +343,7 @@ struct WEval {
 
 // SEED = true: the erfcx pair in fp32 on the FMA pipe (~2e-6): enough for the node of the seed interpolant and for every
 // Householder step but the last.
-template <bool SEED = false>
+template <bool SEED = false, bool INPLACE = false>
 __device__ __forceinline__ WEval eval_W(double x, double s) {
   WEval w;
   w.rs = SEED ? rcp_nr1(s) : rcp_nr2(s);
@@ -357,7 +360,7 @@ __device__ __forceinline__ WEval eval_W(double x, double s) {
     const float e = erfcx_dd_seed((sum ? -dzf : dzf) * 0.70710678f, (ahf + tf) * 0.70710678f, (sum ? ahf : tf) * 1.41421356f, sum);
     w.Wd = (double)(1.2533141f * e);
   } else {
-    w.Wd = kSqrtPiOver2 * erfcx_dd((sum ? -dz : dz) * kInvSqrt2, (ah + t) * kInvSqrt2, (sum ? ah : t) * kSqrt2, sum);
+    w.Wd = kSqrtPiOver2 * erfcx_dd<INPLACE>((sum ? -dz : dz) * kInvSqrt2, (ah + t) * kInvSqrt2, (sum ? ah : t) * kSqrt2, sum);
   }
   return w;
 }
@@ -664,9 +667,9 @@ struct NormSolve {
 // One Householder(3) step.  SEED = true evaluates W, exp and log at seed grade (fp32 erfcx pair, MUFU exp / log,
 // ~1e-6 relative in the step): enough for every step but the last, because the step is fourth order and the last step
 // then takes an iterate that is good to ~1e-6 to ~1e-24.
-template <bool SEED>
+template <bool SEED, bool INPLACE>
 __device__ __forceinline__ double householder_step(double x, double s, double p1, double p2, int kind) {
-  const WEval w = eval_W<SEED>(x, s);
+  const WEval w = eval_W<SEED, INPLACE>(x, s);
   const double hr = w.h * w.rs;
   const double B2 = fma(w.h, hr, -0.25 * s);                  // second derivative of b over b'
   const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // third derivative of b over b'
@@ -704,13 +707,13 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
   return s + ds;
 }
 
-template <int NITER, bool FULL>
+template <int NITER, bool FULL, bool INPLACE = false>
 __device__ __forceinline__ NormSolve lbr_refine(double x, double s, double p1, double p2, int kind) {
 #pragma unroll 1
-  for (int it = 0; it < NITER - 1; ++it) s = householder_step<!FULL>(x, s, p1, p2, kind);
+  for (int it = 0; it < NITER - 1; ++it) s = householder_step<!FULL, INPLACE>(x, s, p1, p2, kind);
   NormSolve o;
   o.s1 = s;
-  s = householder_step<false>(x, s, p1, p2, kind);
+  s = householder_step<false, INPLACE>(x, s, p1, p2, kind);
   const double rs = rcp_nr2(s);
   const double h = x * rs, t = 0.5 * s;
   o.s = s;

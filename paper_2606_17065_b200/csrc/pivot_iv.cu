@@ -334,7 +334,7 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       x = sd.x; s0 = sd.s; p1 = sd.p1; p2 = sd.p2; kind = sd.kind;
     }
     PIVOT_ASSERT(j >= 0 && j < cnt && cnt <= rows && n0 + n1 + (int)sm.n2 == cnt);
-    const NormSolve ns = lbr_refine<kHouseholderSteps, FULL>(x, s0, p1, p2, kind);
+    const NormSolve ns = lbr_refine<kHouseholderSteps, FULL, true>(x, s0, p1, p2, kind);
     const int p = sm.pos[j] & 0x3fff;
     PIVOT_ASSERT(p < rows);
     const double tau = sm.sig[p];
