@@ -219,12 +219,12 @@ def main():
         f.write(f"// atanh     : atanh(f) = f (1 + w G(w)), w = f^2, G degree {NATH}, |f| <= {float(FMAX):.4f}, max rel err {eath:.2e}\n")
         f.write("#pragma once\nnamespace pivot {\n")
         f.write(f"constexpr int kExpN = {NEXP};\n")
-        f.write("__constant__ double kExpP[kExpN + 1] = {\n" + fmt(aexp) + "};\n")
+        f.write("static __constant__ double kExpP[kExpN + 1] = {\n" + fmt(aexp) + "};\n")
         f.write(f"constexpr int kAtanhN = {NATH};\n")
-        f.write("__constant__ double kAtanhG[kAtanhN + 1] = {\n" + fmt(aath) + "};\n")
+        f.write("static __constant__ double kAtanhG[kAtanhN + 1] = {\n" + fmt(aath) + "};\n")
         f.write(f"constexpr double kErfcxZmin = {ZMIN};   // the erfcx forms are fitted for z >= kErfcxZmin\n")
         f.write(f"constexpr double kErfcxC = {C64};\nconstexpr int kErfcxN = {N64};\n")
-        f.write("__constant__ __align__(16) double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
+        f.write("static __constant__ __align__(16) double kErfcxQ[kErfcxN + 1] = {\n" + fmt(a64) + "};\n")
         f.write(f"constexpr float kErfcxCf = {C32}f;\nconstexpr int kErfcxNf = {N32};\n")
         f.write("__device__ constexpr float kErfcxQf[kErfcxNf + 1] = {\n" + fmt(a32, 4, True) + "};\n")
         f.write("constexpr int kNinvN = 7;\n")

@@ -40,21 +40,21 @@ namespace pivot {
 // Scalar constants live in constant memory: an fp64 instruction takes a c[bank][offset] operand for free, whereas a
 // 64-bit immediate costs two extra MOV/UMOV issue slots (16.6 % of all issued instructions in the v3 capture,
 // profiles/r1a_forward_v3_ncu_full.md).
-__constant__ double kInvSqrt2 = 0.70710678118654752440;       // 1/sqrt(2)
-__constant__ double kSqrtPiOver2 = 1.2533141373155002512;      // sqrt(pi/2)
-__constant__ double kSqrt2Pi = 2.5066282746310005024;          // sqrt(2 pi)
-__constant__ double kPhi0 = 0.39894228040143267794;            // 1/sqrt(2 pi)
-__constant__ double kLnPhi0 = -0.91893853320467274178;         // ln(1/sqrt(2 pi))
-__constant__ double kTwoThirdsLnPhi0 = -0.61262568880311516119;  // (2/3) ln(1/sqrt(2 pi))
-__constant__ double kInvSqrt3 = 0.57735026918962576451;        // 1/sqrt(3)
-__constant__ double kLog2e = 1.4426950408889634074;            // 1/ln 2
-__constant__ double kLn2 = 0.69314718055994530942;             // ln 2 (nearest double)
-__constant__ double kLn2Lo = 2.3190468138462995584e-17;        // ln 2 - (double)ln 2
-__constant__ double kSmallT = 0.1;                              // |h| - t below -kSmallT: sum form of eval_W; t_c below it: series for s_l
-__constant__ double kSqrt2 = 1.4142135623730950488;            // sqrt(2)
-__constant__ double kSqrt2m1 = 0.41421356237309504880;         // sqrt(2) - 1
-__constant__ double kSeriesC[5] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0};
-__constant__ double kNinvCut = -1.0651;                         // ln 0.345: domain of the Phi^-1 tail fit
+static __constant__ double kInvSqrt2 = 0.70710678118654752440;       // 1/sqrt(2)
+static __constant__ double kSqrtPiOver2 = 1.2533141373155002512;      // sqrt(pi/2)
+static __constant__ double kSqrt2Pi = 2.5066282746310005024;          // sqrt(2 pi)
+static __constant__ double kPhi0 = 0.39894228040143267794;            // 1/sqrt(2 pi)
+static __constant__ double kLnPhi0 = -0.91893853320467274178;         // ln(1/sqrt(2 pi))
+static __constant__ double kTwoThirdsLnPhi0 = -0.61262568880311516119;  // (2/3) ln(1/sqrt(2 pi))
+static __constant__ double kInvSqrt3 = 0.57735026918962576451;        // 1/sqrt(3)
+static __constant__ double kLog2e = 1.4426950408889634074;            // 1/ln 2
+static __constant__ double kLn2 = 0.69314718055994530942;             // ln 2 (nearest double)
+static __constant__ double kLn2Lo = 2.3190468138462995584e-17;        // ln 2 - (double)ln 2
+static __constant__ double kSmallT = 0.1;                              // |h| - t below -kSmallT: sum form of eval_W; t_c below it: series for s_l
+static __constant__ double kSqrt2 = 1.4142135623730950488;            // sqrt(2)
+static __constant__ double kSqrt2m1 = 0.41421356237309504880;         // sqrt(2) - 1
+static __constant__ double kSeriesC[5] = {1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0};
+static __constant__ double kNinvCut = -1.0651;                         // ln 0.345: domain of the Phi^-1 tail fit
 
 enum : int { KIND_LOWER = 0, KIND_LINEAR = 1, KIND_UPPER = 2 };
 
@@ -666,8 +666,11 @@ struct NormSolve {
 
 // One Householder(3) step.  SEED = true evaluates W, exp and log at seed grade (fp32 erfcx pair, MUFU exp / log,
 // ~1e-6 relative in the step): enough for every step but the last, because the step is fourth order and the last step
-// then takes an iterate that is good to ~1e-6 to ~1e-24.
-template <bool SEED, bool INPLACE>
+// then takes an iterate that is good to ~1e-6 to ~1e-24.  In EVERY step the factors that multiply the residual (the reciprocals
+// inside nu, h2, h3 and the final quotient) use the one-Newton reciprocal (1e-12 relative): the step ds is at most 1e-4 s in the
+// last step, so they enter s at 1e-16; the residual itself (W, exp E, ln W, ln beta) is what carries the full precision.
+// (EXACT_RCP: the all-fp64 tier keeps two-Newton reciprocals everywhere.)
+template <bool SEED, bool INPLACE, bool EXACT_RCP = false>
 __device__ __forceinline__ double householder_step(double x, double s, double p1, double p2, int kind) {
   const WEval w = eval_W<SEED, INPLACE>(x, s);
   const double hr = w.h * w.rs;
@@ -687,22 +690,22 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
     const double L = kLnPhi0 - w.E + (SEED ? log_seed(R) : log_fast(R));  // ln b (lower) or ln(b_max - b) (upper)
     if (want_W) {
       // g = 1/ln b - 1/ln beta  (p1 = ln beta)
-      const double rLW = (SEED ? rcp_nr1(L * R) : rcp_nr2(L * R));
+      const double rLW = EXACT_RCP ? rcp_nr2(L * R) : rcp_nr1(L * R);
       const double lam = rLW * R, ub = rLW * L;  // 1/L, b'/b = 1/W
       const double k2 = fma(2.0, lam, 1.0);
-      nu = (p1 - L) * (L * (SEED ? rcp_nr1(p1) : rcp_nr2(p1))) * R;
+      nu = (p1 - L) * (L * (EXACT_RCP ? rcp_nr2(p1) : rcp_nr1(p1))) * R;
       h2 = fma(-ub, k2, B2);
       h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
     } else {
       // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar  (p1 = ln(b_max - beta))
-      const double gp = SEED ? rcp_nr1(R) : rcp_nr2(R);
+      const double gp = EXACT_RCP ? rcp_nr2(R) : rcp_nr1(R);
       nu = (L - p1) * R;
       h2 = B2 + gp;
       h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
     }
   }
   const double den = fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0);
-  double ds = nu * fma(0.5 * h2, nu, 1.0) * (SEED ? rcp_nr1(den) : rcp_nr2(den));
+  double ds = nu * fma(0.5 * h2, nu, 1.0) * (EXACT_RCP ? rcp_nr2(den) : rcp_nr1(den));
   if (!(ds > -0.5 * s)) ds = -0.5 * s;
   return s + ds;
 }
@@ -710,10 +713,10 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
 template <int NITER, bool FULL, bool INPLACE = false>
 __device__ __forceinline__ NormSolve lbr_refine(double x, double s, double p1, double p2, int kind) {
 #pragma unroll 1
-  for (int it = 0; it < NITER - 1; ++it) s = householder_step<!FULL, INPLACE>(x, s, p1, p2, kind);
+  for (int it = 0; it < NITER - 1; ++it) s = householder_step<!FULL, INPLACE, FULL>(x, s, p1, p2, kind);
   NormSolve o;
   o.s1 = s;
-  s = householder_step<false, INPLACE>(x, s, p1, p2, kind);
+  s = householder_step<false, INPLACE, FULL>(x, s, p1, p2, kind);
   const double rs = rcp_nr2(s);
   const double h = x * rs, t = 0.5 * s;
   o.s = s;
@@ -750,7 +753,7 @@ struct Prelude {
 };
 
 template <bool BSM>
-__device__ __noinline__ Prelude lbr_prelude_exact(double SorF, double K, double tau, double r, double q, double P,
+static __device__ __noinline__ Prelude lbr_prelude_exact(double SorF, double K, double tau, double r, double q, double P,
                                                   double flag) {
   Prelude p;
   bool bad = !pos_fin(SorF) || !pos_fin(K) || !pos_fin(tau) || !is_fin(P) || !(flag == 1.0 || flag == -1.0);
@@ -863,9 +866,8 @@ __device__ __forceinline__ Norm lbr_normalise(double U, double O, double B, bool
   } else {
     n.rootFK = sqrt_nr2(FK, r);
   }
-  double q = lo * r;
-  n.bmax = fma(fma(-n.rootFK, q, lo), r, q);
-  q = tv * r;
+  n.bmax = lo * r;   // seed-grade consumers only (the boundary point and the node of the seed); no residual correction
+  double q = tv * r;
   n.beta = fma(fma(-n.rootFK, q, tv), r, q);
   q = ub * r;
   n.bbar = fma(fma(-n.rootFK, q, ub), r, q);

@@ -29,7 +29,7 @@
 
 namespace pivot {
 
-constexpr int kFwdThreads = 128;
+constexpr int kFwdThreads = 256;
 constexpr int kBwdThreads = 256;
 constexpr int kHouseholderSteps = 2;  // north_star: two Householder(3) steps
 
@@ -45,7 +45,7 @@ struct DiagOut {
 // Best when nearly every row solves and neighbouring rows are alike (option chains in strike order).
 // ---------------------------------------------------------------------------------------------------------------
 template <bool BSM, bool DIAG, bool FULL>
-__global__ void __launch_bounds__(kFwdThreads, (FULL || DIAG) ? 1 : 7)
+__global__ void __launch_bounds__(kFwdThreads, (FULL || DIAG) ? 1 : 4)
 forward_kernel_scalar(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, double* __restrict__ vega,
                       uint8_t* __restrict__ status, DiagOut dg) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -117,7 +117,7 @@ __device__ __forceinline__ unsigned smem_atomic_add(unsigned* addr, unsigned var
 // A row the fast prelude could not classify (status 5): lbr_prelude_exact on its inputs, staged outputs, and its own
 // queue slot (flagged: lbr_normalise then takes the IEEE square root).
 template <bool BSM, bool DIAG, int RPT>
-__device__ __noinline__ void tile_rare_row(pivot_iv_inputs in, int64_t base, int p, TileSmem<RPT>& sm, DiagOut dg) {
+static __device__ __noinline__ void tile_rare_row(pivot_iv_inputs in, int64_t base, int p, TileSmem<RPT>& sm, DiagOut dg) {
   const int64_t i = base + p;
   const double tau = in.tau[i];
   const Prelude pr = lbr_prelude_exact<BSM>(in.S_or_F[i], in.K[i], tau, BSM ? in.r[i] : 0.0, BSM ? in.q[i] : 0.0, in.P[i],
