@@ -86,7 +86,7 @@ __device__ __forceinline__ double rcp_nr2(double x) {  // relative error ~1 ulp
 }
 // a/b to ~1 ulp (b normal, finite, non-zero)
 __device__ __forceinline__ double div_fast(double a, double b) {
-  const double r = rcp_nr2(b);
+  const double r = rcp_nr1(b);   // 1e-12: the residual correction below squares it
   const double q = a * r;
   return fma(fma(-b, q, a), r, q);
 }
@@ -116,7 +116,7 @@ __device__ __forceinline__ double exp_fast(double a) {
 
 // ef ln2 + 2 atanh(num/den), |num/den| <= 0.175
 __device__ __forceinline__ double log_core(double num, double den, double ef) {
-  const double r = rcp_nr2(den);
+  const double r = rcp_nr1(den);   // 1e-12: the residual correction of f below squares it
   const double f0 = num * r;
   const double f = fma(fma(-den, f0, num), r, f0);
   const double w = f * f;
@@ -257,7 +257,9 @@ __device__ __forceinline__ double sqrt_nr2(double v, double& rinv) {
 __device__ __forceinline__ double sqrt_nr2(double v) { double r; return sqrt_nr2(v, r); }
 
 // grade-dependent primitives
-template <bool FULL> __device__ __forceinline__ double g_rcp(double x) { return FULL ? rcp_nr2(x) : rcp_nr1(x); }
+// seed-grade reciprocal: MUFU.RCP64H alone (2^-23 relative, PTX rcp.approx.ftz.f64), no Newton step -- every consumer is a
+// rational-seed quantity that is rounded to fp32 or only has to land the seed within ~1e-3
+template <bool FULL> __device__ __forceinline__ double g_rcp(double x) { return FULL ? rcp_nr2(x) : rcp_raw(x); }
 template <bool FULL> __device__ __forceinline__ double g_exp(double a) { return FULL ? exp_fast(a) : exp_seed(a); }
 template <bool FULL> __device__ __forceinline__ double g_log(double v) { return FULL ? log_fast(v) : log_seed(v); }
 template <bool FULL> __device__ __forceinline__ double g_erfcx(double z) {
@@ -669,7 +671,7 @@ struct NormSolve {
 // then takes an iterate that is good to ~1e-6 to ~1e-24.  In EVERY step the factors that multiply the residual (the reciprocals
 // inside nu, h2, h3 and the final quotient) use the one-Newton reciprocal (1e-12 relative): the step ds is at most 1e-4 s in the
 // last step, so they enter s at 1e-16; the residual itself (W, exp E, ln W, ln beta) is what carries the full precision.
-// (EXACT_RCP: the all-fp64 tier keeps two-Newton reciprocals everywhere.)
+// The seed-grade step takes them from MUFU.RCP64H alone (2^-23).  (EXACT_RCP: the all-fp64 tier keeps two-Newton reciprocals.)
 template <bool SEED, bool INPLACE, bool EXACT_RCP = false>
 __device__ __forceinline__ double householder_step(double x, double s, double p1, double p2, int kind) {
   const WEval w = eval_W<SEED, INPLACE>(x, s);
@@ -690,22 +692,22 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
     const double L = kLnPhi0 - w.E + (SEED ? log_seed(R) : log_fast(R));  // ln b (lower) or ln(b_max - b) (upper)
     if (want_W) {
       // g = 1/ln b - 1/ln beta  (p1 = ln beta)
-      const double rLW = EXACT_RCP ? rcp_nr2(L * R) : rcp_nr1(L * R);
+      const double rLW = EXACT_RCP ? rcp_nr2(L * R) : (SEED ? rcp_raw(L * R) : rcp_nr1(L * R));
       const double lam = rLW * R, ub = rLW * L;  // 1/L, b'/b = 1/W
       const double k2 = fma(2.0, lam, 1.0);
-      nu = (p1 - L) * (L * (EXACT_RCP ? rcp_nr2(p1) : rcp_nr1(p1))) * R;
+      nu = (p1 - L) * (L * (EXACT_RCP ? rcp_nr2(p1) : (SEED ? rcp_raw(p1) : rcp_nr1(p1)))) * R;
       h2 = fma(-ub, k2, B2);
       h3 = fma(ub * ub, fma(6.0 * lam, 1.0 + lam, 2.0), fma(-3.0 * B2 * ub, k2, B3));
     } else {
       // g = ln((b_max - beta)/(b_max - b)):  g' = 1/Wbar  (p1 = ln(b_max - beta))
-      const double gp = EXACT_RCP ? rcp_nr2(R) : rcp_nr1(R);
+      const double gp = EXACT_RCP ? rcp_nr2(R) : (SEED ? rcp_raw(R) : rcp_nr1(R));
       nu = (L - p1) * R;
       h2 = B2 + gp;
       h3 = fma(gp, fma(2.0, gp, 3.0 * B2), B3);
     }
   }
   const double den = fma(nu, fma(h3 * (1.0 / 6.0), nu, h2), 1.0);
-  double ds = nu * fma(0.5 * h2, nu, 1.0) * (EXACT_RCP ? rcp_nr2(den) : rcp_nr1(den));
+  double ds = nu * fma(0.5 * h2, nu, 1.0) * (EXACT_RCP ? rcp_nr2(den) : (SEED ? rcp_raw(den) : rcp_nr1(den)));
   if (!(ds > -0.5 * s)) ds = -0.5 * s;
   return s + ds;
 }
