@@ -675,6 +675,46 @@ struct NormSolve {
 template <bool SEED, bool INPLACE, bool EXACT_RCP = false>
 __device__ __forceinline__ double householder_step(double x, double s, double p1, double p2, int kind) {
   const WEval w = eval_W<SEED, INPLACE>(x, s);
+  if (SEED && !EXACT_RCP) {
+    // Seed-grade step: only the residual nu stays in fp64 (it is a cancelling difference); the third-order correction factor
+    // is assembled in fp32 in SCALED variables n = nu/s, h2 s, h3 s^2, which are O(h^2) = O(1e3) at most for every s:
+    //   ds/s = n (1 + h2s n/2) / (1 + n (h2s + h3s n/6)),  (b2/b1) s = h^2 - s^2/4,  (b3/b1) s^2 = ((b2/b1) s)^2 - 3 h^2 - s^2/4
+    // (b1, b2, b3: first to third derivative of b in s).
+    const float hf = __double2float_rn(w.h), sf = __double2float_rn(s);
+    const float hh = hf * hf, sq = 0.25f * sf * sf;
+    const float b2 = hh - sq;
+    const float b3 = fmaf(b2, b2, fmaf(-3.0f, hh, -sq));
+    double nu;
+    float h2s, h3s;
+    if (kind == KIND_LINEAR) {
+      const double inv_v = kSqrt2Pi * exp_seed(w.E);
+      nu = w.have_W ? fma(p1, inv_v, -w.Wd) : fma(-p2, inv_v, w.Wd);
+      h2s = b2;
+      h3s = b3;
+    } else {
+      const bool want_W = kind == KIND_LOWER;
+      double R = w.Wd;
+      if (want_W != w.have_W) R = fma(exp_fast(0.5 * x) * kSqrt2Pi, exp_fast(w.E), -w.Wd);   // rare
+      const double L = kLnPhi0 - w.E + log_seed(R);
+      const float u = __double2float_rn(s * rcp_raw(R));   // s/W or s/Wbar: O(h^2 + s^2)
+      if (want_W) {
+        const float lam = rcpf(__double2float_rn(L));
+        const float k2 = fmaf(2.0f, lam, 1.0f);
+        nu = (p1 - L) * (L * rcp_raw(p1)) * R;
+        h2s = fmaf(-u, k2, b2);
+        h3s = fmaf(u * u, fmaf(6.0f * lam, 1.0f + lam, 2.0f), fmaf(-3.0f * b2 * u, k2, b3));
+      } else {
+        nu = (L - p1) * R;
+        h2s = b2 + u;
+        h3s = fmaf(u, fmaf(2.0f, u, 3.0f * b2), b3);
+      }
+    }
+    const float n = __double2float_rn(nu * w.rs);
+    const float den = fmaf(n, fmaf(h3s * (1.0f / 6.0f), n, h2s), 1.0f);
+    float f = n * fmaf(0.5f * h2s, n, 1.0f) * rcpf(den);
+    if (!(f > -0.5f)) f = -0.5f;
+    return fma(s, (double)f, s);
+  }
   const double hr = w.h * w.rs;
   const double B2 = fma(w.h, hr, -0.25 * s);                  // second derivative of b over b'
   const double B3 = fma(B2, B2, fma(-3.0 * hr, hr, -0.25));   // third derivative of b over b'
