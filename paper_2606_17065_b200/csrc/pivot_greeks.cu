@@ -14,6 +14,12 @@
 namespace pivot {
 
 constexpr int kEwThreads = 256;
+#ifndef PIVOT_EW_MIN_CTAS
+#define PIVOT_EW_MIN_CTAS 4
+#endif
+#ifndef PIVOT_RT_MIN_CTAS
+#define PIVOT_RT_MIN_CTAS 4
+#endif
 
 // Black price through the OTM-normalised form: P = D (intrinsic + sqrt(FK) b(x, s)), b from the same W / Wbar ratios as
 // the solver (no cancellation for deep in-the-money rows).  sigma == 0 gives the discounted intrinsic value; NaN / negative
@@ -53,7 +59,7 @@ __device__ __forceinline__ void black_row(double SorF, double K, double tau, dou
     const double rl = r * rcp_nr2(bmax), d = hi - lo;
     qq = d * rl;
     const double x = -log1p_fast(fma(fma(-lo, qq, d), rl, qq));
-    const WEval w = eval_W(x, s);
+    const WEval w = eval_W<false, true>(x, s);   // table read in place: these kernels are grid-stride loops
     v = kPhi0 * exp_fast(-w.E);
     b = w.have_W ? w.Wd * v : fma(-w.Wd, v, bmax);
     if (d1d2) *d1d2 = fma(w.h, w.h, -0.25 * s * s);   // d1 d2 = h^2 - t^2 (sign of x does not matter)
@@ -63,7 +69,7 @@ __device__ __forceinline__ void black_row(double SorF, double K, double tau, dou
 }
 
 template <bool BSM>
-__global__ void __launch_bounds__(kEwThreads)
+__global__ void __launch_bounds__(kEwThreads, PIVOT_EW_MIN_CTAS)
 black_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, int64_t n, double* __restrict__ price,
                    double* __restrict__ vega) {
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -174,7 +180,7 @@ __device__ __forceinline__ void block_add3(double a, double b, double c, double*
 // eq.(11): out += { sum (P_model - P*)^2, sum |P*|, rows used };  GRAD: grad[i] = grad_scale 2 (P_model - P*) V_hat
 // (0 for rows the sum skips)
 template <bool BSM, bool GRAD>
-__global__ void __launch_bounds__(kEwThreads)
+__global__ void __launch_bounds__(kEwThreads, PIVOT_EW_MIN_CTAS)
 loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int64_t n, double* __restrict__ out,
                   double* __restrict__ grad, double grad_scale) {
   double s2 = 0.0, s1 = 0.0, cnt = 0.0;
@@ -205,7 +211,7 @@ loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int6
 //   MODE = PIVOT_RT_NAIVE (no gate, no sentinel, no sanitisation): out += { sum (sigma_rt - sigma*)^2, rows, rows };
 //       grad[i] = grad_scale STRICT(2 (sigma_rt - sigma*), V_rt; floor) V_hat -- NaN wherever the inverse channel is singular.
 template <bool BSM, int MODE, bool GRAD>
-__global__ void __launch_bounds__(kEwThreads)
+__global__ void __launch_bounds__(kEwThreads, PIVOT_RT_MIN_CTAS)
 loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, const double* __restrict__ sigma_star,
                       double floor_, int64_t n, double* __restrict__ out, double* __restrict__ grad, double grad_scale) {
   double acc = 0.0, wsum = 0.0, cnt = 0.0;
