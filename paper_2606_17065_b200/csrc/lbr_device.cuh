@@ -943,7 +943,8 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
     const Norm nm = lbr_normalise(p.U, p.O, p.B, rare);
     const Seed sd = lbr_seed<FULL>(nm.qrel, nm.beta, nm.bbar, nm.bmax);
     const NormSolve ns = lbr_refine<NITER, FULL>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
-    const double rinv = rsqrt(tau);
+    double rinv;   // as the tile kernel: MUFU.RSQ64H + Newton for the common rows, the library rsqrt for rare ones
+    if (rare) rinv = rsqrt(tau); else (void)sqrt_nr2(tau, rinv);
     o.sigma = ns.s * rinv;
     o.vega = (BSM ? p.D * nm.rootFK : nm.rootFK) * ns.vfin * (tau * rinv);
     o.zone = (int8_t)sd.zone;

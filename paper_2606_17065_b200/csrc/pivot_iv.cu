@@ -227,8 +227,13 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
       if (dg.s1) dg.s1[base + p] = 0.0;
     }
     qmask |= queued ? (1u << k) : 0u;
-    rmask |= (pr.status == 5 && p < rows) ? (1u << k) : 0u;
+    rmask |= (pr.status == 5) ? (1u << k) : 0u;
     vF[k] = pr.U; vK[k] = pr.O; vP[k] = pr.B;   // what the solver pass needs
+  }
+  if (rows != kTileRows) {   // last tile: dead rows (flag read as 0 -> "rare") are dropped here
+#pragma unroll
+    for (int k = 0; k < RPT; ++k)
+      if (k * kTileThreads + tid >= rows) rmask &= ~(1u << k);
   }
   {
     // Queue slots, warp by warp: within a warp the order is k-major then lane, so that a run of 32 CONSECUTIVE rows stays
@@ -338,7 +343,10 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     const int p = sm.pos[j] & 0x3fff;
     PIVOT_ASSERT(p < rows);
     const double tau = sm.sig[p];
-    const double rinv = rsqrt(tau);
+    // 1/sqrt(tau): MUFU.RSQ64H + Newton for the common rows (tau positive normal, checked by the prelude); a rare row may carry
+    // a subnormal tau and takes the library rsqrt
+    double rinv;
+    if (sm.pos[j] & 0x8000) rinv = rsqrt(tau); else (void)sqrt_nr2(tau, rinv);
     sm.sig[p] = ns.s * rinv;
     sm.veg[p] = sm.veg[p] * ns.vfin * (tau * rinv);
     if (DIAG) {
@@ -349,10 +357,17 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
   __syncthreads();
 
   // ---- phase C
-#pragma unroll 4
-  for (int k = 0; k < RPT; ++k) {
-    const int p = k * kTileThreads + tid;
-    if (p < rows) {
+  if (rows == kTileRows) {   // full tile: no bounds tests, one address per array
+    double* __restrict__ gs = sigma + base + tid;
+    double* __restrict__ gv = vega + base + tid;
+#pragma unroll
+    for (int k = 0; k < RPT; ++k) {
+      __stcs(gs + k * kTileThreads, sm.sig[k * kTileThreads + tid]);
+      __stcs(gv + k * kTileThreads, sm.veg[k * kTileThreads + tid]);
+    }
+  } else {
+#pragma unroll 1
+    for (int p = tid; p < rows; p += kTileThreads) {
       __stcs(sigma + base + p, sm.sig[p]);
       __stcs(vega + base + p, sm.veg[p]);
     }
