@@ -257,7 +257,7 @@ __device__ __forceinline__ double sqrt_nr2(double v, double& rinv) {
 __device__ __forceinline__ double sqrt_nr2(double v) { double r; return sqrt_nr2(v, r); }
 
 // grade-dependent primitives
-// seed-grade reciprocal: MUFU.RCP64H alone (2^-23 relative, PTX rcp.approx.ftz.f64), no Newton step -- every consumer is a
+// seed-grade reciprocal: MUFU.RCP64H alone (9e-7 relative, measured: tests/test_gpu_mathlib.py), no Newton step -- every consumer is a
 // rational-seed quantity that is rounded to fp32 or only has to land the seed within ~1e-3
 template <bool FULL> __device__ __forceinline__ double g_rcp(double x) { return FULL ? rcp_nr2(x) : rcp_raw(x); }
 template <bool FULL> __device__ __forceinline__ double g_exp(double a) { return FULL ? exp_fast(a) : exp_seed(a); }
@@ -671,7 +671,7 @@ struct NormSolve {
 // then takes an iterate that is good to ~1e-6 to ~1e-24.  In EVERY step the factors that multiply the residual (the reciprocals
 // inside nu, h2, h3 and the final quotient) use the one-Newton reciprocal (1e-12 relative): the step ds is at most 1e-4 s in the
 // last step, so they enter s at 1e-16; the residual itself (W, exp E, ln W, ln beta) is what carries the full precision.
-// The seed-grade step takes them from MUFU.RCP64H alone (2^-23).  (EXACT_RCP: the all-fp64 tier keeps two-Newton reciprocals.)
+// The seed-grade step takes them from MUFU.RCP64H alone (9e-7).  (EXACT_RCP: the all-fp64 tier keeps two-Newton reciprocals.)
 template <bool SEED, bool INPLACE, bool EXACT_RCP = false>
 __device__ __forceinline__ double householder_step(double x, double s, double p1, double p2, int kind) {
   const WEval w = eval_W<SEED, INPLACE>(x, s);

@@ -180,6 +180,7 @@ def test_reciprocal_division_sqrt():
     x = np.concatenate([_lu(rng, 1e-300, 1e300, 3000), -_lu(rng, 1e-300, 1e300, 500), [1.0, 3.0, 2.0 ** -1000, 2.0 ** 1000]])
     ref = [1 / mp.mpf(float(v)) for v in x]
     e1, e2 = _relerr(_run("rcp_nr1", x), ref), _relerr(_run("rcp_nr2", x), ref)
+    e0 = _relerr(_run("rcp_raw", x), ref)
     a = rng.standard_normal(3504) * _lu(rng, 1e-100, 1e100, 3504)
     xb = np.sign(x) * np.exp(np.log(np.abs(x)) * 0.5)          # 1e-150 .. 1e150: the quotient stays in the normal range
     ed = _relerr(_run("div_fast", a, xb), [mp.mpf(float(p)) / mp.mpf(float(q)) for p, q in zip(a, xb)])
@@ -188,8 +189,8 @@ def test_reciprocal_division_sqrt():
     es1, es2 = _relerr(_run("sqrt_nr1", v), rs), _relerr(_run("sqrt_nr2", v), rs)
     er = _relerr(_run("rsqrt_nr2", v), [1 / t for t in rs])
     assert _run("sqrt_nr1", np.array([0.0]))[0] == 0.0
-    print(f"rcp_nr1 {e1:.2e} rcp_nr2 {e2:.2e} div_fast {ed:.2e} sqrt_nr1 {es1:.2e} sqrt_nr2 {es2:.2e} rsqrt_nr2 {er:.2e}")
-    assert e1 <= 1e-11 and e2 <= 2 * EPS and ed <= 1.5 * EPS
+    print(f"rcp_raw {e0:.2e} rcp_nr1 {e1:.2e} rcp_nr2 {e2:.2e} div_fast {ed:.2e} sqrt_nr1 {es1:.2e} sqrt_nr2 {es2:.2e} rsqrt_nr2 {er:.2e}")
+    assert e0 <= 2.0 ** -19 and e1 <= 1e-11 and e2 <= 2 * EPS and ed <= 1.5 * EPS
     assert es1 <= 1e-11 and es2 <= 1.5 * EPS and er <= 4 * EPS
 
 
