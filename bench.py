@@ -487,6 +487,28 @@ def main():
         e2e["label_pipeline"] = dict(best, batches=64, batch_rows=65536, h2d_bytes=40 * nl, d2h_bytes=17 * nl,
                                      paper_h100_labels_per_s=48.9e6, sharded_over_ranks=world,
                                      note="config-0 rows, pinned host buffers, one array sharded by shard_rows")
+        # The same 64 x 65,536-row batches already RESIDENT on the device (launch-latency regime: one batch is a 16 us kernel):
+        # 64 forward calls enqueued one by one, and the same 64 launches replayed from ONE CUDA graph.
+        if rank == 0:
+            lab_a = [lab[k] for k in KEYS]
+            lab_o = _alloc_out(nl)
+            bs = 65536
+
+            def batches():
+                for b_ in range(64):
+                    sl = slice(b_ * bs, (b_ + 1) * bs)
+                    pv.pivot_iv_forward(*[t[sl] for t in lab_a], out=tuple(t[sl] for t in lab_o))
+            batches(); torch.cuda.synchronize()
+            ms_calls = _time_calls(batches, torch.cuda.current_stream(), 5, warm=1)
+            side = torch.cuda.Stream()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                batches()
+            ms_graph = _time_calls(g.replay, torch.cuda.current_stream(), 20, warm=2)
+            e2e["device_batches"] = {"batches": 64, "batch_rows": bs, "ms_64_calls": ms_calls, "ms_graph_replay": ms_graph,
+                                     "labels_per_s_graph": nl / (ms_graph * 1e-3), "us_per_batch_graph": ms_graph * 1e3 / 64,
+                                     "note": "inputs resident in HBM; forward only; one CUDA graph of 64 launches vs 64 calls"}
+            del lab_o, g
         del lab, lh, lo
 
     # --- zone mix of this workload (diagnostic kernel variant; not timed)

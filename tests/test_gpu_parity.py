@@ -480,3 +480,31 @@ def test_rows_at_zone_edges_meet_the_bar():
     assert (st.cpu().numpy() == 0).all()
 
 
+
+
+def test_forward_backward_replay_from_a_cuda_graph():
+    """The two calls of the hot path are plain stream-ordered launches (no allocation, no synchronisation, no host read): a
+    label-generation batch loop captured once in a CUDA graph replays with the same bits (the launch-latency regime of the
+    paper's 65,536-row batches)."""
+    nb, rows = 8, 65_536
+    cfg = wl.config0(nb * rows, seed=11)
+    d = to_device(cfg)
+    a = [d[k] for k in KEYS]
+    gs = torch.ones(nb * rows, dtype=torch.float64, device="cuda")
+    ref = pv.pivot_iv_forward(*a)
+    ref_g = pv.pivot_iv_backward(gs, ref[1], ref[2], 1e-8, pv.GATE_MASK)
+    out = tuple(torch.zeros_like(t) for t in ref)
+    gP = torch.zeros_like(ref_g)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        for b in range(nb):
+            sl = slice(b * rows, (b + 1) * rows)
+            o = tuple(t[sl] for t in out)
+            pv.pivot_iv_forward(*[t[sl] for t in a], out=o)
+            pv.pivot_iv_backward(gs[sl], o[1], o[2], 1e-8, pv.GATE_MASK, out=gP[sl])
+    for _ in range(2):
+        graph.replay()
+    torch.cuda.synchronize()
+    for x, y in zip(out + (gP,), ref + (ref_g,)):
+        assert torch.equal(x.view(torch.int64) if x.dtype == torch.float64 else x, y.view(torch.int64) if y.dtype == torch.float64 else y)
