@@ -44,7 +44,8 @@ extern "C" {
 #define PIVOT_ST_BELOW_INTRINSIC 1 /* undiscounted price < max(theta (F-K), 0)        -> sigma = NaN, vega = 0 */
 #define PIVOT_ST_ABOVE_MAX 2       /* undiscounted price >= F (call) or >= K (put)     -> sigma = NaN, vega = 0 */
 #define PIVOT_ST_BAD_INPUT 3       /* tau <= 0, non-finite or non-positive S|F, K, non-finite P, r, q, flag not +-1,
-                                      or |ln(F/K)| > 693                               -> sigma = NaN, vega = 0 */
+                                      or |ln(F/K)| > 693, or F K overflows / underflows in fp64 (sqrt(F K) must be a
+                                      positive normal number: e.g. F = K = 2e154 is rejected) -> sigma = NaN, vega = 0 */
 #define PIVOT_ST_AT_INTRINSIC 4    /* time value is zero or subnormal after normalisation -> sigma = +0, vega = 0 */
 
 /* gate modes of the backward pass (eq.(9), :148-150 eq.(10)) */
