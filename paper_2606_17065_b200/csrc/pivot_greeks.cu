@@ -92,35 +92,71 @@ __device__ __forceinline__ void Phi_pair(double z1, double z2, double& P1, doubl
   P2 = (z2 < 0.0) ? t2 : 1.0 - t2;
 }
 
+// Each warp walks blocks of 128 consecutive rows.  Pass 1 (all rows, coalesced): the gated common factor c = grad_P (exactly
+// pivot_iv_backward's arithmetic) and the outputs of the rows that need no Greeks; the rows that do (OK, on the gate, c != 0:
+// 26 % of config 4, scattered) are appended to a per-warp list in shared memory.  Pass 2 (dense over that list): the analytic
+// Greeks, one listed row per lane -- in one pass they ran at ~8 of 32 lanes.
 template <bool BSM, int MODE>
 __global__ void __launch_bounds__(kEwThreads)
 backward_inputs_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, const double* __restrict__ vega,
                        const uint8_t* __restrict__ status, const double* __restrict__ gs, double floor_, int64_t n,
                        double* __restrict__ gP, double* __restrict__ gS, double* __restrict__ gK, double* __restrict__ gT,
                        double* __restrict__ gR, double* __restrict__ gQ) {
+  constexpr int kBlockRows = 128, kWarps = kEwThreads / 32;
+  __shared__ double c_list[kWarps][kBlockRows];
+  __shared__ uint8_t i_list[kWarps][kBlockRows];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const double floor2 = __dmul_rn(floor_, floor_);
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double V = __ldcs(vega + i), g = __ldcs(gs + i);
-    const uint8_t st = status[i];
-    // the gated common factor: exactly pivot_iv_backward's grad_P
-    double c;
-    bool strict_off = false;
-    if (MODE == PIVOT_GATE_MASK) {
-      c = ((st == PIVOT_ST_OK) && (fabs(V) > floor_)) ? __ddiv_rn(g, V) : 0.0;
-    } else if (MODE == PIVOT_GATE_STRICT) {
-      const bool on = (st == PIVOT_ST_OK) && (fabs(V) > floor_);
-      c = on ? __ddiv_rn(g, V) : ((g == 0.0) ? 0.0 : canonical_nan());
-      strict_off = !on;
-    } else {
-      const double den = __dadd_rn(__dmul_rn(V, V), floor2);
-      c = ((st == PIVOT_ST_OK) && (den > 0.0)) ? __ddiv_rn(__dmul_rn(g, V), den) : 0.0;
+  const int64_t nblocks = (n + kBlockRows - 1) / kBlockRows;
+  const int64_t wstride = (int64_t)gridDim.x * kWarps;
+  for (int64_t blk = (int64_t)blockIdx.x * kWarps + warp; blk < nblocks; blk += wstride) {
+    const int64_t base = blk * kBlockRows;
+    int count = 0;
+#pragma unroll
+    for (int k = 0; k < kBlockRows / 32; ++k) {
+      const int64_t i = base + k * 32 + lane;
+      bool heavy = false;
+      double c = 0.0;
+      if (i < n) {
+        const double V = __ldcs(vega + i), g = __ldcs(gs + i);
+        const uint8_t st = status[i];
+        bool strict_off = false;
+        if (MODE == PIVOT_GATE_MASK) {
+          c = ((st == PIVOT_ST_OK) && (fabs(V) > floor_)) ? __ddiv_rn(g, V) : 0.0;
+        } else if (MODE == PIVOT_GATE_STRICT) {
+          const bool on = (st == PIVOT_ST_OK) && (fabs(V) > floor_);
+          c = on ? __ddiv_rn(g, V) : ((g == 0.0) ? 0.0 : canonical_nan());
+          strict_off = !on;
+        } else {
+          const double den = __dadd_rn(__dmul_rn(V, V), floor2);
+          c = ((st == PIVOT_ST_OK) && (den > 0.0)) ? __ddiv_rn(__dmul_rn(g, V), den) : 0.0;
+        }
+        heavy = !strict_off && st == PIVOT_ST_OK && c != 0.0;
+        __stcs(gP + i, c);
+        if (!heavy) {
+          const double z = strict_off ? c : 0.0;   // 0, or NaN with grad_P under the strict contract
+          __stcs(gS + i, z);
+          __stcs(gK + i, z);
+          __stcs(gT + i, z);
+          if (BSM) {
+            __stcs(gR + i, z);
+            __stcs(gQ + i, z);
+          }
+        }
+      }
+      const unsigned m = __ballot_sync(0xffffffffu, heavy);
+      if (heavy) {
+        const int e = count + __popc(m & ((1u << lane) - 1u));
+        c_list[warp][e] = c;
+        i_list[warp][e] = (uint8_t)(k * 32 + lane);
+      }
+      count += __popc(m);
     }
-    double dS = 0.0, dK = 0.0, dT = 0.0, dR = 0.0, dQ = 0.0;
-    if (strict_off) {
-      dS = dK = dT = c;                 // 0 or NaN with grad_P
-      dR = dQ = c;
-    } else if (st == PIVOT_ST_OK && c != 0.0) {
+    __syncwarp();
+    for (int e = lane; e < count; e += 32) {
+      const int64_t i = base + i_list[warp][e];
+      const double c = c_list[warp][e];
+      const double V = __ldcs(vega + i);
       const double S = __ldcs(in.S_or_F + i), K = __ldcs(in.K + i), tau = __ldcs(in.tau + i), sg = __ldcs(sigma + i);
       const double th = (__ldcs(in.flag + i) > 0.0) ? 1.0 : -1.0;
       const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
@@ -131,20 +167,15 @@ backward_inputs_kernel(pivot_iv_inputs in, const double* __restrict__ sigma, con
       Phi_pair(th * d1, th * d2, N1, N2);
       const double Dq = BSM ? exp_fast(-q * tau) : 1.0, Dr = BSM ? exp_fast(-r * tau) : 1.0;
       const double a1 = th * Dq * N1, a2 = th * Dr * N2;   // dP/dS, -dP/dK
-      dS = -c * a1;
-      dK = c * a2;
-      dT = -c * (fma(-q * S, a1, r * K * a2) + V * sg / (2.0 * tau));
-      dR = -c * (K * tau * a2);
-      dQ = c * (S * tau * a1);
+      __stcs(gS + i, -c * a1);
+      __stcs(gK + i, c * a2);
+      __stcs(gT + i, -c * (fma(-q * S, a1, r * K * a2) + V * sg / (2.0 * tau)));
+      if (BSM) {
+        __stcs(gR + i, -c * (K * tau * a2));
+        __stcs(gQ + i, c * (S * tau * a1));
+      }
     }
-    __stcs(gP + i, c);
-    __stcs(gS + i, dS);
-    __stcs(gK + i, dK);
-    __stcs(gT + i, dT);
-    if (BSM) {
-      __stcs(gR + i, dR);
-      __stcs(gQ + i, dQ);
-    }
+    __syncwarp();
   }
 }
 
