@@ -119,41 +119,73 @@ def _stream_ptr(stream) -> int:
     return int(stream.cuda_stream)
 
 
+class _NoGuard:
+    def __enter__(self):
+        return None
+
+    def __exit__(self, *a):
+        return False
+
+
+_NOGUARD = _NoGuard()
+
+
+def _guard(device):
+    """Device guard around a launch; skipped (it costs several microseconds per call) when `device` is already current."""
+    idx = device.index
+    if idx is None or idx == torch.cuda.current_device():
+        return _NOGUARD
+    return torch.cuda.device(device)
+
+
 def _require_cuda():
     if not torch.cuda.is_available():
         raise PivotError("no CUDA device: the PIVOT path runs only on the GPU (no CPU fallback)")
 
 
+_F64, _U8 = torch.float64, torch.uint8
+
+
+def _ptr(t, name, n, dev, dtype=_F64):
+    """data_ptr() of a contiguous 1-D CUDA tensor of `dtype` with n elements on `dev` (one pass: this sits on the per-call path)."""
+    if not isinstance(t, torch.Tensor):
+        raise PivotError(f"{name}: expected a contiguous 1-D CUDA tensor of {dtype}")
+    if t.dtype is not dtype or t.device != dev or t.dim() != 1 or t.shape[0] != n or not t.is_contiguous():
+        if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.dim() == 1):
+            raise PivotError(f"{name}: expected a contiguous 1-D CUDA tensor of {dtype}")
+        if t.numel() != n:
+            raise PivotError(f"{name}: length {t.numel()} != {n}")
+        raise PivotError(f"{name}: on {t.device}, expected {dev}")
+    return t.data_ptr()
+
+
 def _forward(SorF, K, tau, P, flag, r, q, out, stream, zones, kernel=None):
     _require_cuda()
     lib = load_library()
-    n = SorF.numel()
-    _same_len(n, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
-    _same_device(SorF, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
-    if out is not None:
-        _same_len(n, **{f"out[{i}]": t for i, t in enumerate(out)})
-        _same_device(SorF, **{f"out[{i}]": t for i, t in enumerate(out)})
-    inp = _Inputs(_dev(SorF, "S_or_F"), _dev(K, "K"), _dev(tau, "tau"), _dev(r, "r"), _dev(q, "q"), _dev(P, "P"),
-                  _dev(flag, "flag"))
+    if not (isinstance(SorF, torch.Tensor) and SorF.is_cuda and SorF.dim() == 1):
+        raise PivotError("S_or_F: expected a contiguous 1-D CUDA tensor of torch.float64")
+    n = SorF.shape[0]
+    dev = SorF.device
+    inp = _Inputs(_ptr(SorF, "S_or_F", n, dev), _ptr(K, "K", n, dev), _ptr(tau, "tau", n, dev),
+                  None if r is None else _ptr(r, "r", n, dev), None if q is None else _ptr(q, "q", n, dev),
+                  _ptr(P, "P", n, dev), _ptr(flag, "flag", n, dev))
     if out is None:
-        sigma = torch.empty(n, dtype=torch.float64, device=SorF.device)
-        vega = torch.empty(n, dtype=torch.float64, device=SorF.device)
-        status = torch.empty(n, dtype=torch.uint8, device=SorF.device)
+        sigma = torch.empty(n, dtype=_F64, device=dev)
+        vega = torch.empty(n, dtype=_F64, device=dev)
+        status = torch.empty(n, dtype=_U8, device=dev)
     else:
         sigma, vega, status = out[:3]
+    ps, pv_, pst = _ptr(sigma, "out[0]", n, dev), _ptr(vega, "out[1]", n, dev), _ptr(status, "out[2]", n, dev, _U8)
     sp = _stream_ptr(stream)
-    with torch.cuda.device(SorF.device):
+    with _guard(dev):
         if zones:
-            zone = torch.empty(n, dtype=torch.int8, device=SorF.device) if out is None or len(out) < 4 else out[3]
-            _check(lib.pivot_iv_forward_zones(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
-                                              _dev(status, "status", torch.uint8), _dev(zone, "zone", torch.int8), sp))
+            zone = torch.empty(n, dtype=torch.int8, device=dev) if out is None or len(out) < 4 else out[3]
+            _check(lib.pivot_iv_forward_zones(C.byref(inp), n, ps, pv_, pst, _ptr(zone, "out[3]", n, dev, torch.int8), sp))
             return sigma, vega, status, zone
         if kernel is not None:
-            _check(lib.pivot_iv_forward_ex(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
-                                           _dev(status, "status", torch.uint8), int(kernel), sp))
+            _check(lib.pivot_iv_forward_ex(C.byref(inp), n, ps, pv_, pst, int(kernel), sp))
         else:
-            _check(lib.pivot_iv_forward(C.byref(inp), n, _dev(sigma, "sigma"), _dev(vega, "vega"),
-                                        _dev(status, "status", torch.uint8), sp))
+            _check(lib.pivot_iv_forward(C.byref(inp), n, ps, pv_, pst, sp))
     return sigma, vega, status
 
 
@@ -200,7 +232,7 @@ def pivot_iv_debug_math(fn: str, a: torch.Tensor, b: Optional[torch.Tensor] = No
     n = a.numel()
     _same_len(n, b=b)
     out = torch.empty_like(a)
-    with torch.cuda.device(a.device):
+    with _guard(a.device):
         _check(load_library().pivot_iv_debug_math(DBG[fn], _dev(a, "a"), _dev(b, "b"), n, _dev(out, "out"),
                                                   _stream_ptr(stream)))
     return out
@@ -219,7 +251,7 @@ def pivot_iv_backward(grad_sigma, vega, status, vega_floor: float, mode: int, ou
     _same_len(n, vega=vega, status=status, out=out)
     _same_device(grad_sigma, vega=vega, status=status, out=out)
     gP = torch.empty_like(grad_sigma) if out is None else out
-    with torch.cuda.device(grad_sigma.device):
+    with _guard(grad_sigma.device):
         _check(lib.pivot_iv_backward(_dev(grad_sigma, "grad_sigma"), _dev(vega, "vega"),
                                      _dev(status, "status", torch.uint8), float(vega_floor), int(mode), n,
                                      _dev(gP, "grad_P"), _stream_ptr(stream)))
@@ -237,7 +269,7 @@ def pivot_iv_black_price(S_or_F, K, tau, sigma, flag, r=None, q=None, with_vega=
                   _dev(flag, "flag"))
     price = torch.empty(n, dtype=torch.float64, device=S_or_F.device)
     vega = torch.empty(n, dtype=torch.float64, device=S_or_F.device) if with_vega else None
-    with torch.cuda.device(S_or_F.device):
+    with _guard(S_or_F.device):
         _check(lib.pivot_iv_black_price(C.byref(inp), _dev(sigma, "sigma"), n, _dev(price, "price"), _dev(vega, "vega"),
                                      _stream_ptr(stream)))
     return price, vega
@@ -256,7 +288,7 @@ def pivot_iv_backward_inputs(S_or_F, K, tau, flag, sigma, vega, status, grad_sig
                   _dev(flag, "flag"))
     outs = [torch.empty(n, dtype=torch.float64, device=S_or_F.device) for _ in range(4)]
     outs += [torch.empty(n, dtype=torch.float64, device=S_or_F.device) if r is not None else None for _ in range(2)]
-    with torch.cuda.device(S_or_F.device):
+    with _guard(S_or_F.device):
         _check(lib.pivot_iv_backward_inputs(C.byref(inp), _dev(sigma, "sigma"), _dev(vega, "vega"),
                                             _dev(status, "status", torch.uint8), _dev(grad_sigma, "grad_sigma"),
                                             float(vega_floor), int(mode), n, *[_dev(o, "grad") for o in outs],
@@ -281,7 +313,7 @@ def pivot_iv_loss_price(S_or_F, K, tau, P_star, flag, sigma_hat, r=None, q=None,
                   _dev(flag, "flag"))
     out = torch.zeros(3, dtype=torch.float64, device=S_or_F.device)
     grad = torch.empty(n, dtype=torch.float64, device=S_or_F.device) if grad_scale is not None else None
-    with torch.cuda.device(S_or_F.device):
+    with _guard(S_or_F.device):
         _check(lib.pivot_iv_loss_price(C.byref(inp), _dev(sigma_hat, "sigma_hat"), n, _dev(out, "out"), _dev(grad, "grad"),
                                        float(grad_scale or 0.0), _stream_ptr(stream)))
     return out if grad is None else (out, grad)
@@ -300,7 +332,7 @@ def pivot_iv_loss_roundtrip(S_or_F, K, tau, P_star, flag, sigma_hat, sigma_star,
                   _dev(flag, "flag"))
     out = torch.zeros(3, dtype=torch.float64, device=S_or_F.device)
     grad = torch.empty(n, dtype=torch.float64, device=S_or_F.device) if grad_scale is not None else None
-    with torch.cuda.device(S_or_F.device):
+    with _guard(S_or_F.device):
         _check(lib.pivot_iv_loss_roundtrip(C.byref(inp), _dev(sigma_hat, "sigma_hat"), _dev(sigma_star, "sigma_star"),
                                            float(vega_floor), int(mode), n, _dev(out, "out"), _dev(grad, "grad"),
                                            float(grad_scale or 0.0), _stream_ptr(stream)))
