@@ -67,14 +67,14 @@ forward_kernel_scalar(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma,
 // Forward kernel, "tile compaction".  A CTA owns a tile of kTileRows consecutive rows.
 //   Phase A  (all rows, coalesced 8-byte loads): lbr_prelude -> status, decided on the high words and five exact
 //            subtractions / comparisons; no square root, no division.  Rows that need the solver are appended to a
-//            compact queue (U, O, B) in shared memory (one warp prefix scan and one shared atomic per warp per tile);
-//            the others get their final sigma / vega straight away.  For queued rows the staged sigma slot carries tau
-//            meanwhile (and the vega slot the discount factor in BSM mode).
+//            compact queue (U, O, B) in shared memory (RPT ballots and one shared atomic per warp per tile; slots in row
+//            order within the warp); the others get their final sigma / vega straight away.  For queued rows the staged sigma
+//            slot carries tau meanwhile (and the vega slot the discount factor in BSM mode).
 //   Phase B1 (queued rows, DENSE warps): lbr_normalise (sqrt(FK) and the four quotients) + lbr_seed_head: x, boundary
-//            point, node, zone; the middle zones get their seed here; rows are regrouped by zone class (warp ballots +
-//            one packed shared counter).
-//   Phase B2 (queued rows, grouped zone 0 / middle / zone 3): the tail seeds (lbr_seed_tail0 / _tail3) fused with the
-//            two Householder(3) steps (lbr_refine); sigma and vega into the staged output slots of the row.
+//            point, node, zone, and four handover words per row (tails: the node; middle zones: the three fp32 parameters
+//            of their rational cubic); rows are regrouped by zone class (warp ballots + two shared counters).
+//   Phase B2 (queued rows, grouped zone 0 / middle / zone 3): the seed of the row's zone (lbr_seed_tail0 / _mid / _tail3)
+//            fused with the two Householder(3) steps (lbr_refine); sigma and vega into the staged output slots of the row.
 //   Phase C: the staged sigma, vega and status of the tile are streamed out with coalesced stores.
 // Every row still touches HBM exactly once (57 B Black-76, 73 B BSM); both partitions cost shared-memory traffic only.
 // ---------------------------------------------------------------------------------------------------------------
@@ -95,7 +95,7 @@ struct TileSmem {
   double q2[kTileRows];
   double q3[kTileRows];
   uint16_t pos[kTileRows];    // tile position of the queued row; bit 15 = rare row (exact prelude, IEEE square root)
-  uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, finished middle-zone rows from the back
+  uint16_t perm[kTileRows];   // queue indices: zone 0 rows from the front, middle-zone rows from the back
   uint16_t permU[kTileRows];  // ... and zone 3 rows
   uint8_t status[kTileRows];
   unsigned n01;               // rows per class: zone 0 | zones 1-2 << 16  (one native 32-bit shared atomic per warp)
