@@ -928,7 +928,7 @@ struct RowOut {
 };
 
 // Full row (Alg.1 l.1-3).  BSM = true: (S,K,tau,r,q,P,flag); false: Black-76 with discount factor 1.
-template <bool BSM, int NITER, bool FULL>
+template <bool BSM, int NITER, bool FULL, bool INPLACE = false>
 __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, double r, double q, double P, double flag) {
   RowOut o;
   Prelude p = lbr_prelude<BSM>(SorF, K, tau, r, q, P, flag);
@@ -942,7 +942,7 @@ __device__ __forceinline__ RowOut lbr_row(double SorF, double K, double tau, dou
   if (p.status == 0) {
     const Norm nm = lbr_normalise(p.U, p.O, p.B, rare);
     const Seed sd = lbr_seed<FULL>(nm.qrel, nm.beta, nm.bbar, nm.bmax);
-    const NormSolve ns = lbr_refine<NITER, FULL>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
+    const NormSolve ns = lbr_refine<NITER, FULL, INPLACE>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
     double rinv;   // as the tile kernel: MUFU.RSQ64H + Newton for the common rows, the library rsqrt for rare ones
     if (rare) rinv = rsqrt(tau); else (void)sqrt_nr2(tau, rinv);
     o.sigma = ns.s * rinv;

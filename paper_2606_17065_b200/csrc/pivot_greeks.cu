@@ -260,7 +260,7 @@ loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, 
       if (!usable) {
         acc += canonical_nan(); cnt += 1.0; g = canonical_nan();
       } else {
-        const RowOut o = lbr_row<BSM, 2, false>(S, K, tau, r, q, pm, flag);
+        const RowOut o = lbr_row<BSM, 2, false, true>(S, K, tau, r, q, pm, flag);
         const double d = o.sigma - ss;
         acc = fma(d, d, acc); cnt += 1.0;
         const double up = 2.0 * d;
@@ -270,7 +270,7 @@ loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, 
       wsum = cnt;
     } else if (usable) {
       const bool on = fabs(vh) > floor_;
-      const RowOut o = lbr_row<BSM, 2, false>(S, K, tau, r, q, on ? pm : __ldcs(in.P + i), flag);
+      const RowOut o = lbr_row<BSM, 2, false, true>(S, K, tau, r, q, on ? pm : __ldcs(in.P + i), flag);
       if (o.status == PIVOT_ST_OK) {
         const double v2 = vh * vh, den = v2 + f2;
         const double w = v2 / den;
