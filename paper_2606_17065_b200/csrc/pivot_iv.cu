@@ -83,7 +83,7 @@ constexpr int kTileThreads = 256;
 #define PIVOT_PREFETCH_DIST 222
 #endif
 // RPT rows per thread: 4 (1024-row tiles, 55 KB of shared memory, 4 CTAs per SM at 64 registers, both modes) for large n;
-// 1 (256-row tiles) for small n, so that a launch of 65,536 rows still spreads over every SM.
+// 2 (512-row tiles) up to 2^20 rows and 1 (256-row tiles) up to 2^17, so that a small launch still spreads over every SM.
 
 template <int RPT>
 struct TileSmem {
@@ -515,9 +515,14 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
   if (rowwise) {
     const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
     forward_kernel_scalar<BSM, DIAG, FULL><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, n, sigma, vega, status, dg);
-  } else if (!DIAG && !FULL && n <= ((int64_t)1 << 19)) {
-    // small launches use 256-row tiles so that the grid still covers the chip (n <= 2^19: at most 2048 CTAs)
+  } else if (!DIAG && !FULL && n <= ((int64_t)1 << 17)) {
+    // small launches use smaller tiles so that the grid still covers the chip and no SM is left with one long CTA:
+    // 256-row tiles up to 2^17 rows, 512-row tiles up to 2^20 (kernel time from a CUDA graph, mixed / 1-solve rows, in us:
+    // 2^18: 256-row 12.8 / 15.6, 512-row 10.5 / 17.0, 1024-row 11.9 / 18.6;  2^19: 22.8 / 28.0, 16.7 / 27.0, 18.4 / 31.3;
+    // 2^20: 41.5 / 53.1, 29.9 / 50.0, 30.0 / 51.1)
     rc = launch_tile<BSM, false, 1, false>(in, n, sigma, vega, status, dg, st);
+  } else if (!DIAG && !FULL && n <= ((int64_t)1 << 20)) {
+    rc = launch_tile<BSM, false, 2, false>(in, n, sigma, vega, status, dg, st);
   } else {
     rc = launch_tile<BSM, DIAG, 4, FULL>(in, n, sigma, vega, status, dg, st);
   }

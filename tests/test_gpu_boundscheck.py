@@ -43,10 +43,11 @@ def _run(chk, d, n=None):
 
 def test_bounds_checked_build_on_ragged_edge_and_dense_tiles(chk):
     dev = lambda c: {k: (v.cuda() if isinstance(v, torch.Tensor) else v) for k, v in c.items()}
-    mixed = dev(wl.config1((1 << 19) + 1029, seed=3))
-    for n in (1, 2, 31, 255, 256, 257, 1023, 1025, 65_537, (1 << 19) - 3, (1 << 19) + 1029):   # both tile sizes, ragged tails
+    mixed = dev(wl.config1((1 << 20) + 1029, seed=3))
+    for n in (1, 2, 31, 255, 256, 257, 1023, 1025, 65_537, (1 << 17) + 1, (1 << 19) - 3, (1 << 20) + 1029):   # all three tile sizes, ragged tails
         _run(chk, mixed, n)
-    _run(chk, dev(wl.config1(600_000, seed=4, solve_only=True)))          # every row queued: full queues
+    _run(chk, dev(wl.config1(600_000, seed=4, solve_only=True)))          # every row queued: full queues (512-row tiles)
+    _run(chk, dev(wl.config1(1_200_000, seed=6, solve_only=True)))        # ... 1024-row tiles
     _run(chk, dev(wl.config2(days=40, seed=5)))                           # BSM chains, 640,000 rows
     _run(chk, dev(wl.config2(days=1, expiries=3, strikes=77)))            # BSM, small tiles
     # tiles made of rows the fast prelude cannot classify (huge / tiny F, K: every row takes the exact prelude and its own

@@ -348,18 +348,22 @@ def _bits(t):
 
 
 def test_kernel_variants_agree_bit_for_bit():
-    """The 256-row-tile kernel (n <= 2^19), the 1024-row-tile kernel (n > 2^19) and the one-row-per-thread organisation
-    (pivot_iv_forward_ex, PIVOT_FWD_ROWWISE) run the same per-row arithmetic: identical bits on the same rows."""
-    n_big = (1 << 19) + 1029
+    """The 256-row-tile kernel (n <= 2^17), the 512-row-tile kernel (n <= 2^20), the 1024-row-tile kernel (n > 2^20) and the
+    one-row-per-thread organisation (pivot_iv_forward_ex, PIVOT_FWD_ROWWISE) run the same per-row arithmetic: identical bits on
+    the same rows."""
+    n_big = (1 << 20) + 1029
     cfg = wl.config1(n_big, seed=77)
     d = to_device(cfg)
     a = [d[k] for k in KEYS]
     big = pv.pivot_iv_forward(*a)                                          # 1024-row tiles
     m = (1 << 19) - 3
-    small = pv.pivot_iv_forward(*[t[:m] for t in a])                       # 256-row tiles
+    mid = pv.pivot_iv_forward(*[t[:m] for t in a])                         # 512-row tiles
+    m1 = (1 << 17) - 5
+    small = pv.pivot_iv_forward(*[t[:m1] for t in a])                      # 256-row tiles
     rw = pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE)                        # one row per thread
-    for x, y, z in zip(big, small, rw):
+    for x, y, y1, z in zip(big, mid, small, rw):
         assert np.array_equal(_bits(x[:m]), _bits(y))
+        assert np.array_equal(_bits(x[:m1]), _bits(y1))
         assert np.array_equal(_bits(x), _bits(z))
 
 
