@@ -203,7 +203,7 @@ def main():
     print(f"erfcx fp64: C={C64} N={N64} z >= {ZMIN}: max rel err (fp64 Horner, no FMA) = {e64:.3e}; Q - (1-y)Q' truncation = {b64:.3e}")
     print(f"erfcx fp32: C={C32} N={N32} z >= {ZMIN}: max rel err (fp32 Horner) = {e32:.3e}; Q - (1-y)Q' truncation = {b32:.3e}")
     print(f"ninv tail : deg 7 in w=1/(1+u), max rel err = {en:.3e}")
-    NEXP, NATH = 11, 8
+    NEXP, NATH = 11, 6
     aexp, eexp = fit_exp(NEXP)
     FMAX = (mp.sqrt(2) - 1) / (mp.sqrt(2) + 1) * mp.mpf("1.02")
     aath, eath = fit_atanh(NATH, FMAX)
