@@ -79,10 +79,12 @@ __device__ __forceinline__ double rcp_nr1(double x) {  // relative error ~1e-12:
   r = fma(r, fma(-x, r, 1.0), r);
   return r;
 }
-__device__ __forceinline__ double rcp_nr2(double x) {  // relative error ~1 ulp
-  double r = rcp_nr1(x);
-  r = fma(r, fma(-x, r, 1.0), r);
-  return r;
+// relative error ~1 ulp: ONE third-order step from the MUFU value r0 (9e-7):  e = 1 - x r0,  1/x = r0 (1 + e + e^2) (1 + O(e^3)).
+// Three dependent fp64 instructions (two Newton steps take four).
+__device__ __forceinline__ double rcp_nr2(double x) {
+  const double r0 = rcp_raw(x);
+  const double e = fma(-x, r0, 1.0);
+  return fma(r0, fma(e, e, e), r0);
 }
 // a/b to ~1 ulp (b normal, finite, non-zero)
 __device__ __forceinline__ double div_fast(double a, double b) {
@@ -255,6 +257,17 @@ __device__ __forceinline__ double sqrt_nr2(double v, double& rinv) {
 }
 
 __device__ __forceinline__ double sqrt_nr2(double v) { double r; return sqrt_nr2(v, r); }
+
+// sqrt(v) to ~1 ulp with 1/sqrt(v) only to ~1e-12: one Newton step + the residual correction (which squares the error of the
+// Newton value).  For callers that use the reciprocal root only inside residual-corrected quotients (lbr_normalise).
+__device__ __forceinline__ double sqrt_nr1c(double v, double& rinv) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(v));
+  y = y * fma(-0.5 * v, y * y, 1.5);
+  const double s = v * y;
+  rinv = y;
+  return fma(fma(-s, s, v), 0.5 * y, s);
+}
 
 // grade-dependent primitives
 // seed-grade reciprocal: MUFU.RCP64H alone (9e-7 relative, measured: tests/test_gpu_mathlib.py), no Newton step -- every consumer is a
@@ -906,7 +919,7 @@ __device__ __forceinline__ Norm lbr_normalise(double U, double O, double B, bool
     n.rootFK = __dsqrt_rn(FK);
     r = rcp_nr2(n.rootFK);
   } else {
-    n.rootFK = sqrt_nr2(FK, r);
+    n.rootFK = sqrt_nr1c(FK, r);   // r to 1e-12: every quotient below carries its own residual correction; b_max is seed-grade
   }
   n.bmax = lo * r;   // seed-grade consumers only (the boundary point and the node of the seed); no residual correction
   double q = tv * r;
