@@ -246,7 +246,8 @@ int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivo
 #define PIVOT_DBG_W_FULL 23        /* eval_W at x = a <= 0, s = b > 0: W = b/b' if the difference form was taken, else -Wbar */
 #define PIVOT_DBG_W_SEED 24        /* ... at seed grade */
 #define PIVOT_DBG_RCP_RAW 25       /* 1/a from MUFU.RCP64H alone (seed grade) */
-#define PIVOT_DBG_COUNT 26
+#define PIVOT_DBG_RSQRT_C3 26     /* 1/sqrt(a), a positive normal: MUFU.RSQ64H + one third-order step */
+#define PIVOT_DBG_COUNT 27
 int pivot_iv_debug_math(int fn, const double* a, const double* b, int64_t n, double* out, pivot_iv_stream stream);
 
 /* Number of kernels a call launches (for bench.py's `gpu_launches` bookkeeping). */

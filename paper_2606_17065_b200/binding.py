@@ -223,7 +223,7 @@ def pivot_iv_forward_diag(S_or_F, K, tau, P, flag, r=None, q=None, kernel: int =
 DBG = {name: i for i, name in enumerate((
     "erfcx_one", "erfcx_pair_1", "erfcx_pair_2", "erfcx_seed", "exp_fast", "exp_seed", "log_fast", "log_seed", "log1p_fast",
     "rcp_nr1", "rcp_nr2", "div_fast", "sqrt_nr1", "sqrt_nr2", "rsqrt_nr2", "ninv_tail_seed", "ninv_tail_full", "expf_seed",
-    "logf_seed", "erfcx_dd_diff", "erfcx_dd_sum", "erfcx_dd_seed_diff", "erfcx_dd_seed_sum", "w_full", "w_seed", "rcp_raw"))}
+    "logf_seed", "erfcx_dd_diff", "erfcx_dd_sum", "erfcx_dd_seed_diff", "erfcx_dd_seed_sum", "w_full", "w_seed", "rcp_raw", "rsqrt_c3"))}
 
 
 def pivot_iv_debug_math(fn: str, a: torch.Tensor, b: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:

@@ -47,6 +47,7 @@ debug_math_kernel(int fn, const double* __restrict__ a, const double* __restrict
     case PIVOT_DBG_W_FULL: { const WEval w = eval_W<false>(x, y); r = w.have_W ? w.Wd : -w.Wd; break; }
     case PIVOT_DBG_W_SEED: { const WEval w = eval_W<true>(x, y); r = w.have_W ? w.Wd : -w.Wd; break; }
     case PIVOT_DBG_RCP_RAW: r = rcp_raw(x); break;
+    case PIVOT_DBG_RSQRT_C3: r = rsqrt_c3(x); break;
     default: r = canonical_nan(); break;
   }
   out[i] = r;

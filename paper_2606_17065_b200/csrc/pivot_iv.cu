@@ -344,10 +344,9 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
     const int p = sm.pos[j] & 0x3fff;
     PIVOT_ASSERT(p < rows);
     const double tau = sm.sig[p];
-    // 1/sqrt(tau): MUFU.RSQ64H + Newton for the common rows (tau positive normal, checked by the prelude); a rare row may carry
+    // 1/sqrt(tau): MUFU.RSQ64H + one third-order step for the common rows (tau positive normal, checked by the prelude); a rare row may carry
     // a subnormal tau and takes the library rsqrt
-    double rinv;
-    if (sm.pos[j] & 0x8000) rinv = rsqrt(tau); else (void)sqrt_nr2(tau, rinv);
+    const double rinv = (sm.pos[j] & 0x8000) ? rsqrt(tau) : rsqrt_c3(tau);
     sm.sig[p] = ns.s * rinv;
     sm.veg[p] = sm.veg[p] * ns.vfin * (tau * rinv);
     if (DIAG) {

@@ -188,10 +188,11 @@ def test_reciprocal_division_sqrt():
     rs = [mp.sqrt(mp.mpf(float(t))) for t in v]
     es1, es2 = _relerr(_run("sqrt_nr1", v), rs), _relerr(_run("sqrt_nr2", v), rs)
     er = _relerr(_run("rsqrt_nr2", v), [1 / t for t in rs])
+    er3 = _relerr(_run("rsqrt_c3", v), [1 / t for t in rs])
     assert _run("sqrt_nr1", np.array([0.0]))[0] == 0.0
-    print(f"rcp_raw {e0:.2e} rcp_nr1 {e1:.2e} rcp_nr2 {e2:.2e} div_fast {ed:.2e} sqrt_nr1 {es1:.2e} sqrt_nr2 {es2:.2e} rsqrt_nr2 {er:.2e}")
+    print(f"rcp_raw {e0:.2e} rcp_nr1 {e1:.2e} rcp_nr2 {e2:.2e} div_fast {ed:.2e} sqrt_nr1 {es1:.2e} sqrt_nr2 {es2:.2e} rsqrt_nr2 {er:.2e} rsqrt_c3 {er3:.2e}")
     assert e0 <= 2.0 ** -19 and e1 <= 1e-11 and e2 <= 2 * EPS and ed <= 1.5 * EPS
-    assert es1 <= 1e-11 and es2 <= 1.5 * EPS and er <= 4 * EPS
+    assert es1 <= 1e-11 and es2 <= 1.5 * EPS and er <= 4 * EPS and er3 <= 4 * EPS
 
 
 def test_ninv_tail():
