@@ -47,10 +47,10 @@ BWD_BYTES_PER_ROW = 25
 NCU = {
     "source": "profiles/r2d_forward_tile_ncu_full.md, profiles/r2d_backward_ncu_full.md (ncu --set full of this kernel, config 4)",
     "fwd_dram_bytes_per_row": 56.2,          # dram__bytes_read.sum + dram__bytes_write.sum per row (40.0 read + 16.2 written)
-    "fwd_issued_fp64_flops_per_row": 202.4,  # 2 DFMA + DADD + DMUL thread instructions per row
-    "fwd_fp64_pipe_busy_pct": 39.0,
-    "fwd_issue_active_pct": 68.2,
-    "fwd_warp_inst_per_row": 18.06,
+    "fwd_issued_fp64_flops_per_row": 193.6,  # 2 DFMA + DADD + DMUL thread instructions per row
+    "fwd_fp64_pipe_busy_pct": 37.8,
+    "fwd_issue_active_pct": 68.1,
+    "fwd_warp_inst_per_row": 17.87,
     "bwd_dram_bytes_per_row": 24.5,          # 17.0 read + 7.5 written
 }
 # per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
