@@ -254,7 +254,7 @@ def run_configs(pv, wl, po, hbm_peak, quick):
     torch.cuda.empty_cache()
     days = 128 if quick else 2048
     fwd_case("config2_bsm_chains", wl.config2(days=days, seed=2, device="cuda"), 1 << 18,
-             kernels=(("default", None), ("rowwise", pv.FWD_ROWWISE)))
+             kernels=(("default", None), ("compact", pv.FWD_COMPACT), ("rowwise", pv.FWD_ROWWISE)))
     torch.cuda.empty_cache()
     # config 3: training batch fwd+bwd, both gate modes
     n3 = 1 << 22
@@ -354,6 +354,9 @@ def main():
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config table (configs 0-3)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 size sweep")
     ap.add_argument("--quick", action="store_true", help="smaller configs / sweep up to 2^24 (profiling, smoke runs)")
+    ap.add_argument("--fwd-kernel", default="auto", choices=["auto", "compact", "rowwise"],
+                    help="kernel organisation of the headline step's forward call (default: the library's default call; `compact` "
+                         "launches the same tile kernel without the probe + IF/ELSE graph, whose body ncu cannot see kernel by kernel)")
     ap.add_argument("--selftest-launch", action="store_true", help="CPU-only check of the N > 1 launcher and sharding")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
@@ -392,8 +395,16 @@ def main():
     gP = torch.empty(n, dtype=torch.float64, device="cuda")
     stream = torch.cuda.current_stream()
 
+    fwd_kernel = {"auto": pv.FWD_AUTO, "compact": pv.FWD_COMPACT, "rowwise": pv.FWD_ROWWISE}[args.fwd_kernel]
+
+    def forward():
+        if fwd_kernel == pv.FWD_AUTO:
+            pv.pivot_iv_forward(*a, out=out, stream=stream)        # the default call
+        else:
+            pv.pivot_iv_forward_ex(*a, fwd_kernel, out=out, stream=stream)
+
     def step():
-        pv.pivot_iv_forward(*a, out=out, stream=stream)
+        forward()
         pv.pivot_iv_backward(gsig, out[1], out[2], VEGA_FLOOR, pv.GATE_MASK, out=gP, stream=stream)
 
     for _ in range(W):
@@ -412,7 +423,7 @@ def main():
     t_begin.record(stream)
     for i in range(K):
         ev[i][0].record(stream)
-        pv.pivot_iv_forward(*a, out=out, stream=stream)
+        forward()
         ev[i][1].record(stream)
         pv.pivot_iv_backward(gsig, out[1], out[2], VEGA_FLOOR, pv.GATE_MASK, out=gP, stream=stream)
         ev[i][2].record(stream)
@@ -428,9 +439,10 @@ def main():
         total_ms, fwd_ms, bwd_ms = (float(x) for x in t.tolist())
     ms_per_step = total_ms / K
     value = world * n / (ms_per_step * 1e-3)
-    # kernels launched per step: counted from the library's own dispatch (forward: 1; backward: the 4-row vector body,
-    # plus a scalar tail only when n is not a multiple of 4 or a pointer is not 16-byte aligned -- neither here)
-    launches_per_step = int(lib.pivot_iv_launches_per_forward()) + int(lib.pivot_iv_launches_per_backward()) + (1 if n % 4 else 0)
+    # kernels launched per step: counted from the library's own dispatch (forward: 1, or 2 = probe + chosen kernel in one graph
+    # launch for the default organisation from PIVOT_AUTO_MIN_ROWS rows on; backward: the 4-row vector body, plus a scalar tail
+    # only when n is not a multiple of 4 or a pointer is not 16-byte aligned -- neither here)
+    launches_per_step = int(lib.pivot_iv_forward_launches(n, fwd_kernel)) + int(lib.pivot_iv_launches_per_backward()) + (1 if n % 4 else 0)
 
     # --- e2e: the same step through the C-ABI host entry point (pinned host buffers, H2D + D2H inside the timed region)
     e2e = None
@@ -638,7 +650,12 @@ def main():
                                        "call/put 50/50, Black-76 D=1); step = fused forward + MASK backward (floor 1e-8)",
                            "rows_per_gpu": n, "l2": "inputs+outputs 5.5 GB per step >> 126 MB L2, no flush needed",
                            "global_rows": world * n, "rank0_shard": [g_begin, g_end],
-                           "zone_mix_rows[z0,z1,z2,z3,non_ok]": mix},
+                           "zone_mix_rows[z0,z1,z2,z3,non_ok]": mix,
+                           "forward_call": {"auto": "pivot_iv_forward (default): ONE graph launch = one-warp probe kernel -> IF/ELSE node -> "
+                                                    "forward_kernel_tile here (forward_kernel_scalar on option chains); fwd_ms and "
+                                                    "roofline.avg_launch_ms bracket the whole graph launch (~20 us more than the kernel alone)",
+                                            "compact": "pivot_iv_forward_ex(PIVOT_FWD_COMPACT): forward_kernel_tile launched directly",
+                                            "rowwise": "pivot_iv_forward_ex(PIVOT_FWD_ROWWISE): forward_kernel_scalar launched directly"}[args.fwd_kernel]},
                 "fwd_iv_per_s": world * n / (fwd_ms * 1e-3), "fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
                 "bwd_rows_per_s": world * n / (bwd_ms * 1e-3),
                 "solved_rows_per_s_fwd": world * sum(mix[:4]) / (fwd_ms * 1e-3),

@@ -87,8 +87,13 @@ int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double
  *                      solver passes run: best when the batch is mixed (degenerate / invalid rows, zones in random order);
  *   PIVOT_FWD_ROWWISE  one row per thread, no shared memory, no barriers: best when nearly every row solves and
  *                      neighbouring rows are alike (option chains in strike order);
- *   PIVOT_FWD_AUTO     what pivot_iv_forward uses (COMPACT).
- * COMPACT and ROWWISE run the same per-row arithmetic: bit-identical results.
+ *   PIVOT_FWD_AUTO     what pivot_iv_forward uses: COMPACT below PIVOT_AUTO_MIN_ROWS rows; from there on the choice is made
+ *                      on the device, inside ONE graph launch: a one-warp probe kernel reads 4 x 32 rows spread over the
+ *                      arrays and an IF / ELSE graph node runs ROWWISE if at least three quarters of the neighbour pairs
+ *                      sit close to each other in (moneyness, time value, tau, carry), else COMPACT (~20 us on the GPU time
+ *                      line, ~3 us of host time; serialised per device by a mutex around the launch).  A call made while
+ *                      the stream is being captured takes COMPACT (a graph launch cannot be captured).
+ * COMPACT and ROWWISE run the same per-row arithmetic: bit-identical results, whichever AUTO picks.
  *   PIVOT_FWD_FP64_ONLY (flag, OR it into any of the three): every special function, reciprocal and interpolant of the
  *                      seed and of the first Householder step at full fp64 instead of "seed grade" (fp32 erfcx, MUFU
  *                      exp / log, fp32 rational cubics).  The default tiering only has to land inside the basin of the
@@ -99,6 +104,7 @@ int pivot_iv_forward(const pivot_iv_inputs* in, int64_t n, double* sigma, double
 #define PIVOT_FWD_COMPACT 1
 #define PIVOT_FWD_ROWWISE 2
 #define PIVOT_FWD_FP64_ONLY 4
+#define PIVOT_AUTO_MIN_ROWS 25165824 /* 3 * 2^23 */
 int pivot_iv_forward_ex(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, int kernel,
                         pivot_iv_stream stream);
 
@@ -250,9 +256,20 @@ int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivo
 #define PIVOT_DBG_COUNT 27
 int pivot_iv_debug_math(int fn, const double* a, const double* b, int64_t n, double* out, pivot_iv_stream stream);
 
-/* Number of kernels a call launches (for bench.py's `gpu_launches` bookkeeping). */
+/* Number of kernels a call launches (for bench.py's `gpu_launches` bookkeeping): pivot_iv_launches_per_forward is the
+ * count of an explicit organisation (and of PIVOT_FWD_AUTO below PIVOT_AUTO_MIN_ROWS); pivot_iv_forward_launches(n, kernel)
+ * is the count of pivot_iv_forward_ex(..., kernel, ...) on n rows outside stream capture: 2 (probe + chosen kernel, one
+ * graph launch) for PIVOT_FWD_AUTO at n >= PIVOT_AUTO_MIN_ROWS, else 1. */
 int pivot_iv_launches_per_forward(void);
 int pivot_iv_launches_per_backward(void);
+int pivot_iv_forward_launches(int64_t n, int kernel);
+
+/* The launch probe of PIVOT_FWD_AUTO on its own (diagnostic; tests): *rowwise = 1 if the rows follow each other closely enough
+ * for the row-per-thread organisation, else 0 (n < 256: 0).
+ *   in       as pivot_iv_forward (P is read)
+ *   rowwise  [out, device, one int]
+ * Returns PIVOT_ERR_NULL / _BAD_N / _MIXED_RQ / _CUDA. */
+int pivot_iv_forward_probe(const pivot_iv_inputs* in, int64_t n, int* rowwise, pivot_iv_stream stream);
 
 const char* pivot_iv_strerror(int code);
 int pivot_iv_version(void);

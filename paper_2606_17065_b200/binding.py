@@ -25,7 +25,7 @@ EXPORTS = (
     "pivot_iv_launches_per_forward", "pivot_iv_launches_per_backward", "pivot_iv_strerror", "pivot_iv_version",
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
-    "pivot_iv_forward_diag", "pivot_iv_debug_math",
+    "pivot_iv_forward_diag", "pivot_iv_debug_math", "pivot_iv_forward_launches", "pivot_iv_forward_probe",
 )
 
 
@@ -56,6 +56,8 @@ def load_library():
     vp, i64, dbl, cint = C.c_void_p, C.c_int64, C.c_double, C.c_int
     lib.pivot_iv_forward.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
     lib.pivot_iv_forward_ex.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, cint, vp]
+    lib.pivot_iv_forward_probe.argtypes = [C.POINTER(_Inputs), i64, vp, vp]
+    lib.pivot_iv_forward_launches.argtypes = [i64, cint]
     lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
     lib.pivot_iv_debug_math.argtypes = [cint, vp, vp, i64, vp, vp]
     lib.pivot_iv_forward_diag.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp, vp, cint, vp]
@@ -199,6 +201,30 @@ def pivot_iv_forward(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=N
 def pivot_iv_forward_ex(S_or_F, K, tau, P, flag, kernel: int, r=None, q=None, out=None, stream=None):
     """pivot_iv_forward with an explicit kernel organisation: FWD_AUTO, FWD_COMPACT or FWD_ROWWISE (same results)."""
     return _forward(S_or_F, K, tau, P, flag, r, q, out, stream, False, kernel=kernel)
+
+
+AUTO_MIN_ROWS = 3 << 23   # PIVOT_AUTO_MIN_ROWS: from here on FWD_AUTO chooses on the device (probe kernel + IF / ELSE graph node)
+
+
+def pivot_iv_forward_probe(S_or_F, K, tau, P, flag, r=None, q=None, stream=None) -> torch.Tensor:
+    """The launch probe of FWD_AUTO on its own: a one-element int32 CUDA tensor, 1 if the rows follow each other closely
+    enough for the row-per-thread organisation (option chains in strike order), else 0."""
+    _require_cuda()
+    lib = load_library()
+    n = S_or_F.shape[0]
+    dev = S_or_F.device
+    inp = _Inputs(_ptr(S_or_F, "S_or_F", n, dev), _ptr(K, "K", n, dev), _ptr(tau, "tau", n, dev),
+                  None if r is None else _ptr(r, "r", n, dev), None if q is None else _ptr(q, "q", n, dev),
+                  _ptr(P, "P", n, dev), _ptr(flag, "flag", n, dev))
+    verdict = torch.zeros(1, dtype=torch.int32, device=dev)
+    with _guard(dev):
+        _check(lib.pivot_iv_forward_probe(C.byref(inp), n, verdict.data_ptr(), _stream_ptr(stream)))
+    return verdict
+
+
+def pivot_iv_forward_launches(n: int, kernel: int = FWD_AUTO) -> int:
+    """Kernels launched by one forward call on n rows with this organisation (2 = probe + chosen kernel, one graph launch)."""
+    return int(load_library().pivot_iv_forward_launches(int(n), int(kernel)))
 
 
 def pivot_iv_forward_diag(S_or_F, K, tau, P, flag, r=None, q=None, kernel: int = FWD_AUTO, stream=None):

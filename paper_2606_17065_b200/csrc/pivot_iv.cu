@@ -12,6 +12,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <new>
 
 #include "../../include/pivot_iv.h"
@@ -380,6 +381,46 @@ forward_kernel_tile(pivot_iv_inputs in, int64_t n, double* __restrict__ sigma, d
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Launch probe of PIVOT_FWD_AUTO (large launches only; see launch_auto): ONE warp looks at kProbeSegs groups of 32 consecutive
+// rows spread over the arrays and counts the neighbour pairs that sit close to each other in (moneyness, time value over
+// min(S, K), tau, carry): such rows follow the same branches of the solver, and row-per-thread is then the faster organisation
+// (option chains in strike order).  Density does not enter: dense RANDOM rows are 12-19 % faster
+// regrouped.  Close pairs of 124 on the workloads of DESIGN.md section 6: BSM chains 124, every other workload 0 ... 3.
+// The test works on the raw inputs (BSM: S for F and P for P / D: along a chain carry and discount factor are common factors
+// of neighbouring rows).  The verdict goes to the IF / ELSE node of the launch graph (handle) and / or to *verdict.
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int kProbeSegs = 4;
+constexpr int kProbeClosePairs = 93;   // of 31 kProbeSegs = 124: three quarters
+
+template <bool BSM>
+__global__ void __launch_bounds__(32) forward_probe_kernel(pivot_iv_inputs in, int64_t n, cudaGraphConditionalHandle handle,
+                                                           int use_handle, int* verdict) {
+  const int lane = threadIdx.x;
+  int close_pairs = 0;
+  if (n >= 32 * 2 * kProbeSegs) {
+#pragma unroll
+    for (int s = 0; s < kProbeSegs; ++s) {
+      const int64_t i = ((((int64_t)(2 * s + 1) * (n / (2 * kProbeSegs))) >> 5) << 5) + lane;   // i + (31 - lane) < n
+      const double F = in.S_or_F[i], K = in.K[i], T = in.tau[i], P = in.P[i], f = in.flag[i];
+      const double c = BSM ? (in.r[i] - in.q[i]) * T : 0.0;
+      const double lo = fmin(F, K), hi = fmax(F, K), iota = fmax(f * (F - K), 0.0);
+      // fp32 is plenty; the quotients are formed in double first (F, K may lie outside the fp32 range).  NaN / Inf compare false.
+      const float a = (float)(lo / hi), b = (float)((P - iota) / lo), t = (float)T, cf = (float)c;
+      const float an = __shfl_down_sync(0xffffffffu, a, 1), bn = __shfl_down_sync(0xffffffffu, b, 1),
+                  tn = __shfl_down_sync(0xffffffffu, t, 1), cn = __shfl_down_sync(0xffffffffu, cf, 1);
+      const bool close = (lane < 31) & (fabsf(a - an) <= 0.05f) & (fabsf(b - bn) <= 0.05f) & (fabsf(t - tn) <= 0.125f * t) &
+                         (fabsf(cf - cn) <= 0.05f);
+      close_pairs += __popc(__ballot_sync(0xffffffffu, close));
+    }
+  }
+  if (lane == 0) {
+    const unsigned rowwise = close_pairs >= kProbeClosePairs ? 1u : 0u;
+    if (use_handle) cudaGraphSetConditional(handle, rowwise);
+    if (verdict) *verdict = (int)rowwise;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Backward kernel: grad_P = gate * grad_sigma / vega  (eq.(8)-(10)); 25 B/row, HBM-bound.
 // ---------------------------------------------------------------------------------------------------------------
 template <int MODE>
@@ -507,10 +548,21 @@ int launch_tile(const pivot_iv_inputs& in, int64_t n, double* sigma, double* veg
   return PIVOT_OK;
 }
 
+constexpr int64_t kAutoMinRows = PIVOT_AUTO_MIN_ROWS;
+static_assert(kAutoMinRows == ((int64_t)3 << 23), "PIVOT_AUTO_MIN_ROWS");
+template <bool BSM>
+int launch_auto(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, cudaStream_t st,
+                bool* launched);   // below
+
 template <bool BSM, bool DIAG, bool FULL>
 int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, const DiagOut& dg,
-                     bool rowwise, cudaStream_t st) {
+                     bool rowwise, bool autosel, cudaStream_t st) {
   int rc = PIVOT_OK;
+  if (!DIAG && !FULL && autosel && n >= kAutoMinRows) {
+    bool launched = false;
+    rc = launch_auto<BSM>(in, n, sigma, vega, status, st, &launched);
+    if (rc != PIVOT_OK || launched) return rc;
+  }
   if (rowwise) {
     const int64_t blocks = (n + kFwdThreads - 1) / kFwdThreads;
     forward_kernel_scalar<BSM, DIAG, FULL><<<(unsigned)blocks, kFwdThreads, 0, st>>>(in, n, sigma, vega, status, dg);
@@ -529,6 +581,117 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// PIVOT_FWD_AUTO on large launches (n >= kAutoMinRows): ONE graph launch = forward_probe_kernel -> IF / ELSE node ->
+// forward_kernel_scalar (rows that follow each other closely) | forward_kernel_tile (everything else).  The choice is made on
+// the device, between two separate kernels: every way tried to make it INSIDE one kernel cost the tile kernel more than it
+// gained, because its hot code already fills the 32 KB instruction cache of the SM.  The graph costs
+// ~20 us on the GPU time line (probe + conditional node + launch of the body: 1.519 -> 1.540 ms at 2^26 mixed rows, where the
+// row-per-thread branch saves 9 % on option chains) and ~3 us of host time per call (three parameter updates + launch), hence
+// the size limit: <= 3.5 % of a launch of kAutoMinRows rows.  One executable graph per device and mode, built on first use;
+// calls are serialised by a mutex around update + launch (the launches themselves are asynchronous as ever).  During stream
+// capture (a graph launch cannot be captured) and after any failure to build the graph the call takes the tile kernel.
+// ---------------------------------------------------------------------------------------------------------------
+
+struct AutoGraph {
+  std::mutex mu;
+  bool failed = false;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  cudaGraphNode_t probe = nullptr, row = nullptr, tile = nullptr;
+  cudaGraphConditionalHandle handle{};
+};
+
+struct AutoArgs {   // argument storage the kernel-node parameter arrays point into
+  pivot_iv_inputs in;
+  int64_t n;
+  double* sigma;
+  double* vega;
+  uint8_t* status;
+  DiagOut dg;
+  cudaGraphConditionalHandle handle;
+  int use_handle;
+  int* verdict;
+};
+
+template <bool BSM>
+void auto_node_params(AutoArgs& a, void** pargs, void** fargs, cudaKernelNodeParams& kprobe, cudaKernelNodeParams& krow,
+                      cudaKernelNodeParams& ktile) {
+  pargs[0] = &a.in; pargs[1] = &a.n; pargs[2] = &a.handle; pargs[3] = &a.use_handle; pargs[4] = &a.verdict;
+  fargs[0] = &a.in; fargs[1] = &a.n; fargs[2] = &a.sigma; fargs[3] = &a.vega; fargs[4] = &a.status; fargs[5] = &a.dg;
+  kprobe = cudaKernelNodeParams{};
+  kprobe.func = reinterpret_cast<void*>(forward_probe_kernel<BSM>);
+  kprobe.gridDim = dim3(1); kprobe.blockDim = dim3(32); kprobe.kernelParams = pargs;
+  krow = cudaKernelNodeParams{};
+  krow.func = reinterpret_cast<void*>(forward_kernel_scalar<BSM, false, false>);
+  krow.gridDim = dim3((unsigned)((a.n + kFwdThreads - 1) / kFwdThreads)); krow.blockDim = dim3(kFwdThreads); krow.kernelParams = fargs;
+  ktile = cudaKernelNodeParams{};
+  ktile.func = reinterpret_cast<void*>(forward_kernel_tile<BSM, false, 4, false>);
+  ktile.gridDim = dim3((unsigned)((a.n + 4 * kTileThreads - 1) / (4 * kTileThreads))); ktile.blockDim = dim3(kTileThreads);
+  ktile.sharedMemBytes = (unsigned)sizeof(TileSmem<4>); ktile.kernelParams = fargs;
+}
+
+// returns PIVOT_OK and *launched = true when the graph has been enqueued; *launched = false: the caller takes the tile kernel
+template <bool BSM>
+int launch_auto(const pivot_iv_inputs& in, int64_t n, double* sigma, double* vega, uint8_t* status, cudaStream_t st,
+                bool* launched) {
+  static AutoGraph graphs[kMaxDevices];
+  *launched = false;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) { (void)cudaGetLastError(); return PIVOT_OK; }
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); return PIVOT_OK; }
+  if (cs != cudaStreamCaptureStatusNone) return PIVOT_OK;
+  const int rc = ensure_dynamic_smem<forward_kernel_tile<BSM, false, 4, false>>((int)sizeof(TileSmem<4>));
+  if (rc != PIVOT_OK) return rc;
+  AutoGraph& g = graphs[dev];
+  std::lock_guard<std::mutex> lock(g.mu);
+  if (g.failed) return PIVOT_OK;
+  AutoArgs a{in, n, sigma, vega, status, DiagOut{nullptr, nullptr, nullptr}, g.handle, 1, nullptr};
+  void* pargs[5];
+  void* fargs[6];
+  cudaKernelNodeParams kprobe, krow, ktile;
+  if (!g.exec) {
+    bool ok = cudaGraphCreate(&g.graph, 0) == cudaSuccess &&
+              cudaGraphConditionalHandleCreate(&g.handle, g.graph, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+    if (ok) {
+      a.handle = g.handle;
+      auto_node_params<BSM>(a, pargs, fargs, kprobe, krow, ktile);
+      ok = cudaGraphAddKernelNode(&g.probe, g.graph, nullptr, 0, &kprobe) == cudaSuccess;
+    }
+    cudaGraphNodeParams cp{};
+    if (ok) {
+      cp.type = cudaGraphNodeTypeConditional;
+      cp.conditional.handle = g.handle;
+      cp.conditional.type = cudaGraphCondTypeIf;
+      cp.conditional.size = 2;   // [0]: condition != 0 (row per thread), [1]: else (tile)
+      cudaGraphNode_t cond = nullptr;
+      ok = cudaGraphAddNode(&cond, g.graph, &g.probe, 1, &cp) == cudaSuccess;
+    }
+    ok = ok && cudaGraphAddKernelNode(&g.row, cp.conditional.phGraph_out[0], nullptr, 0, &krow) == cudaSuccess &&
+         cudaGraphAddKernelNode(&g.tile, cp.conditional.phGraph_out[1], nullptr, 0, &ktile) == cudaSuccess &&
+         cudaGraphInstantiate(&g.exec, g.graph, 0) == cudaSuccess;
+    if (!ok) {
+      (void)cudaGetLastError();
+      if (g.graph) (void)cudaGraphDestroy(g.graph);
+      g.graph = nullptr; g.exec = nullptr; g.failed = true;
+      return PIVOT_OK;
+    }
+  } else {
+    auto_node_params<BSM>(a, pargs, fargs, kprobe, krow, ktile);
+    if (cudaGraphExecKernelNodeSetParams(g.exec, g.probe, &kprobe) != cudaSuccess ||
+        cudaGraphExecKernelNodeSetParams(g.exec, g.row, &krow) != cudaSuccess ||
+        cudaGraphExecKernelNodeSetParams(g.exec, g.tile, &ktile) != cudaSuccess) {
+      (void)cudaGetLastError();
+      g.failed = true;   // the executable graph may hold a partial update: never launched again
+      return PIVOT_OK;
+    }
+  }
+  if (cudaGraphLaunch(g.exec, st) != cudaSuccess) { (void)cudaGetLastError(); return PIVOT_ERR_CUDA; }
+  *launched = true;
+  return PIVOT_OK;
+}
+
 int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status, const DiagOut* dg,
                  cudaStream_t st, int kernel = PIVOT_FWD_AUTO) {
   if (!in) return PIVOT_ERR_NULL;
@@ -539,10 +702,11 @@ int forward_impl(const pivot_iv_inputs* in, int64_t n, double* sigma, double* ve
   if (n == 0) return PIVOT_OK;
   if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status) return PIVOT_ERR_NULL;
   if (n > ((int64_t)1 << 37)) return PIVOT_ERR_BAD_N;  // grid.x limit
-  const bool bsm = in->r != nullptr, full = (kernel & PIVOT_FWD_FP64_ONLY) != 0, rowwise = org == PIVOT_FWD_ROWWISE;
+  const bool bsm = in->r != nullptr, full = (kernel & PIVOT_FWD_FP64_ONLY) != 0, rowwise = org == PIVOT_FWD_ROWWISE,
+             autosel = org == PIVOT_FWD_AUTO;
   const DiagOut none{nullptr, nullptr, nullptr};
   const DiagOut& d = dg ? *dg : none;
-#define PIVOT_DISPATCH(B, G, F) return launch_forward_t<B, G, F>(*in, n, sigma, vega, status, d, rowwise, st)
+#define PIVOT_DISPATCH(B, G, F) return launch_forward_t<B, G, F>(*in, n, sigma, vega, status, d, rowwise, autosel, st)
   if (dg) {
     if (bsm) { if (full) PIVOT_DISPATCH(true, true, true); PIVOT_DISPATCH(true, true, false); }
     if (full) PIVOT_DISPATCH(false, true, true);
@@ -632,6 +796,21 @@ int pivot_iv_probe_dfma(int64_t iters, double* sink, double* fma_count_out, pivo
 }
 
 int pivot_iv_launches_per_forward(void) { return 1; }
+
+int pivot_iv_forward_launches(int64_t n, int kernel) {
+  return ((kernel & ~PIVOT_FWD_FP64_ONLY) == PIVOT_FWD_AUTO && !(kernel & PIVOT_FWD_FP64_ONLY) && n >= kAutoMinRows) ? 2 : 1;
+}
+
+int pivot_iv_forward_probe(const pivot_iv_inputs* in, int64_t n, int* rowwise, pivot_iv_stream stream) {
+  if (!in || !rowwise) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag) return PIVOT_ERR_NULL;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (in->r) forward_probe_kernel<true><<<1, 32, 0, st>>>(*in, n, cudaGraphConditionalHandle{}, 0, rowwise);
+  else forward_probe_kernel<false><<<1, 32, 0, st>>>(*in, n, cudaGraphConditionalHandle{}, 0, rowwise);
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
 int pivot_iv_launches_per_backward(void) { return 1; }
 
 const char* pivot_iv_strerror(int code) {

@@ -395,6 +395,73 @@ def test_forward_ex_kernel_choices_are_bit_identical():
     assert np.array_equal(hst.numpy(), ref[2].cpu().numpy())
 
 
+def test_auto_probe_verdicts():
+    """The launch probe of FWD_AUTO (pivot_iv_forward_probe): row-per-thread for option chains in strike order (BSM and
+    Black-76 views of them), the regrouping kernel for every workload whose neighbouring rows are unrelated; too few rows: 0."""
+    ch = to_device(wl.config2(days=3, seed=5))
+    a = [ch[k] for k in KEYS]
+    assert int(pv.pivot_iv_forward_probe(*a, r=ch["r"], q=ch["q"]).item()) == 1
+    assert int(pv.pivot_iv_forward_probe(*a).item()) == 1                       # the same rows read as Black-76 (F = S, D = 1)
+    assert int(pv.pivot_iv_forward_probe(*[t[:255] for t in a]).item()) == 0    # fewer than 4 x 2 x 32 rows
+    for cfg in (wl.config0(100_000, seed=6), wl.config1(100_000, seed=7), wl.config1(100_000, seed=8, solve_only=True),
+                wl.config3(100_000, seed=9)):
+        d = to_device(cfg)
+        assert int(pv.pivot_iv_forward_probe(*[d[k] for k in KEYS]).item()) == 0
+    # non-finite rows never count as close
+    bad = [t.clone() for t in a]
+    bad[3][:] = float("nan")
+    assert int(pv.pivot_iv_forward_probe(*bad, r=ch["r"], q=ch["q"]).item()) == 0
+    assert pv.pivot_iv_forward_launches(pv.AUTO_MIN_ROWS) == 2 and pv.pivot_iv_forward_launches(pv.AUTO_MIN_ROWS - 1) == 1
+    assert pv.pivot_iv_forward_launches(pv.AUTO_MIN_ROWS, pv.FWD_COMPACT) == 1
+
+
+def test_auto_graph_launch_on_large_inputs():
+    """From AUTO_MIN_ROWS rows on the default call is ONE graph launch: probe kernel -> IF / ELSE node -> row-per-thread or
+    regrouping kernel.  Both branches, repeated calls with other sizes and pointers (the executable graph is updated in
+    place), a second stream, and a call inside stream capture (which takes the plain kernel) give the bits of the explicit
+    organisations."""
+    n = pv.AUTO_MIN_ROWS + 1027
+    mixed = to_device(wl.config1(n, seed=31))
+    days = -(-n // 16000)
+    chains = to_device(wl.config2(days=days, seed=32))
+    side = torch.cuda.Stream()
+    for d in (mixed, chains, mixed):
+        a = [d[k] for k in KEYS]
+        m = a[0].numel()
+        kw = dict(r=d.get("r"), q=d.get("q"))
+        ref = pv.pivot_iv_forward_ex(*a, pv.FWD_COMPACT, **kw)
+        got = pv.pivot_iv_forward(*a, **kw)
+        for x, y in zip(got, ref):
+            assert np.array_equal(_bits(x), _bits(y))
+        del got
+        # fewer rows from an offset (other grid sizes, other pointers), on another stream
+        lo, hi = 4096, m - 513
+        sub = [t[lo:hi] for t in a]
+        kws = {k: (v[lo:hi] if v is not None else None) for k, v in kw.items()}
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            got = pv.pivot_iv_forward(*sub, **kws)
+        side.synchronize()
+        for x, y in zip(got, ref):
+            assert np.array_equal(_bits(x), _bits(y[lo:hi]))
+        del got, ref
+    # stream capture: the call is recorded as a plain kernel launch and replays with the same bits
+    a = [chains[k] for k in KEYS]
+    kw = dict(r=chains["r"], q=chains["q"])
+    ref = pv.pivot_iv_forward_ex(*a, pv.FWD_ROWWISE, **kw)
+    out = tuple(torch.empty_like(t) for t in ref)
+    g = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g):
+        pv.pivot_iv_forward(*a, out=out, **kw)
+    for t in out:
+        t.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    for x, y in zip(out, ref):
+        assert np.array_equal(_bits(x), _bits(y))
+
+
 def _tier_cases():
     """Workloads of the precision-tier tests: the four-zone stress (config 1), its 1-solve variant, config 0 and the wide
     domain (|x| <= 12, F over nine decades, total volatility up to 40)."""
