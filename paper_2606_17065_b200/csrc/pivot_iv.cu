@@ -589,7 +589,8 @@ int launch_forward_t(const pivot_iv_inputs& in, int64_t n, double* sigma, double
 // ~20 us on the GPU time line (probe + conditional node + launch of the body: 1.519 -> 1.540 ms at 2^26 mixed rows, where the
 // row-per-thread branch saves 9 % on option chains) and ~3 us of host time per call (three parameter updates + launch), hence
 // the size limit: <= 3.5 % of a launch of kAutoMinRows rows.  One executable graph per device and mode, built on first use;
-// calls are serialised by a mutex around update + launch (the launches themselves are asynchronous as ever).  During stream
+// calls are serialised by a mutex around update + launch (the launches themselves are asynchronous as ever; CUDA runs two launches
+// of one executable graph one after the other, also from different streams: at these sizes each fills the GPU anyway).  During stream
 // capture (a graph launch cannot be captured) and after any failure to build the graph the call takes the tile kernel.
 // ---------------------------------------------------------------------------------------------------------------
 
@@ -687,7 +688,11 @@ int launch_auto(const pivot_iv_inputs& in, int64_t n, double* sigma, double* veg
       return PIVOT_OK;
     }
   }
-  if (cudaGraphLaunch(g.exec, st) != cudaSuccess) { (void)cudaGetLastError(); return PIVOT_ERR_CUDA; }
+  if (cudaGraphLaunch(g.exec, st) != cudaSuccess) {   // e.g. after cudaDeviceReset: the plain launch reports what is really wrong
+    (void)cudaGetLastError();
+    g.failed = true;
+    return PIVOT_OK;
+  }
   *launched = true;
   return PIVOT_OK;
 }
