@@ -462,6 +462,41 @@ def test_auto_graph_launch_on_large_inputs():
         assert np.array_equal(_bits(x), _bits(y))
 
 
+def test_auto_graph_launch_from_two_threads():
+    """Two host threads issue large default calls at the same time, each on its own stream with its own outputs: the calls share
+    one executable graph per device (parameters updated in place under a mutex) and must not see each other's parameters."""
+    import threading
+    n = pv.AUTO_MIN_ROWS
+    d = to_device(wl.config1(n, seed=41))
+    a = [d[k] for k in KEYS]
+    ref = pv.pivot_iv_forward_ex(*a, pv.FWD_COMPACT)
+    cuts = ((0, n), (8192, n - 1024))
+    outs = [tuple(torch.empty(hi - lo, dtype=t.dtype, device="cuda") for t in ref) for lo, hi in cuts]
+    streams = [torch.cuda.Stream() for _ in cuts]
+    torch.cuda.synchronize()
+    errors = []
+
+    def work(i):
+        try:
+            lo, hi = cuts[i]
+            with torch.cuda.stream(streams[i]):
+                for _ in range(4):
+                    pv.pivot_iv_forward(*[t[lo:hi] for t in a], out=outs[i])
+            streams[i].synchronize()
+        except Exception as e:   # surfaced in the main thread
+            errors.append(e)
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(len(cuts))]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for (lo, hi), out in zip(cuts, outs):
+        for x, y in zip(out, ref):
+            assert np.array_equal(_bits(x), _bits(y[lo:hi]))
+
+
 def _tier_cases():
     """Workloads of the precision-tier tests: the four-zone stress (config 1), its 1-solve variant, config 0 and the wide
     domain (|x| <= 12, F over nine decades, total volatility up to 40)."""
