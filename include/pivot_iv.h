@@ -38,6 +38,7 @@ extern "C" {
 #define PIVOT_ERR_MIXED_RQ (-5)  /* exactly one of r, q is NULL */
 #define PIVOT_ERR_CUDA (-6)      /* CUDA runtime error (launch, copy, allocation inside a pipeline) */
 #define PIVOT_ERR_BAD_ARG (-7)   /* other invalid argument (pipeline geometry, device index) */
+#define PIVOT_ERR_STATIC_MAX (-8) /* pivot_iv_forward_host_static: n > PIVOT_STATIC_MAX_ROWS */
 
 /* per-row status byte written by the forward pass (PAPER.md:98 Alg.1 l.3, :125, :363; readings in DESIGN.md) */
 #define PIVOT_ST_OK 0              /* sigma, vega valid */
@@ -213,6 +214,24 @@ int pivot_iv_forward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, int64
 int pivot_iv_forward_backward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* grad_sigma,
                                    double vega_floor, int mode, int64_t n, double* sigma, double* vega,
                                    uint8_t* status, double* grad_P);
+
+/* Forward on HOST arrays without any allocation (for callers that cannot call cudaMalloc: code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same operation and same bits as pivot_iv_forward (Alg.1 l.1-3);
+ * the device staging is a file-scope `static __device__` array of the library instead of a pipeline's cudaMalloc buffers:
+ * PIVOT_STATIC_MAX_ROWS rows x (9 doubles + 1 byte) = 4,784,128 B, held by every GPU that loads the library until exit.
+ *   in       host pointers, n doubles each (r = q = NULL: Black-76); pin them for copies that are asynchronous to the host
+ *   n        0 <= n <= PIVOT_STATIC_MAX_ROWS, else PIVOT_ERR_STATIC_MAX (nothing is enqueued)
+ *   sigma, vega [out, host, n doubles], status [out, host, n bytes]
+ *   stream   the H2D copies, the kernel and the D2H copies are enqueued on it, on the current device; the call does NOT
+ *            synchronise: the outputs are valid once the caller has synchronised the stream (or waited on an event)
+ * Calls no cudaMalloc / cudaFree / allocating library routine; the first call on a device looks the array's address up
+ * (cudaGetSymbolAddress) and opts the kernel in to its shared-memory size.  Every call shares the one array per GPU, which keeps
+ * the previous call's contents: nothing in it has to start at zero (the call overwrites every byte it reads), but two calls
+ * that overlap on the GPU -- different streams without a dependency, several host threads -- race on it; calls on one stream
+ * are ordered.  Returns PIVOT_ERR_NULL / _BAD_N / _STATIC_MAX / _MIXED_RQ / _CUDA. */
+#define PIVOT_STATIC_MAX_ROWS 65536
+int pivot_iv_forward_host_static(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                                 pivot_iv_stream stream);
 
 /* ---- measurement helpers ---- */
 /* Dependent-DFMA-chain microbenchmark on `stream`: every thread of a full-occupancy grid runs `iters` rounds of 8

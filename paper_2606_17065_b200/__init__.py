@@ -27,6 +27,8 @@ from .binding import (  # noqa: F401
     pivot_iv_debug_math,
     pivot_iv_forward_ex,
     pivot_iv_forward_probe,
+    pivot_iv_forward_host_static,
+    STATIC_MAX_ROWS,
     pivot_iv_forward_launches,
     AUTO_MIN_ROWS,
     pivot_iv_forward_zones,
@@ -45,4 +47,5 @@ __all__ = [
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
     "GATE_ATTENUATE", "GATE_STRICT", "RT_GATED", "RT_NAIVE", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "pivot_iv_debug_math", "EXPORTS",
     "pivot_iv_forward_probe", "pivot_iv_forward_launches", "AUTO_MIN_ROWS",
+    "pivot_iv_forward_host_static", "STATIC_MAX_ROWS",
 ]

@@ -26,6 +26,7 @@ EXPORTS = (
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
     "pivot_iv_forward_diag", "pivot_iv_debug_math", "pivot_iv_forward_launches", "pivot_iv_forward_probe",
+    "pivot_iv_forward_host_static",
 )
 
 
@@ -66,6 +67,7 @@ def load_library():
     lib.pivot_iv_pipeline_create.argtypes = [C.POINTER(vp), cint, i64, cint]
     lib.pivot_iv_pipeline_destroy.argtypes = [vp]
     lib.pivot_iv_forward_host.argtypes = [vp, C.POINTER(_Inputs), i64, vp, vp, vp]
+    lib.pivot_iv_forward_host_static.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp]
     lib.pivot_iv_forward_backward_host.argtypes = [vp, C.POINTER(_Inputs), vp, dbl, cint, i64, vp, vp, vp, vp]
     lib.pivot_iv_probe_dfma.argtypes = [i64, vp, C.POINTER(dbl), vp]
     lib.pivot_iv_black_price.argtypes = [C.POINTER(_Inputs), vp, i64, vp, vp, vp]
@@ -433,6 +435,34 @@ class Pipeline:
                                                         _host(vega, "vega"), _host(status, "status", torch.uint8),
                                                         _host(gP, "grad_P")))
         return sigma, vega, status, gP
+
+
+STATIC_MAX_ROWS = 65536   # PIVOT_STATIC_MAX_ROWS
+
+
+def pivot_iv_forward_host_static(S_or_F, K, tau, P, flag, r=None, q=None, out=None, stream=None, sync=True):
+    """Forward on HOST tensors with no device allocation (pivot_iv_forward_host_static): the device staging is a static array
+    of the library (at most STATIC_MAX_ROWS rows per call).  `out` = (sigma, vega, status) host tensors, allocated here (on the
+    host) if not given -- pass them, pinned, from a loop that must not allocate at all.  The C call only enqueues on `stream`;
+    with sync=True (default) this wrapper waits for the stream before it returns.  Calls that overlap on the GPU race on the
+    shared staging array."""
+    _require_cuda()
+    lib = load_library()
+    n = S_or_F.numel()
+    _same_len(n, K=K, tau=tau, P=P, flag=flag, r=r, q=q)
+    if out is None:
+        out = (torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.float64), torch.empty(n, dtype=torch.uint8))
+    _same_len(n, **{f"out[{i}]": t for i, t in enumerate(out)})
+    sigma, vega, status = out
+    inp = _Inputs(_host(S_or_F, "S_or_F"), _host(K, "K"), _host(tau, "tau"), _host(r, "r"), _host(q, "q"),
+                  _host(P, "P"), _host(flag, "flag"))
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    _check(lib.pivot_iv_forward_host_static(C.byref(inp), n, _host(sigma, "sigma"), _host(vega, "vega"),
+                                            _host(status, "status", torch.uint8), int(stream.cuda_stream)))
+    if sync:
+        stream.synchronize()
+    return sigma, vega, status
 
 
 class ShardedPipeline:

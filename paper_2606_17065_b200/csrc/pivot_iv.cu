@@ -828,6 +828,7 @@ const char* pivot_iv_strerror(int code) {
     case PIVOT_ERR_MIXED_RQ: return "r and q must both be NULL (Black-76) or both non-NULL (BSM)";
     case PIVOT_ERR_CUDA: return "CUDA runtime error";
     case PIVOT_ERR_BAD_ARG: return "invalid argument";
+    case PIVOT_ERR_STATIC_MAX: return "n exceeds PIVOT_STATIC_MAX_ROWS (65536), the capacity of the static staging of pivot_iv_forward_host_static";
     default: return "unknown pivot_iv error code";
   }
 }
@@ -973,6 +974,75 @@ int pivot_iv_forward_backward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* 
                                    double vega_floor, int mode, int64_t n, double* sigma, double* vega,
                                    uint8_t* status, double* grad_P) {
   return pipeline_run(p, in, grad_sigma, vega_floor, mode, true, n, sigma, vega, status, grad_P);
+}
+
+}  // extern "C"
+
+// ===============================================================================================================
+// pivot_iv_forward_host_static: the host-array forward call for callers that must not allocate (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc).  The device staging that a pipeline object obtains
+// from cudaMalloc is here a file-scope array, held by every GPU that loads the library until the process exits:
+// PIVOT_STATIC_MAX_ROWS rows of 9 doubles (S_or_F, K, tau, r, q, P, flag, sigma, vega) + 1 status byte = 4,784,128 B.
+// In host code `g_static_stage` is a host-side stand-in for the symbol, NOT a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+// Nothing in the array has to start at zero: every input byte the kernel reads is written by this call's own H2D copies
+// first, and the kernel writes all n rows of the three outputs before they are copied back; rows n ... MAX keep the last
+// call's contents and are never read.  Every call shares the array, so two calls that overlap on the GPU (different
+// streams, no dependency between them) race; calls on one stream are ordered by the stream.
+// ===============================================================================================================
+static __device__ __align__(256) unsigned char g_static_stage[(size_t)PIVOT_STATIC_MAX_ROWS * (9 * sizeof(double) + 1)];
+
+namespace {
+
+// device address of g_static_stage on the CURRENT device (looked up once per device ordinal, then cached)
+int static_stage_address(unsigned char** out) {
+  static std::atomic<unsigned char*> cache[kMaxDevices];
+  int dev = 0;
+  PIVOT_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev >= 0 && dev < kMaxDevices) {
+    unsigned char* c = cache[dev].load(std::memory_order_acquire);
+    if (c) { *out = c; return PIVOT_OK; }
+  }
+  unsigned char* ptr = nullptr;
+  PIVOT_CUDA_TRY(cudaGetSymbolAddress((void**)&ptr, g_static_stage));
+  if (!ptr) return PIVOT_ERR_CUDA;
+  if (dev >= 0 && dev < kMaxDevices) cache[dev].store(ptr, std::memory_order_release);
+  *out = ptr;
+  return PIVOT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pivot_iv_forward_host_static(const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega, uint8_t* status,
+                                 pivot_iv_stream stream) {
+  if (!in) return PIVOT_ERR_NULL;
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if (n > PIVOT_STATIC_MAX_ROWS) return PIVOT_ERR_STATIC_MAX;
+  if ((in->r == nullptr) != (in->q == nullptr)) return PIVOT_ERR_MIXED_RQ;
+  if (n == 0) return PIVOT_OK;
+  if (!in->S_or_F || !in->K || !in->tau || !in->P || !in->flag || !sigma || !vega || !status) return PIVOT_ERR_NULL;
+  unsigned char* stage = nullptr;
+  const int rc0 = static_stage_address(&stage);
+  if (rc0 != PIVOT_OK) return rc0;
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  double* d[9];
+  for (int k = 0; k < 9; ++k) d[k] = reinterpret_cast<double*>(stage) + (size_t)k * PIVOT_STATIC_MAX_ROWS;
+  uint8_t* dst = stage + (size_t)9 * PIVOT_STATIC_MAX_ROWS * sizeof(double);
+  const bool bsm = in->r != nullptr;
+  const size_t bytes = (size_t)n * sizeof(double);
+  const double* src[7] = {in->S_or_F, in->K, in->tau, in->r, in->q, in->P, in->flag};
+  for (int k = 0; k < 7; ++k)
+    if (src[k]) PIVOT_CUDA_TRY(cudaMemcpyAsync(d[k], src[k], bytes, cudaMemcpyHostToDevice, s));
+  const pivot_iv_inputs din{d[0], d[1], d[2], bsm ? d[3] : nullptr, bsm ? d[4] : nullptr, d[5], d[6]};
+  // an explicit organisation: the default call's probe + graph launch starts far above PIVOT_STATIC_MAX_ROWS anyway
+  const int rc = forward_impl(&din, n, d[7], d[8], dst, nullptr, s, PIVOT_FWD_COMPACT);
+  if (rc != PIVOT_OK) return rc;
+  PIVOT_CUDA_TRY(cudaMemcpyAsync(sigma, d[7], bytes, cudaMemcpyDeviceToHost, s));
+  PIVOT_CUDA_TRY(cudaMemcpyAsync(vega, d[8], bytes, cudaMemcpyDeviceToHost, s));
+  PIVOT_CUDA_TRY(cudaMemcpyAsync(status, dst, (size_t)n, cudaMemcpyDeviceToHost, s));
+  return PIVOT_OK;
 }
 
 }  // extern "C"

@@ -35,7 +35,7 @@ def test_every_declared_symbol_is_exported(lib):
 
 def test_version_and_strerror(lib):
     assert pv.pivot_iv_version() == 100
-    for code in range(0, -8, -1):
+    for code in range(0, -9, -1):
         assert "unknown" not in pv.pivot_iv_strerror(code)
     assert "unknown" in pv.pivot_iv_strerror(-99)
 
