@@ -716,7 +716,8 @@ __device__ __forceinline__ double householder_step(double x, double s, double p1
     } else {
       const bool want_W = kind == KIND_LOWER;
       double R = w.Wd;
-      if (want_W != w.have_W) R = fma(exp_fast(0.5 * x) * kSqrt2Pi, exp_fast(w.E), -w.Wd);   // rare
+      // rare; one exponential of the summed exponent (relative error |x/2 + E| 2^-53 <= 1e-13: seed grade)
+      if (want_W != w.have_W) R = fma(kSqrt2Pi, exp_fast(fma(0.5, x, w.E)), -w.Wd);
       const double L = kLnPhi0 - w.E + log_seed(R);
       const float u = __double2float_rn(s * rcp_raw(R));   // s/W or s/Wbar: O(h^2 + s^2)
       if (want_W) {
