@@ -234,59 +234,133 @@ loss_price_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, int6
 }
 
 // eq.(12), fused: price node P_model(sigma_hat), V_hat  ->  P~ (model price on the gate, the sentinel P* off it)  ->  the LBR
-// inversion (lbr_row, the forward kernel's own per-row arithmetic)  ->  weighted residual and, GRAD, its gradient by
-// eq.(17) -- all in registers, one pass over the inputs, no workspace.
+// inversion (the forward kernel's own per-row arithmetic: lbr_prelude, lbr_normalise, lbr_seed, lbr_refine)  ->  weighted
+// residual and, GRAD, its gradient by eq.(17) -- one pass over the inputs, no HBM workspace.
 //   MODE = PIVOT_RT_GATED: out += { sum w (sigma_rt - sigma*)^2, sum w, rows used },  w = V_hat^2 / (V_hat^2 + floor^2) (eq.(10));
 //       grad[i] = grad_scale { [on the gate] w 2 (sigma_rt - sigma*) MASK(1/V_rt) V_hat  +  w'(V_hat) (sigma_rt - sigma*)^2 V_hat' },
 //       w' = 2 V floor^2 / (V^2 + floor^2)^2,  V_hat' = dV/dsigma = V_hat d1 d2 / sigma_hat;  0 for rows the sum skips.
 //   MODE = PIVOT_RT_NAIVE (no gate, no sentinel, no sanitisation): out += { sum (sigma_rt - sigma*)^2, rows, rows };
 //       grad[i] = grad_scale STRICT(2 (sigma_rt - sigma*), V_rt; floor) V_hat -- NaN wherever the inverse channel is singular.
+// Organisation: each warp walks blocks of 32 consecutive rows (grid-stride).  Pass 1 (every row, coalesced): price node, P~ and
+// the status prelude of the inversion; a row the prelude finishes is accounted for at once, a row that needs the solver is
+// pushed on a per-warp stack in shared memory (U, O, B, tau, sigma*, V_hat, the vomma term, row index: 64 B/row, 72 B in BSM
+// mode).  As soon as the stack holds 32 rows the warp solves its top 32, one per lane: FULL warps whatever share of the rows
+// solves (in a single pass the inversion ran at 16 of 32 lanes on the mixed workload); what is left is flushed after the warp's
+// last block.  Warp-synchronous: no CTA barrier but the one of the final sum.
+constexpr int kRtCap = 64;   // stack capacity per warp: at most 31 rows left over + one block of 32
+
 template <bool BSM, int MODE, bool GRAD>
 __global__ void __launch_bounds__(kEwThreads, PIVOT_RT_MIN_CTAS)
 loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, const double* __restrict__ sigma_star,
                       double floor_, int64_t n, double* __restrict__ out, double* __restrict__ grad, double grad_scale) {
+  constexpr int kWarps = kEwThreads / 32;
+  __shared__ double qU[kWarps][kRtCap], qO[kWarps][kRtCap], qB[kWarps][kRtCap], qT[kWarps][kRtCap], qS[kWarps][kRtCap],
+      qV[kWarps][kRtCap], qG[kWarps][kRtCap], qD[BSM ? kWarps : 1][BSM ? kRtCap : 1];
+  __shared__ long long qI[kWarps][kRtCap];   // row index; bit 62: rare row (exact prelude), bit 61: on the gate
   double acc = 0.0, wsum = 0.0, cnt = 0.0;
   const double f2 = floor_ * floor_;
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
-    const double S = __ldcs(in.S_or_F + i), K = __ldcs(in.K + i), tau = __ldcs(in.tau + i), flag = __ldcs(in.flag + i);
-    const double sh = __ldcs(sigma_hat + i), ss = __ldcs(sigma_star + i);
-    double pm, vh, dd;
-    black_row<BSM>(S, K, tau, r, q, sh, flag, pm, vh, &dd);
-    const bool usable = is_fin(pm) && is_fin(vh) && is_fin(ss);     // a non-finite sigma_hat gives a NaN price
-    double g = 0.0;
-    if (MODE == PIVOT_RT_NAIVE) {
-      if (!usable) {
-        acc += canonical_nan(); cnt += 1.0; g = canonical_nan();
-      } else {
-        const RowOut o = lbr_row<BSM, 2, false, true>(S, K, tau, r, q, pm, flag);
-        const double d = o.sigma - ss;
-        acc = fma(d, d, acc); cnt += 1.0;
-        const double up = 2.0 * d;
-        const bool on = (o.status == PIVOT_ST_OK) && (fabs(o.vega) > floor_);
-        g = grad_scale * ((on ? __ddiv_rn(up, o.vega) : ((up == 0.0) ? 0.0 : canonical_nan())) * vh);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t nblocks = (n + 31) >> 5;
+  const int64_t wstride = (int64_t)gridDim.x * kWarps;
+  int64_t blk = (int64_t)blockIdx.x * kWarps + warp;
+  int count = 0;   // rows on the warp's stack (warp-uniform)
+  for (;;) {
+    const bool more = blk < nblocks;   // warp-uniform
+    if (more) {
+      // ---- pass 1: one row per lane
+      const int64_t i = (blk << 5) + lane;
+      blk += wstride;
+      bool push = false;
+      double eU = 0.0, eO = 0.0, eB = 0.0, eD = 1.0, eT = 0.0, eS = 0.0, eV = 0.0, eG = 0.0;
+      long long eI = i;
+      if (i < n) {
+        const double r = BSM ? __ldcs(in.r + i) : 0.0, q = BSM ? __ldcs(in.q + i) : 0.0;
+        const double S = __ldcs(in.S_or_F + i), K = __ldcs(in.K + i), tau = __ldcs(in.tau + i), flag = __ldcs(in.flag + i);
+        const double sh = __ldcs(sigma_hat + i), ss = __ldcs(sigma_star + i);
+        double pm, vh, dd;
+        black_row<BSM>(S, K, tau, r, q, sh, flag, pm, vh, &dd);
+        const bool usable = is_fin(pm) && is_fin(vh) && is_fin(ss);     // a non-finite sigma_hat gives a NaN price
+        double g = 0.0, pt = pm;
+        bool on = true;
+        if (MODE == PIVOT_RT_NAIVE) {
+          if (!usable) { acc += canonical_nan(); cnt += 1.0; g = canonical_nan(); }
+        } else if (usable) {
+          on = fabs(vh) > floor_;
+          if (!on) pt = __ldcs(in.P + i);
+        }
+        if (usable) {
+          Prelude p = lbr_prelude<BSM>(S, K, tau, r, q, pt, flag);
+          const bool rare = p.status == 5;
+          if (rare) p = lbr_prelude_exact<BSM>(S, K, tau, r, q, pt, flag);
+          push = p.status == 0;
+          if (push) {
+            eU = p.U; eO = p.O; eB = p.B; eD = p.D; eT = tau; eS = ss; eV = vh;
+            eI |= (rare ? (1LL << 62) : 0LL) | (on ? (1LL << 61) : 0LL);
+            if (MODE == PIVOT_RT_GATED && GRAD) {
+              const double den = fma(vh, vh, f2);
+              const double wp = (den > 0.0) ? 2.0 * vh * f2 / (den * den) : 0.0;
+              eG = wp * ((sh > 0.0) ? vh * dd / sh : 0.0);   // w'(V_hat) V_hat'
+            }
+          } else if (MODE == PIVOT_RT_NAIVE) {
+            // the inversion stops at the prelude: sigma_rt = 0 (AT_INTRINSIC) or NaN, no usable vega
+            const double d = ((p.status == 4) ? 0.0 : canonical_nan()) - ss;
+            acc = fma(d, d, acc); cnt += 1.0;
+            g = grad_scale * (((2.0 * d == 0.0) ? 0.0 : canonical_nan()) * vh);
+          }
+        }
+        if (GRAD && !push) __stcs(grad + i, g);
       }
-      wsum = cnt;
-    } else if (usable) {
-      const bool on = fabs(vh) > floor_;
-      const RowOut o = lbr_row<BSM, 2, false, true>(S, K, tau, r, q, on ? pm : __ldcs(in.P + i), flag);
-      if (o.status == PIVOT_ST_OK) {
-        const double v2 = vh * vh, den = v2 + f2;
-        const double w = v2 / den;
-        const double d = o.sigma - ss;
-        acc = fma(w * d, d, acc); wsum += w; cnt += 1.0;
-        if (GRAD) {
-          const double wp = (den > 0.0) ? 2.0 * vh * f2 / (den * den) : 0.0;
-          const double vomma = (sh > 0.0) ? vh * dd / sh : 0.0;
-          double gi = wp * d * d * vomma;
-          if (on && fabs(o.vega) > floor_) gi += w * __ddiv_rn(2.0 * d, o.vega) * vh;
+      const unsigned m = __ballot_sync(0xffffffffu, push);
+      if (push) {
+        const int e = count + __popc(m & ((1u << lane) - 1u));
+        qU[warp][e] = eU; qO[warp][e] = eO; qB[warp][e] = eB; qT[warp][e] = eT; qS[warp][e] = eS; qV[warp][e] = eV;
+        if (MODE == PIVOT_RT_GATED && GRAD) qG[warp][e] = eG;
+        if (BSM) qD[warp][e] = eD;
+        qI[warp][e] = eI;
+      }
+      count += __popc(m);
+      __syncwarp();
+    }
+    if (count >= 32 || (!more && count > 0)) {
+      // ---- pass 2: the top min(count, 32) rows of the stack, one per lane
+      const int take = count < 32 ? count : 32;
+      count -= take;
+      if (lane < take) {
+        const int e = count + lane;
+        const long long ei = qI[warp][e];
+        const bool rare = (ei >> 62) & 1, on = (ei >> 61) & 1;
+        const int64_t i = ei & ((1LL << 61) - 1);
+        const double tau = qT[warp][e], ss = qS[warp][e], vh = qV[warp][e];
+        const Norm nm = lbr_normalise(qU[warp][e], qO[warp][e], qB[warp][e], rare);
+        const Seed sd = lbr_seed<false>(nm.qrel, nm.beta, nm.bbar, nm.bmax);
+        const NormSolve ns = lbr_refine<2, false, true>(sd.x, sd.s, sd.p1, sd.p2, sd.kind);
+        const double rinv = rare ? rsqrt(tau) : rsqrt_c3(tau);   // as lbr_row
+        const double sig = ns.s * rinv;
+        const double veg = (BSM ? qD[warp][e] * nm.rootFK : nm.rootFK) * ns.vfin * (tau * rinv);
+        const double d = sig - ss;
+        double g;
+        if (MODE == PIVOT_RT_NAIVE) {
+          acc = fma(d, d, acc); cnt += 1.0;
+          const double up = 2.0 * d;
+          g = grad_scale * (((fabs(veg) > floor_) ? __ddiv_rn(up, veg) : ((up == 0.0) ? 0.0 : canonical_nan())) * vh);
+        } else {
+          const double v2 = vh * vh, den = v2 + f2;
+          const double w = v2 / den;
+          acc = fma(w * d, d, acc); wsum += w; cnt += 1.0;
+          double gi = 0.0;
+          if (GRAD) {
+            gi = qG[warp][e] * (d * d);
+            if (on && fabs(veg) > floor_) gi += w * __ddiv_rn(2.0 * d, veg) * vh;
+          }
           g = grad_scale * gi;
         }
+        if (GRAD) __stcs(grad + i, g);
       }
+      __syncwarp();
     }
-    if (GRAD) __stcs(grad + i, g);
+    if (!more && count == 0) break;
   }
+  if (MODE == PIVOT_RT_NAIVE) wsum = cnt;
   block_add3(acc, wsum, cnt, out);
 }
 

@@ -239,6 +239,50 @@ def test_loss_gradients_match_oracle(bsm):
     assert np.isnan(sums_n[0].item())                     # the NaN sigma_hat rows poison the naive sum
 
 
+@pytest.mark.parametrize("bsm", [False, True])
+def test_roundtrip_ragged_sizes_and_row_independence(bsm):
+    """The fused round trip walks 32-row blocks per warp and solves from a per-warp stack: sizes around the block and the stack
+    capacity (empty, 1, 31 ... 97 rows, a ragged tail, one size that wraps the grid-stride loop) must give, row for row, the
+    bits of the full-size call (a row's arithmetic does not depend on where it sits in a stack), and sums that match the
+    oracle's on the same slice; mixed rows (config 4: most rows never reach the solver) and BSM chains (all do)."""
+    cfg = wl.config2(days=1, expiries=4, strikes=2000, seed=71) if bsm else wl.config4(1_300_000, seed=72)
+    d, c = to_device(cfg), to_numpy(cfg)
+    n = c["K"].size
+    names = ("SorF", "K", "tau", "P", "flag") + (("r", "q") if bsm else ())
+    sstar, _, _ = pv.pivot_iv_forward(*[d[k] for k in KEYS], r=d.get("r"), q=d.get("q"))
+    sstar_h = np.where(np.isfinite(sstar.cpu().numpy()), sstar.cpu().numpy(), 0.25)
+    rng = np.random.default_rng(9)
+    sig_hat = np.where(sstar_h > 0, sstar_h, 0.3) * (1 + 0.05 * rng.standard_normal(n))
+    sig_hat[::613] = np.nan
+    sh, ss = torch.from_numpy(sig_hat).cuda(), torch.from_numpy(sstar_h).cuda()
+    floor = 1e-6
+
+    def call(m, mode):
+        a = [d[k][:m] for k in names[:5]]
+        rq = dict(r=d["r"][:m], q=d["q"][:m]) if bsm else {}
+        sums, g = pv.pivot_iv_loss_roundtrip(*a, sh[:m], ss[:m], floor, mode=mode, grad_scale=0.5, **rq)
+        return sums.cpu().numpy(), g.cpu().numpy()
+
+    for mode in (pv.RT_GATED, pv.RT_NAIVE):
+        sums_full, g_full = call(n, mode)
+        assert g_full.shape == (n,)
+        for m in (0, 1, 31, 32, 33, 63, 64, 65, 97, 1000, 8191, 300_001):
+            m = min(m, n)
+            sums, g = call(m, mode)
+            assert g.shape == (m,)
+            assert np.array_equal(g.view(np.int64), g_full[:m].view(np.int64)), (mode, m)
+            if mode == pv.RT_GATED and 0 < m <= 8191:
+                ah = [c[k][:m] for k in names[:5]]
+                rqh = dict(r=c["r"][:m], q=c["q"][:m]) if bsm else {}
+                ref = po.loss_roundtrip(*ah, sig_hat[:m], sstar_h[:m], floor, **rqh)
+                assert abs(sums[2] - ref[2]) <= 1
+                if sums[2] == ref[2]:
+                    assert sums[1] == pytest.approx(ref[1], rel=1e-9, abs=1e-300)
+                    assert sums[0] == pytest.approx(ref[0], rel=1e-8, abs=1e-300)
+            if m == 0:
+                assert (sums == 0).all()
+
+
 def test_nan_poisoning_diagnostic():
     """PAPER.md:404-428 (App. B.2, Fig.6): on the low_vega_tail chain (N = 65,536, seed 31, ~91 % of rows |V| <= 1e-14) the
     naive composition poisons every row of the singular set within one Adam step and never recovers; the gated objective
