@@ -186,6 +186,52 @@ def test_rational_cubic_end_conditions():
     assert np.all(np.diff(y) > 0)
 
 
+def _shape_ok(kind, H, yl, yr, dl, dr, r, m=4001):
+    u = np.linspace(0.0, 1.0, m)
+    y = po.rational_cubic(u, H, yl, yr, dl, dr, r)
+    if not np.all(np.isfinite(y)):
+        return False
+    if kind == "monotone":
+        return bool(np.all(np.diff(y) > 0))
+    d2 = np.diff(y, 2)
+    tol = 1e-13 * np.max(np.abs(y))
+    return bool(np.all(d2 >= -tol)) if kind == "convex" else bool(np.all(d2 <= tol))
+
+
+def test_shape_floor_is_the_smallest_shape_preserving_control():
+    """min_control (the floor under every fitted control parameter) pinned by brute force on the interpolant itself,
+    not by its formula: for convex / concave data the floor must be the smallest r whose rational cubic keeps the shape on a
+    fine grid (found by bisection on r: the second derivative at one end changes sign there), on data sets in which each of the
+    two ratio terms is the binding one; for monotone data with an inflection (where the (dl + dr)/Delta term binds) the floor
+    keeps the interpolant monotone and a control of a tenth of that size does not.  A dropped or mis-signed term fails one of these."""
+    cases = [("convex", 1.0, 0.0, 1.0, 0.2, 1.1),     # dr close to Delta: |dr - dl| / (dr - Delta) binds
+             ("convex", 0.7, 0.3, 1.0, 0.9, 4.0),     # dl close to Delta: |dr - dl| / (Delta - dl) binds
+             ("convex", 2.0, -1.0, 3.0, 0.5, 3.0),
+             ("concave", 1.0, 0.0, 1.0, 3.0, 0.8),
+             ("concave", 0.5, 2.0, 2.6, 1.3, 0.1)]
+    binding = set()
+    for kind, H, yl, yr, dl, dr in cases:
+        Delta = (yr - yl) / H
+        rmin = po.control_fit(0, H, yl, yr, dl, dr, -1e300 if Delta > dl else 1e300, floor_it=True)   # fitted r -> -inf: the floor
+        assert rmin == po.control_fit(1, H, yl, yr, dl, dr, -1e300 if dr > Delta else 1e300, floor_it=True)
+        assert _shape_ok(kind, H, yl, yr, dl, dr, rmin * (1 + 1e-6))
+        lo, hi = 0.0, rmin * (1 + 1e-6)           # bisection for the smallest shape-preserving r
+        assert not _shape_ok(kind, H, yl, yr, dl, dr, lo + 1e-3)
+        for _ in range(60):
+            mid = 0.5 * (lo + hi)
+            lo, hi = (lo, mid) if _shape_ok(kind, H, yl, yr, dl, dr, mid) else (mid, hi)
+        assert hi == pytest.approx(rmin, rel=2e-3), (kind, H, yl, yr, dl, dr, hi, rmin)
+        binding.add(abs(dr - Delta) < abs(Delta - dl))
+    assert binding == {True, False}
+    # monotone data with an inflection: slopes on both sides above the secant slope
+    for H, yl, yr, dl, dr in [(1.0, 0.0, 1.0, 2.0, 2.0), (0.4, 1.0, 1.2, 1.5, 0.9), (1.0, 0.0, 1.0, 5.0, 5.0)]:
+        Delta = (yr - yl) / H
+        rmin = po.control_fit(0, H, yl, yr, dl, dr, 1e300 if Delta < dl else -1e300, floor_it=True)
+        assert rmin >= (dl + dr) / Delta * (1 - 1e-12)
+        assert _shape_ok("monotone", H, yl, yr, dl, dr, rmin)
+        assert not _shape_ok("monotone", H, yl, yr, dl, dr, 0.1 * rmin)   # far below the floor the interpolant overshoots
+
+
 def test_seed_transform_end_derivatives():
     """f_low, f_up and their first/second derivatives w.r.t. beta vs mpmath differentiation of f(s(beta))."""
     for x, s in [(-0.4, 0.5), (-2.0, 1.2), (-4.5, 2.0)]:
@@ -265,6 +311,37 @@ def test_truth_solver_against_mpmath_root():
             return th * (Fi * mp_Phi(th * d1) - Ki * mp_Phi(th * d2)) - mp.mpf(float(P[i]))
         ref = mp.findroot(price, mp.mpf(float(sig[i])), tol=1e-40, maxsteps=100)
         assert tr[i] == pytest.approx(float(ref), rel=2 * EPS)
+
+
+def test_truth_solver_bsm_branch_against_mpmath_root_of_eq2():
+    """The (S, K, tau, r, q) branch of the __float128 bisection pinned by mpmath.findroot on the literal SPOT form of eq.(2)
+    (PAPER.md:55-57): theta (S e^{-q tau} Phi(theta d1) - K e^{-r tau} Phi(theta d2)), d1 = (ln(S/K) + (r - q + sigma^2/2) tau) /
+    (sigma sqrt(tau)) -- a different arrangement from the forward / discount-factor form the oracle evaluates, so a wrong sign of
+    r or q, a missing discount factor or a swapped carry term shows; calls and puts, in and out of the money, r < q included."""
+    rng = np.random.default_rng(21)
+    n = 16
+    S = rng.lognormal(np.log(100.0), 0.2, n); K = S * rng.uniform(0.6, 1.5, n)
+    tau = np.exp(rng.uniform(np.log(5 / 365), np.log(2.5), n)); r = rng.uniform(-0.01, 0.08, n); q = rng.uniform(0.0, 0.06, n)
+    sig = rng.uniform(0.08, 0.9, n); flag = np.where(rng.random(n) < 0.5, 1.0, -1.0)
+    P = np.empty(n)
+    for i in range(n):
+        Si, Ki, Ti, ri, qi, th = (mp.mpf(float(v)) for v in (S[i], K[i], tau[i], r[i], q[i], flag[i]))
+        def price(v, Si=Si, Ki=Ki, Ti=Ti, ri=ri, qi=qi, th=th):
+            st = v * mp.sqrt(Ti); d1 = (mp.log(Si / Ki) + (ri - qi + v * v / 2) * Ti) / st; d2 = d1 - st
+            return th * (Si * mp.exp(-qi * Ti) * mp_Phi(th * d1) - Ki * mp.exp(-ri * Ti) * mp_Phi(th * d2))
+        P[i] = float(price(mp.mpf(float(sig[i]))))
+    tr = po.truth_iv(S, K, tau, P, flag, r=r, q=q)
+    assert (r < q).any() and (flag > 0).any() and (flag < 0).any()
+    for i in range(n):
+        Si, Ki, Ti, ri, qi, th = (mp.mpf(float(v)) for v in (S[i], K[i], tau[i], r[i], q[i], flag[i]))
+        def resid(v):
+            st = v * mp.sqrt(Ti); d1 = (mp.log(Si / Ki) + (ri - qi + v * v / 2) * Ti) / st; d2 = d1 - st
+            return th * (Si * mp.exp(-qi * Ti) * mp_Phi(th * d1) - Ki * mp.exp(-ri * Ti) * mp_Phi(th * d2)) - mp.mpf(float(P[i]))
+        ref = mp.findroot(resid, mp.mpf(float(sig[i])), tol=1e-40, maxsteps=100)
+        assert tr[i] == pytest.approx(float(ref), rel=2 * EPS), i
+        # and the oracle's own forward pass agrees with that root (conditioning: sigma moves by ~ eps P / (V sigma))
+        sg, vega, st_ = po.forward(S[i:i + 1], K[i:i + 1], tau[i:i + 1], P[i:i + 1], flag[i:i + 1], r=r[i:i + 1], q=q[i:i + 1])
+        assert st_[0] == 0 and abs(sg[0] / float(ref) - 1) <= 8 * EPS * (1 + P[i] / (vega[0] * float(ref)))
 
 
 def test_lbr_matches_float128_bisection_all_zones():
