@@ -45,12 +45,12 @@ FWD_BYTES = {"b76": 57, "bsm": 73}
 BWD_BYTES_PER_ROW = 25
 # Constants QUOTED from the ncu --set full captures of the committed kernels (profiles/r2*_ncu_full.md; config 4 mixed rows):
 NCU = {
-    "source": "profiles/r2d_forward_tile_ncu_full.md, profiles/r2d_backward_ncu_full.md (ncu --set full of this kernel, config 4)",
+    "source": "profiles/r2e_forward_tile_ncu_full.md, profiles/r2e_backward_ncu_full.md (ncu --set full of this kernel, config 4)",
     "fwd_dram_bytes_per_row": 56.2,          # dram__bytes_read.sum + dram__bytes_write.sum per row (40.0 read + 16.2 written)
     "fwd_issued_fp64_flops_per_row": 193.6,  # 2 DFMA + DADD + DMUL thread instructions per row
-    "fwd_fp64_pipe_busy_pct": 37.8,
-    "fwd_issue_active_pct": 68.1,
-    "fwd_warp_inst_per_row": 17.87,
+    "fwd_fp64_pipe_busy_pct": 38.9,
+    "fwd_issue_active_pct": 70.5,
+    "fwd_warp_inst_per_row": 18.00,
     "bwd_dram_bytes_per_row": 24.5,          # 17.0 read + 7.5 written
 }
 # per-call flop costs of the device fp64 math functions (static DFMA*2+DMUL+DADD counts of the sm_100a SASS of the
@@ -594,7 +594,7 @@ def main():
                              "note": "constants quoted from the ncu --set full capture of the committed kernel", "source": NCU["source"]},
                 "traffic": NCU["fwd_dram_bytes_per_row"] * n,
                 "traffic_source": "constant: dram__bytes_read.sum + dram__bytes_write.sum per row of the ncu --set full capture "
-                                  "named in `executed.source`, scaled to this launch's rows (40.0 B read + 16.5 B written per row; part of "
+                                  "named in `executed.source`, scaled to this launch's rows (40.0 B read + 16.2 B written per row; part of "
                                   "the 17 B written is still dirty in L2 when the kernel ends)",
                 "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x 1.965 GHz (DESIGN.md s7)",
                 "dfma_probe_tflops": probe_tflops,
@@ -629,7 +629,7 @@ def main():
                                               "hbm_frac": 56.0 * n / (ms_lp * 1e-3) / 1e9 / hbm_peak},
                      "loss_roundtrip_with_grad": {"ms": ms_lr, "rows_per_s": n / (ms_lr * 1e-3), "bytes_per_row": 64.0,
                                                   "hbm_frac": 64.0 * n / (ms_lr * 1e-3) / 1e9 / hbm_peak,
-                                                  "note": "one fused kernel: price node + LBR inversion + weighted residual + gradient"}}
+                                                  "note": "one fused kernel: price node -> per-warp stack in shared memory -> LBR inversion 32 rows at a time in full warps -> weighted residual + gradient"}}
         del sig_in
 
     sweep = configs = None
