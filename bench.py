@@ -451,7 +451,7 @@ def main():
         hgs = gsig.cpu().pin_memory()
         hout = (torch.empty(n, dtype=torch.float64).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory(),
                 torch.empty(n, dtype=torch.uint8).pin_memory(), torch.empty(n, dtype=torch.float64).pin_memory())
-        pipe = pv.Pipeline(chunk_rows=1 << 21, n_slots=4)
+        pipe = pv.Pipeline(chunk_rows=1 << 23, n_slots=4)
         ke = max(1, min(K, 3))
         pipe.forward_backward_host(*host, hgs, VEGA_FLOOR, pv.GATE_MASK, out=hout)
         barrier()
@@ -478,7 +478,7 @@ def main():
         lo = (torch.empty(m_l, dtype=torch.float64).pin_memory(), torch.empty(m_l, dtype=torch.float64).pin_memory(),
               torch.empty(m_l, dtype=torch.uint8).pin_memory())
         best = None
-        for chunk, slots in ((65536, 4), (1 << 19, 4)):
+        for chunk, slots in ((65536, 4), (1 << 19, 4), (1 << 20, 4)):
             lp = pv.Pipeline(chunk_rows=chunk, n_slots=slots)
             lp.forward_host(*lh, out=lo)
             barrier()

@@ -196,8 +196,10 @@ int pivot_iv_loss_roundtrip(const pivot_iv_inputs* in, const double* sigma_hat, 
 /* ---- host-buffer pipeline (the streaming label-generation setting: batches of rows, H2D included) ----
  * A pipeline owns `n_slots` device staging slots of `chunk_rows` rows each, one CUDA stream per slot and pinned
  * bounce buffers are NOT used: host arrays are copied directly (pin them for full PCIe speed).  The *_host calls split
- * the n rows into chunks, overlap H2D copy, kernels and D2H copy across slots, and return after the last byte of
- * output is in host memory (they synchronise).  Not thread-safe per pipeline object. */
+ * the n rows into chunks of at most `chunk_rows` rows (with chunk_rows > 2^19 the first chunks ramp up from 2^19 or
+ * chunk_rows/8 rows by doubling and the last ones halve what is left, so that the copies nothing overlaps stay short),
+ * overlap H2D copy, kernels and D2H copy across slots, and return after the last byte of output is in host memory (they
+ * synchronise).  Not thread-safe per pipeline object. */
 typedef struct pivot_iv_pipeline pivot_iv_pipeline;
 
 /* Creates a pipeline on CUDA device `device` (-1 = current).  chunk_rows > 0, 1 <= n_slots <= 8. */

@@ -236,6 +236,20 @@ def test_host_pipeline_matches_device_path():
     out = pipe.forward_host(*[c2[k] for k in KEYS], r=c2["r"], q=c2["q"])
     assert np.array_equal(out[0].numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
     pipe.close()
+    # chunks above 2^19 rows ramp up (2^19, 2^20, ...) and down again (the rest halved): every row still exactly once
+    big = wl.config4(5_000_003, seed=29)
+    db = to_device(big)
+    ref = gpu_forward(db)
+    gsb = torch.randn(5_000_003, dtype=torch.float64)
+    gPb = pv.pivot_iv_backward(gsb.cuda(), ref[1], ref[2], 1e-8, 0)
+    for chunk in (1 << 20, 1 << 22):
+        pipe = pv.Pipeline(chunk_rows=chunk, n_slots=3)
+        sb, vb, stb, gb = pipe.forward_backward_host(*[big[k].pin_memory() for k in KEYS], gsb.pin_memory(), 1e-8, 0)
+        pipe.close()
+        assert torch.equal(stb, ref[2].cpu())
+        assert np.array_equal(sb.numpy().view(np.uint64), ref[0].cpu().numpy().view(np.uint64))
+        assert np.array_equal(vb.numpy().view(np.uint64), ref[1].cpu().numpy().view(np.uint64))
+        assert np.array_equal(gb.numpy().view(np.uint64), gPb.cpu().numpy().view(np.uint64))
 
 
 def test_host_pipeline_matches_oracle():
