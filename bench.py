@@ -72,7 +72,10 @@ def _peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    """Samples nvidia-smi SM clocks and throttle reasons (every 100 ms).  Started BEFORE the warm-up so that nvidia-smi is already
+    running when the timed region begins (its start-up takes longer than a short timed region); each sample carries its host
+    arrival time, and stop(t0, t1, t2) keeps those of the timed region [t0, t1] and of the untimed tail (t1, t2] in which the
+    caller goes on running the same steps when the region was too short for five samples."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -91,9 +94,12 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append(line.strip())
+            self.rows.append((time.perf_counter(), line.strip()))
 
-    def stop(self):
+    def count_since(self, t0):
+        return sum(1 for ts, _ in list(self.rows) if ts >= t0)
+
+    def stop(self, t0=None, t1=None, t2=None):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -103,7 +109,10 @@ class ClockSampler:
             self.proc.kill()
         sm, mx, reasons = [], None, set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for r in self.rows:
+        n_in = n_tail = 0
+        for ts, r in self.rows:
+            if t0 is not None and not (t0 <= ts <= (t2 if t2 is not None else t1)):
+                continue
             f = [x.strip() for x in r.split(",")]
             if len(f) < 6:
                 continue
@@ -111,11 +120,15 @@ class ClockSampler:
                 sm.append(float(f[0])); mx = float(f[1])
             except ValueError:
                 continue
+            if t1 is not None and ts > t1:
+                n_tail += 1
+            else:
+                n_in += 1
             for nm, v in zip(names, f[2:6]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "samples": len(sm), "samples_in_timed_region": n_in, "samples_in_untimed_tail_same_steps": n_tail}
 
 
 def _flops_per_row_from_counts(counts, rows):
@@ -407,6 +420,8 @@ def main():
         forward()
         pv.pivot_iv_backward(gsig, out[1], out[2], VEGA_FLOOR, pv.GATE_MASK, out=gP, stream=stream)
 
+    sampler = ClockSampler(local)
+    sampler.start()   # before the warm-up: see ClockSampler
     for _ in range(W):
         step()
 
@@ -415,10 +430,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    sampler = ClockSampler(local)
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(K)]
     barrier()
-    sampler.start()
+    t_host0 = time.perf_counter()
     t_begin = torch.cuda.Event(enable_timing=True); t_end = torch.cuda.Event(enable_timing=True)
     t_begin.record(stream)
     for i in range(K):
@@ -429,7 +443,13 @@ def main():
         ev[i][2].record(stream)
     t_end.record(stream)
     barrier()
-    clocks = sampler.stop()
+    t_host1 = time.perf_counter()
+    # a timed region shorter than five sampling periods: the same steps go on, untimed, until five samples exist (at most 1.5 s)
+    while sampler.proc is not None and sampler.count_since(t_host0) < 5 and time.perf_counter() - t_host1 < 1.5:
+        for _ in range(10):
+            step()
+        torch.cuda.synchronize()
+    clocks = sampler.stop(t_host0, t_host1, time.perf_counter())
     total_ms = t_begin.elapsed_time(t_end)
     fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
     bwd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
