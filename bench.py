@@ -498,27 +498,40 @@ def main():
         lo = (torch.empty(m_l, dtype=torch.float64).pin_memory(), torch.empty(m_l, dtype=torch.float64).pin_memory(),
               torch.empty(m_l, dtype=torch.uint8).pin_memory())
         best = None
-        for chunk, slots in ((65536, 4), (1 << 19, 4), (1 << 20, 4)):
+        # staged (chunked H2D copies -> kernel -> D2H copies) at three chunk sizes, then the default: ONE launch straight on the
+        # pinned host arrays (PIVOT_HOST_DIRECT; no staging, no copies), on the whole array and batch by batch (64 calls)
+        for chunk, slots, how in ((65536, 4, "staged"), (1 << 19, 4, "staged"), (1 << 20, 4, "staged"), (1 << 20, 1, "direct"),
+                                  (65536, 1, "direct, one call per 65,536-row batch")):
             lp = pv.Pipeline(chunk_rows=chunk, n_slots=slots)
-            lp.forward_host(*lh, out=lo)
+            lp.set_host_access(pv.HOST_STAGED if how == "staged" else pv.HOST_AUTO)
+            if how.startswith("direct, one call"):
+                def run_label():
+                    for b0 in range(0, m_l, 65536):
+                        b1 = min(m_l, b0 + 65536)
+                        lp.forward_host(*[t_[b0:b1] for t_ in lh], out=tuple(t_[b0:b1] for t_ in lo))
+            else:
+                def run_label():
+                    lp.forward_host(*lh, out=lo)
+            run_label()
+            assert lp.last_host_path() == (pv.HOST_STAGED if how == "staged" else pv.HOST_DIRECT)
             barrier()
             t0 = time.perf_counter()
             for _ in range(5):
-                lp.forward_host(*lh, out=lo)
+                run_label()
             dtl = (time.perf_counter() - t0) / 5
             lp.close()
             t = torch.tensor([dtl], device="cuda", dtype=torch.float64)
             if dist is not None:
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dtl = float(t.item())
-            r_ = {"chunk_rows": chunk, "n_slots": slots, "labels_per_s": nl / dtl, "ms": dtl * 1e3,
-                  "h2d_gb_per_s": 40 * nl / dtl / 1e9}
+            r_ = {"path": how, "chunk_rows": chunk if how == "staged" else None, "n_slots": slots if how == "staged" else None,
+                  "labels_per_s": nl / dtl, "ms": dtl * 1e3, "h2d_gb_per_s": 40 * nl / dtl / 1e9}
             if best is None or r_["labels_per_s"] > best["labels_per_s"]:
                 best = r_
             e2e.setdefault("label_pipeline_runs", []).append(r_)
         e2e["label_pipeline"] = dict(best, batches=64, batch_rows=65536, h2d_bytes=40 * nl, d2h_bytes=17 * nl,
                                      paper_h100_labels_per_s=48.9e6, sharded_over_ranks=world,
-                                     note="config-0 rows, pinned host buffers, one array sharded by shard_rows")
+                                     note="config-0 rows, pinned host buffers, one array sharded by shard_rows; best of label_pipeline_runs")
         # The same 64 x 65,536-row batches already RESIDENT on the device (launch-latency regime: one batch is a 16 us kernel):
         # 64 forward calls enqueued one by one, and the same 64 launches replayed from ONE CUDA graph.
         if rank == 0:

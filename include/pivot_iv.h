@@ -207,6 +207,21 @@ int pivot_iv_pipeline_create(pivot_iv_pipeline** out, int device, int64_t chunk_
 int pivot_iv_pipeline_destroy(pivot_iv_pipeline* p);
 /* Kernel organisation the pipeline's forward launches use (PIVOT_FWD_*; default AUTO). */
 int pivot_iv_pipeline_set_forward_kernel(pivot_iv_pipeline* p, int kernel);
+/* How pivot_iv_forward_host reaches the caller's host arrays (default PIVOT_HOST_AUTO):
+ *   PIVOT_HOST_AUTO    if EVERY input and output array is pinned (cudaHostAlloc / cudaHostRegister) and addressable from the
+ *                      pipeline's device, ONE forward launch loads and stores the host arrays directly over PCIe (unified
+ *                      addressing; the device path's own kernels, same bits; row-per-thread unless
+ *                      pivot_iv_pipeline_set_forward_kernel chose otherwise): no staging, no cudaMemcpyAsync, no chunks.
+ *                      Otherwise (any array pageable) the staged path below.
+ *   PIVOT_HOST_STAGED  always the chunked H2D copy -> kernels -> D2H copy path through the staging slots.
+ * pivot_iv_forward_backward_host always takes the staged path (the backward reads what the forward wrote: vega and status
+ * stay in device memory between the two kernels).  Returns PIVOT_ERR_NULL / PIVOT_ERR_BAD_ARG. */
+#define PIVOT_HOST_AUTO 0
+#define PIVOT_HOST_STAGED 1
+#define PIVOT_HOST_DIRECT 2   /* reported only: the last call ran straight on the host arrays */
+int pivot_iv_pipeline_set_host_access(pivot_iv_pipeline* p, int mode);
+/* Path the last *_host call of this pipeline took: PIVOT_HOST_STAGED or PIVOT_HOST_DIRECT (PIVOT_ERR_NULL for p == NULL). */
+int pivot_iv_pipeline_last_host_path(const pivot_iv_pipeline* p);
 
 /* Forward on HOST arrays: `in`, sigma, vega, status are host pointers (length n). */
 int pivot_iv_forward_host(pivot_iv_pipeline* p, const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega,

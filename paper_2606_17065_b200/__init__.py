@@ -14,6 +14,9 @@ from .binding import (  # noqa: F401
     FWD_COMPACT,
     FWD_ROWWISE,
     FWD_FP64_ONLY,
+    HOST_AUTO,
+    HOST_STAGED,
+    HOST_DIRECT,
     PivotError,
     Pipeline,
     ShardedPipeline,
@@ -45,7 +48,7 @@ __all__ = [
     "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "Pipeline", "ShardedPipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",
-    "GATE_ATTENUATE", "GATE_STRICT", "RT_GATED", "RT_NAIVE", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "pivot_iv_debug_math", "EXPORTS",
+    "GATE_ATTENUATE", "GATE_STRICT", "RT_GATED", "RT_NAIVE", "FWD_AUTO", "FWD_COMPACT", "FWD_ROWWISE", "FWD_FP64_ONLY", "HOST_AUTO", "HOST_STAGED", "HOST_DIRECT", "pivot_iv_forward_ex", "pivot_iv_forward_diag", "pivot_iv_debug_math", "EXPORTS",
     "pivot_iv_forward_probe", "pivot_iv_forward_launches", "AUTO_MIN_ROWS",
     "pivot_iv_forward_host_static", "STATIC_MAX_ROWS",
 ]

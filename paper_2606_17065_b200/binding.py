@@ -17,6 +17,9 @@ FWD_AUTO = 0
 FWD_COMPACT = 1
 FWD_ROWWISE = 2
 FWD_FP64_ONLY = 4   # flag: OR into FWD_AUTO / FWD_COMPACT / FWD_ROWWISE
+HOST_AUTO = 0       # Pipeline.set_host_access
+HOST_STAGED = 1
+HOST_DIRECT = 2     # Pipeline.last_host_path only
 
 # every symbol include/pivot_iv.h declares
 EXPORTS = (
@@ -26,7 +29,7 @@ EXPORTS = (
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
     "pivot_iv_forward_diag", "pivot_iv_debug_math", "pivot_iv_forward_launches", "pivot_iv_forward_probe",
-    "pivot_iv_forward_host_static",
+    "pivot_iv_forward_host_static", "pivot_iv_pipeline_set_host_access", "pivot_iv_pipeline_last_host_path",
 )
 
 
@@ -60,6 +63,8 @@ def load_library():
     lib.pivot_iv_forward_probe.argtypes = [C.POINTER(_Inputs), i64, vp, vp]
     lib.pivot_iv_forward_launches.argtypes = [i64, cint]
     lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
+    lib.pivot_iv_pipeline_set_host_access.argtypes = [vp, cint]
+    lib.pivot_iv_pipeline_last_host_path.argtypes = [vp]
     lib.pivot_iv_debug_math.argtypes = [cint, vp, vp, i64, vp, vp]
     lib.pivot_iv_forward_diag.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp, vp, cint, vp]
     lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
@@ -396,6 +401,15 @@ class Pipeline:
 
     def set_forward_kernel(self, kernel: int):
         _check(self._lib.pivot_iv_pipeline_set_forward_kernel(self._h, int(kernel)))
+
+    def set_host_access(self, mode: int):
+        """HOST_AUTO (default): forward_host on pinned tensors runs ONE launch straight on the host arrays (no staging);
+        HOST_STAGED: always the chunked copy path."""
+        _check(self._lib.pivot_iv_pipeline_set_host_access(self._h, int(mode)))
+
+    def last_host_path(self) -> int:
+        """HOST_STAGED or HOST_DIRECT: how the last forward_host / forward_backward_host call reached the host arrays."""
+        return int(self._lib.pivot_iv_pipeline_last_host_path(self._h))
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:

@@ -839,6 +839,8 @@ struct pivot_iv_pipeline {
   int64_t chunk = 0;
   int nslots = 0;
   int fwd_kernel = PIVOT_FWD_AUTO;
+  int host_access = PIVOT_HOST_AUTO;
+  int last_path = PIVOT_HOST_STAGED;   // path of the last *_host call: PIVOT_HOST_STAGED or PIVOT_HOST_DIRECT
   cudaStream_t streams[8] = {};
   double* dbl[8] = {};   // per slot: 11 fp64 arrays of `chunk` rows: S,K,tau,r,q,P,flag,sigma,vega,gs,gP
   uint8_t* st[8] = {};   // per slot: status bytes
@@ -853,6 +855,49 @@ namespace {
       return PIVOT_ERR_CUDA;                    \
     }                                           \
   } while (0)
+
+// Device alias of the pinned, device-accessible host range [h, h + bytes), or nullptr: pageable memory, memory the device cannot
+// reach, or a range that does not lie inside one pinned allocation (both ends are looked up and must map consistently).
+template <typename T>
+T* mapped_alias(T* h, size_t bytes) {
+  if (!h || bytes == 0) return nullptr;
+  cudaPointerAttributes a0{}, a1{};
+  const char* hb = reinterpret_cast<const char*>(h);
+  if (cudaPointerGetAttributes(&a0, hb) != cudaSuccess || cudaPointerGetAttributes(&a1, hb + bytes - 1) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return nullptr;
+  }
+  if (a0.type != cudaMemoryTypeHost || a1.type != cudaMemoryTypeHost || !a0.devicePointer || !a1.devicePointer) return nullptr;
+  if (static_cast<const char*>(a1.devicePointer) - static_cast<const char*>(a0.devicePointer) != (ptrdiff_t)(bytes - 1)) return nullptr;
+  return reinterpret_cast<T*>(a0.devicePointer);
+}
+
+// pivot_iv_forward_host without staging: ONE forward launch whose loads and stores go to the caller's pinned host arrays over
+// PCIe (unified addressing: the kernels are the device path's own).  No cudaMemcpyAsync, no chunks, both link directions busy
+// from one kernel: 4,194,304 labels 3.75 -> 3.40 ms, one 65,536-row batch 0.129 -> 0.069 ms (per-copy overhead gone).
+// `applied` says whether the path was taken (every array pinned and device-accessible); if so the return value is the call's.
+int pipeline_run_zero_copy(pivot_iv_pipeline* p, const pivot_iv_inputs* in, int64_t n, double* sigma, double* vega,
+                           uint8_t* status, bool* applied) {
+  *applied = false;
+  const size_t bytes = (size_t)n * sizeof(double);
+  pivot_iv_inputs din{mapped_alias(in->S_or_F, bytes), mapped_alias(in->K, bytes), mapped_alias(in->tau, bytes),
+                      mapped_alias(in->r, bytes), mapped_alias(in->q, bytes), mapped_alias(in->P, bytes),
+                      mapped_alias(in->flag, bytes)};
+  double* dsig = mapped_alias(sigma, bytes);
+  double* dveg = mapped_alias(vega, bytes);
+  uint8_t* dst = mapped_alias(status, (size_t)n);
+  const bool bsm = in->r != nullptr;
+  if (!din.S_or_F || !din.K || !din.tau || !din.P || !din.flag || (bsm && (!din.r || !din.q)) || !dsig || !dveg || !dst) return PIVOT_OK;
+  *applied = true;
+  // PCIe-bound whatever the organisation; the row-per-thread kernel streams more evenly (49 against 47 GB/s) -- an explicit
+  // choice of the caller is kept
+  const int flags = p->fwd_kernel & PIVOT_FWD_FP64_ONLY, org = p->fwd_kernel & ~PIVOT_FWD_FP64_ONLY;
+  const int kernel = ((org == PIVOT_FWD_AUTO) ? PIVOT_FWD_ROWWISE : org) | flags;
+  cudaStream_t s = p->streams[0];
+  int rc = forward_impl(&din, n, dsig, dveg, dst, nullptr, s, kernel);
+  if (cudaStreamSynchronize(s) != cudaSuccess) { (void)cudaGetLastError(); rc = PIVOT_ERR_CUDA; }
+  return rc;
+}
 
 int pipeline_run(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* gs, double floor_, int mode, bool bwd,
                  int64_t n, double* sigma, double* vega, uint8_t* status, double* gP) {
@@ -872,6 +917,16 @@ int pipeline_run(pivot_iv_pipeline* p, const pivot_iv_inputs* in, const double* 
   const bool bsm = in->r != nullptr;
   const int64_t C = p->chunk;
   int rc = PIVOT_OK;
+  if (!bwd && p->host_access == PIVOT_HOST_AUTO) {   // every array pinned and reachable from the device: no staging at all
+    bool applied = false;
+    rc = pipeline_run_zero_copy(p, in, n, sigma, vega, status, &applied);
+    if (applied) {
+      p->last_path = PIVOT_HOST_DIRECT;
+      (void)cudaSetDevice(prev);
+      return rc;
+    }
+  }
+  p->last_path = PIVOT_HOST_STAGED;
   // Chunks of more than 2^19 rows ramp up (2^19 or C/8 rows first, then doubling) and down again (halving what is left):
   // nothing overlaps the first chunk's H2D copies and the last chunk's D2H copies, so those two are kept short, while the
   // chunks in between stay large -- every cudaMemcpyAsync costs ~8 us of idle link (2^26 rows, forward + backward: 40 GB/s H2D
@@ -952,6 +1007,15 @@ int pivot_iv_pipeline_set_forward_kernel(pivot_iv_pipeline* p, int kernel) {
   p->fwd_kernel = kernel;
   return PIVOT_OK;
 }
+
+int pivot_iv_pipeline_set_host_access(pivot_iv_pipeline* p, int mode) {
+  if (!p) return PIVOT_ERR_NULL;
+  if (mode != PIVOT_HOST_AUTO && mode != PIVOT_HOST_STAGED) return PIVOT_ERR_BAD_ARG;
+  p->host_access = mode;
+  return PIVOT_OK;
+}
+
+int pivot_iv_pipeline_last_host_path(const pivot_iv_pipeline* p) { return p ? p->last_path : PIVOT_ERR_NULL; }
 
 int pivot_iv_pipeline_destroy(pivot_iv_pipeline* p) {
   if (!p) return PIVOT_OK;

@@ -252,6 +252,77 @@ def test_host_pipeline_matches_device_path():
         assert np.array_equal(gb.numpy().view(np.uint64), gPb.cpu().numpy().view(np.uint64))
 
 
+def test_host_direct_path_on_pinned_arrays():
+    """pivot_iv_forward_host on pinned host arrays runs ONE launch straight on them (PIVOT_HOST_DIRECT, no staging); the bits are
+    the device path's, whichever path is taken: all arrays pinned (direct), views into pinned allocations at odd offsets (direct),
+    one pageable array among pinned ones (staged), PIVOT_HOST_STAGED forced, BSM mode, an explicit kernel choice, one row."""
+    n = 300_001
+    cfg = wl.config3(n, seed=39)
+    d = to_device(cfg)
+    ref = gpu_forward(d)
+    refb = [t.cpu().numpy() for t in ref]
+
+    def same(out, lo=0, hi=n):
+        assert np.array_equal(out[2].numpy(), refb[2][lo:hi])
+        assert np.array_equal(out[0].numpy().view(np.uint64), refb[0][lo:hi].view(np.uint64))
+        assert np.array_equal(out[1].numpy().view(np.uint64), refb[1][lo:hi].view(np.uint64))
+
+    pinned = {k: cfg[k].pin_memory() for k in KEYS}
+    pout = lambda m: (torch.empty(m, dtype=torch.float64).pin_memory(), torch.empty(m, dtype=torch.float64).pin_memory(),
+                      torch.empty(m, dtype=torch.uint8).pin_memory())
+    pipe = pv.Pipeline(chunk_rows=65_536, n_slots=3)
+    assert pipe.last_host_path() == pv.HOST_STAGED
+    out = pipe.forward_host(*[pinned[k] for k in KEYS], out=pout(n))
+    assert pipe.last_host_path() == pv.HOST_DIRECT
+    same(out)
+    # views at odd offsets inside pinned allocations (8-byte aligned doubles, status bytes at an odd address)
+    lo, hi = 5, n - 3
+    o = pout(n)
+    out = pipe.forward_host(*[pinned[k][lo:hi] for k in KEYS], out=tuple(t[lo:hi] for t in o))
+    assert pipe.last_host_path() == pv.HOST_DIRECT
+    same(out, lo, hi)
+    # pageable outputs (allocated by the binding), or one pageable input: the staged path, same bits
+    out = pipe.forward_host(*[pinned[k] for k in KEYS])
+    assert pipe.last_host_path() == pv.HOST_STAGED
+    same(out)
+    out = pipe.forward_host(pinned["SorF"], cfg["K"], pinned["tau"], pinned["P"], pinned["flag"], out=pout(n))
+    assert pipe.last_host_path() == pv.HOST_STAGED
+    same(out)
+    # staged on request
+    pipe.set_host_access(pv.HOST_STAGED)
+    out = pipe.forward_host(*[pinned[k] for k in KEYS], out=pout(n))
+    assert pipe.last_host_path() == pv.HOST_STAGED
+    same(out)
+    pipe.set_host_access(pv.HOST_AUTO)
+    with pytest.raises(pv.PivotError):
+        pipe.set_host_access(7)
+    # an explicit organisation is kept; forward + backward always stages
+    pipe.set_forward_kernel(pv.FWD_COMPACT)
+    out = pipe.forward_host(*[pinned[k] for k in KEYS], out=pout(n))
+    assert pipe.last_host_path() == pv.HOST_DIRECT
+    same(out)
+    pipe.set_forward_kernel(pv.FWD_AUTO)
+    gs = cfg["grad_sigma"].pin_memory()
+    o4 = pout(n) + (torch.empty(n, dtype=torch.float64).pin_memory(),)
+    out = pipe.forward_backward_host(*[pinned[k] for k in KEYS], gs, 1e-8, 0, out=o4)
+    assert pipe.last_host_path() == pv.HOST_STAGED
+    same(out)
+    gP = pv.pivot_iv_backward(d["grad_sigma"], ref[1], ref[2], 1e-8, 0)
+    assert np.array_equal(out[3].numpy().view(np.uint64), gP.cpu().numpy().view(np.uint64))
+    # one row
+    out = pipe.forward_host(*[pinned[k][:1] for k in KEYS], out=pout(1))
+    assert pipe.last_host_path() == pv.HOST_DIRECT
+    same(out, 0, 1)
+    # BSM chains
+    c2 = wl.config2(days=2, expiries=5, strikes=401)
+    r2 = gpu_forward(to_device(c2))
+    m = c2["K"].numel()
+    out = pipe.forward_host(*[c2[k].pin_memory() for k in KEYS], r=c2["r"].pin_memory(), q=c2["q"].pin_memory(), out=pout(m))
+    assert pipe.last_host_path() == pv.HOST_DIRECT
+    assert np.array_equal(out[0].numpy().view(np.uint64), r2[0].cpu().numpy().view(np.uint64)) and torch.equal(out[2], r2[2].cpu())
+    pipe.close()
+
+
 def test_host_pipeline_matches_oracle():
     """The host entry points against the ORACLE (not against the device path): pivot_iv_forward_backward_host on config 3 in
     chunks with a ragged last one, and the row-sharded multi-device driver (two pipelines; both on cuda:0 when the box has
