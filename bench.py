@@ -486,7 +486,8 @@ def main():
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dt = float(t.item())
         e2e = {"value": world * n / dt, "unit": "rows/s", "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 25 * n,
-               "ms_per_step": dt * 1e3, "steps": ke, "api": "pivot_iv_forward_backward_host (pinned host buffers)"}
+               "ms_per_step": dt * 1e3, "steps": ke, "api": "pivot_iv_forward_backward_host (pinned host buffers)",
+               "staging": "chunks of up to 2^23 rows, ramped (2^20, 2^21, 2^22, 2^23 ... and halved again at the end), 4 slots"}
         del host, hgs, hout
         # Label generation (64 batches x 65,536 options, H2D included): ONE host array of 4,194,304 config-0 rows,
         # forward only.  With N ranks each takes its contiguous shard (sharding.shard_rows) through its own pipeline.
