@@ -283,6 +283,51 @@ def test_roundtrip_ragged_sizes_and_row_independence(bsm):
                 assert (sums == 0).all()
 
 
+def test_roundtrip_matches_the_composition_of_the_public_calls_at_scale():
+    """4,194,304 mixed rows (more than the oracle does in seconds): the fused round-trip kernel against the same objective
+    composed from the separately tested calls -- pivot_iv_black_price (price node, V_hat), pivot_iv_forward on P~ (the tile
+    kernel; the fused kernel solves from its per-warp stack) and plain torch fp64 for the weights: same rows used, sums to
+    1e-11, every gradient entry to 1e-9 of its own size (+ 1e-12 of the largest), nothing but +0 on the rows the sum skips."""
+    n = 1 << 22
+    cfg = wl.config4(n, seed=81, device="cuda")
+    a = [cfg[k] for k in ("SorF", "K", "tau", "P", "flag")]
+    F, K, tau, Pstar, flag = a
+    sstar, _, st0 = pv.pivot_iv_forward(*a)
+    g0 = torch.Generator(device="cuda").manual_seed(3)
+    base = torch.where((st0 == 0) & (sstar > 0), sstar, torch.full_like(sstar, 0.3))
+    sh = base * (1 + 0.05 * torch.randn(n, generator=g0, device="cuda", dtype=torch.float64))
+    sh[::1009] = float("nan")
+    ss = torch.where(torch.isfinite(sstar), sstar, torch.full_like(sstar, 0.25))
+    floor, scale = 1e-6, 0.5
+    sums, g = pv.pivot_iv_loss_roundtrip(*a, sh, ss, floor, mode=pv.RT_GATED, grad_scale=scale)
+    pm, vh = pv.pivot_iv_black_price(F, K, tau, sh, flag)
+    usable = torch.isfinite(pm) & torch.isfinite(vh) & torch.isfinite(ss)
+    on = vh.abs() > floor
+    Pt = torch.where(usable & on, pm, Pstar)
+    srt, vrt, st = pv.pivot_iv_forward(F, K, tau, Pt, flag)
+    ok = usable & (st == 0)
+    f2 = floor * floor
+    v2 = vh * vh
+    den = v2 + f2
+    w = v2 / den
+    d = srt - ss
+    z = torch.zeros_like(d)
+    ref_sums = torch.stack([torch.where(ok, w * d * d, z).sum(), torch.where(ok, w, z).sum(), ok.double().sum()])
+    assert sums[2].item() == ref_sums[2].item() and 0.3 * n < ref_sums[2].item() < n
+    assert sums[0].item() == pytest.approx(ref_sums[0].item(), rel=1e-11)
+    assert sums[1].item() == pytest.approx(ref_sums[1].item(), rel=1e-11)
+    s_hat = sh * tau.sqrt()
+    d1d2 = (torch.log(F / K) / s_hat) ** 2 - 0.25 * s_hat * s_hat
+    vomma = torch.where(sh > 0, vh * d1d2 / sh, z)
+    wp = torch.where(den > 0, 2.0 * vh * f2 / (den * den), z)
+    gi = wp * d * d * vomma + torch.where(on & (vrt.abs() > floor), w * (2.0 * d / vrt) * vh, z)
+    ref = torch.where(ok, scale * gi, z)
+    assert torch.isfinite(g).all()
+    assert (g[~ok] == 0).all() and not torch.signbit(g[~ok]).any()
+    err = (g - ref).abs()
+    assert (err <= 1e-9 * ref.abs() + 1e-12 * ref.abs().max()).all(), float((err / (ref.abs() + 1e-300)).max())
+
+
 def test_nan_poisoning_diagnostic():
     """PAPER.md:404-428 (App. B.2, Fig.6): on the low_vega_tail chain (N = 65,536, seed 31, ~91 % of rows |V| <= 1e-14) the
     naive composition poisons every row of the singular set within one Adam step and never recovers; the gated objective
