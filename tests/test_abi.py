@@ -65,6 +65,21 @@ def test_argument_validation_without_gpu(lib):
     assert lib.pivot_iv_pipeline_create(ctypes.byref(h), 0, i64(0), 2) == -7
     assert lib.pivot_iv_pipeline_create(ctypes.byref(h), 0, i64(16), 9) == -7
     assert lib.pivot_iv_pipeline_destroy(None) == 0
+    assert lib.pivot_iv_pipeline_set_host_access(None, 0) == -1
+    assert lib.pivot_iv_pipeline_last_host_path(None) == -1
+    assert lib.pivot_iv_pipeline_set_forward_kernel(None, 0) == -1
+
+
+def test_binding_constants_are_the_header_defines():
+    """Every numeric #define of include/pivot_iv.h that the binding mirrors carries the same value there."""
+    text = open(os.path.join(ROOT, "include", "pivot_iv.h")).read()
+    defs = {m.group(1): int(m.group(2)) for m in re.finditer(r"#define\s+PIVOT_([A-Z0-9_]+)\s+\(?(-?\d+)\)?", text)}
+    mirrored = {"GATE_MASK": pv.GATE_MASK, "GATE_ATTENUATE": pv.GATE_ATTENUATE, "GATE_STRICT": pv.GATE_STRICT,
+                "RT_GATED": pv.RT_GATED, "RT_NAIVE": pv.RT_NAIVE, "FWD_AUTO": pv.FWD_AUTO, "FWD_COMPACT": pv.FWD_COMPACT,
+                "FWD_ROWWISE": pv.FWD_ROWWISE, "FWD_FP64_ONLY": pv.FWD_FP64_ONLY, "HOST_AUTO": pv.HOST_AUTO,
+                "HOST_STAGED": pv.HOST_STAGED, "HOST_DIRECT": pv.HOST_DIRECT, "STATIC_MAX_ROWS": pv.STATIC_MAX_ROWS}
+    for name, value in mirrored.items():
+        assert defs[name] == value, name
 
 
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
