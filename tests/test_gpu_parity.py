@@ -321,6 +321,15 @@ def test_host_direct_path_on_pinned_arrays():
     assert pipe.last_host_path() == pv.HOST_DIRECT
     assert np.array_equal(out[0].numpy().view(np.uint64), r2[0].cpu().numpy().view(np.uint64)) and torch.equal(out[2], r2[2].cpu())
     pipe.close()
+    # the row-sharded driver on pinned arrays: every shard's pipeline takes the direct path (two pipelines; on a one-GPU box both
+    # on cuda:0), the shards together give the whole array's bits
+    ndev = torch.cuda.device_count()
+    sp = pv.ShardedPipeline(devices=[0, 1 % ndev], chunk_rows=10_000, n_slots=2)
+    out = sp.forward_host(*[c2[k].pin_memory() for k in KEYS], r=c2["r"].pin_memory(), q=c2["q"].pin_memory(), out=pout(m))
+    assert all(q_.last_host_path() == pv.HOST_DIRECT for q_ in sp.pipes)
+    assert np.array_equal(out[0].numpy().view(np.uint64), r2[0].cpu().numpy().view(np.uint64)) and torch.equal(out[2], r2[2].cpu())
+    assert np.array_equal(out[1].numpy().view(np.uint64), r2[1].cpu().numpy().view(np.uint64))
+    sp.close()
 
 
 def test_host_pipeline_matches_oracle():
