@@ -560,6 +560,7 @@ def main():
     # --- zone mix of this workload (diagnostic kernel variant; not timed)
     zsig, zveg, zst, zone = pv.pivot_iv_forward_zones(*a)
     mix = [int(((zone == z) & (zst == 0)).sum().item()) for z in range(4)] + [int((zst != 0).sum().item())]
+    status_counts = [int(x) for x in pv.pivot_iv_status_histogram(zst).cpu().tolist()]   # the library's own diagnostic kernel
     del zsig, zveg, zone, zst
 
     # --- cpu_baseline + parity sample + algorithmic flop count: the oracle, rank 0 at N = 1 only
@@ -685,6 +686,7 @@ def main():
                            "rows_per_gpu": n, "l2": "inputs+outputs 5.5 GB per step >> 126 MB L2, no flush needed",
                            "global_rows": world * n, "rank0_shard": [g_begin, g_end],
                            "zone_mix_rows[z0,z1,z2,z3,non_ok]": mix,
+                           "status_rows[ok,below_intrinsic,above_max,bad_input,at_intrinsic,other]": status_counts,
                            "forward_call": {"auto": "pivot_iv_forward (default): ONE graph launch = one-warp probe kernel -> IF/ELSE node -> "
                                                     "forward_kernel_tile here (forward_kernel_scalar on option chains); fwd_ms and "
                                                     "roofline.avg_launch_ms bracket the whole graph launch (~20 us more than the kernel alone)",

@@ -193,6 +193,12 @@ int pivot_iv_loss_roundtrip(const pivot_iv_inputs* in, const double* sigma_hat, 
                             int mode, int64_t n, double* out3, double* grad_sigma_hat, double grad_scale,
                             pivot_iv_stream stream);
 
+/* Status histogram (diagnostics): counts6[k] += number of rows with status k for k = PIVOT_ST_OK ..
+ * PIVOT_ST_AT_INTRINSIC (0..4), counts6[5] += rows with any other byte.
+ *   status  [in, device, n bytes], any alignment;  counts6 [device, 6 x uint64] is ACCUMULATED into (zero it first).
+ * Asynchronous on `stream`.  Returns PIVOT_ERR_BAD_N / PIVOT_ERR_NULL / PIVOT_ERR_CUDA. */
+int pivot_iv_status_histogram(const uint8_t* status, int64_t n, unsigned long long* counts6, pivot_iv_stream stream);
+
 /* ---- host-buffer pipeline (the streaming label-generation setting: batches of rows, H2D included) ----
  * A pipeline owns `n_slots` device staging slots of `chunk_rows` rows each, one CUDA stream per slot and pinned
  * bounce buffers are NOT used: host arrays are copied directly (pin them for full PCIe speed).  The *_host calls split

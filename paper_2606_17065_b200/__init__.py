@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     library_path,
     load_library,
     pivot_iv_black_price,
+    pivot_iv_status_histogram,
     pivot_iv_backward,
     pivot_iv_backward_inputs,
     pivot_iv_forward,
@@ -44,7 +45,7 @@ from .binding import (  # noqa: F401
 )
 
 __all__ = [
-    "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_backward_inputs", "pivot_iv_black_price",
+    "pivot_iv_forward", "pivot_iv_forward_zones", "pivot_iv_backward", "pivot_iv_backward_inputs", "pivot_iv_black_price", "pivot_iv_status_histogram",
     "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "Pipeline", "ShardedPipeline", "pivot_iv_probe_dfma",
     "pivot_iv_strerror", "pivot_iv_version", "load_library", "library_path", "PivotError", "GATE_MASK",

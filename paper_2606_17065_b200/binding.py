@@ -29,7 +29,7 @@ EXPORTS = (
     "pivot_iv_black_price", "pivot_iv_backward_inputs", "pivot_iv_loss_price", "pivot_iv_loss_roundtrip",
     "pivot_iv_forward_ex", "pivot_iv_pipeline_set_forward_kernel",
     "pivot_iv_forward_diag", "pivot_iv_debug_math", "pivot_iv_forward_launches", "pivot_iv_forward_probe",
-    "pivot_iv_forward_host_static", "pivot_iv_pipeline_set_host_access", "pivot_iv_pipeline_last_host_path",
+    "pivot_iv_forward_host_static", "pivot_iv_pipeline_set_host_access", "pivot_iv_pipeline_last_host_path", "pivot_iv_status_histogram",
 )
 
 
@@ -65,6 +65,7 @@ def load_library():
     lib.pivot_iv_pipeline_set_forward_kernel.argtypes = [vp, cint]
     lib.pivot_iv_pipeline_set_host_access.argtypes = [vp, cint]
     lib.pivot_iv_pipeline_last_host_path.argtypes = [vp]
+    lib.pivot_iv_status_histogram.argtypes = [vp, i64, vp, vp]
     lib.pivot_iv_debug_math.argtypes = [cint, vp, vp, i64, vp, vp]
     lib.pivot_iv_forward_diag.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp, vp, cint, vp]
     lib.pivot_iv_forward_zones.argtypes = [C.POINTER(_Inputs), i64, vp, vp, vp, vp, vp]
@@ -289,6 +290,20 @@ def pivot_iv_backward(grad_sigma, vega, status, vega_floor: float, mode: int, ou
                                      _dev(status, "status", torch.uint8), float(vega_floor), int(mode), n,
                                      _dev(gP, "grad_P"), _stream_ptr(stream)))
     return gP
+
+
+def pivot_iv_status_histogram(status, out=None, stream=None) -> torch.Tensor:
+    """Rows per status code: an int64 CUDA tensor of 6 counts (status 0..4, anything else); `out` is accumulated into."""
+    _require_cuda()
+    n = status.numel()
+    counts = torch.zeros(6, dtype=torch.int64, device=status.device) if out is None else out
+    if not (counts.is_cuda and counts.dtype == torch.int64 and counts.numel() == 6 and counts.is_contiguous()):
+        raise PivotError("out: expected a contiguous CUDA int64 tensor of 6 elements")
+    _same_device(status, out=counts)
+    with _guard(status.device):
+        _check(load_library().pivot_iv_status_histogram(_dev(status, "status", torch.uint8), n, counts.data_ptr(),
+                                                        _stream_ptr(stream)))
+    return counts
 
 
 def pivot_iv_black_price(S_or_F, K, tau, sigma, flag, r=None, q=None, with_vega=True, stream=None):

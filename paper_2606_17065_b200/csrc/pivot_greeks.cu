@@ -364,6 +364,48 @@ loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, 
   block_add3(acc, wsum, cnt, out);
 }
 
+// Status histogram (optional diagnostics): out[k] += rows with status k, k = 0..4; out[5] += any other byte.
+// 16 status bytes per load where the pointer allows it, four bytes compared at a time (__vcmpeq4 + popc), one warp reduction
+// and at most six 64-bit atomics per warp.
+__device__ __forceinline__ void hist_byte(unsigned st, unsigned long long (&c)[6]) {
+#pragma unroll
+  for (unsigned k = 0; k < 5; ++k) c[k] += (st == k) ? 1ull : 0ull;
+  c[5] += (st > 4u) ? 1ull : 0ull;
+}
+
+__global__ void __launch_bounds__(kEwThreads) status_histogram_kernel(const uint8_t* __restrict__ status, int64_t n,
+                                                                      unsigned long long* __restrict__ out) {
+  unsigned long long c[6] = {0, 0, 0, 0, 0, 0};
+  const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, nthreads = (int64_t)gridDim.x * blockDim.x;
+  const int64_t head = (16 - (int64_t)(reinterpret_cast<uintptr_t>(status) & 15u)) & 15;   // bytes before the first 16-byte boundary
+  const int64_t h = head < n ? head : n;
+  const int64_t nvec = (n - h) / 16;
+  const uint4* __restrict__ v = reinterpret_cast<const uint4*>(status + h);
+  for (int64_t i = tid; i < nvec; i += nthreads) {
+    const uint4 w = __ldcs(v + i);
+    const unsigned words[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      unsigned known = 0u;
+#pragma unroll
+      for (unsigned b = 0; b < 5; ++b) {
+        const unsigned m = (unsigned)__popc(__vcmpeq4(words[k], b * 0x01010101u) & 0x01010101u);
+        c[b] += m;
+        known += m;
+      }
+      c[5] += 4u - known;
+    }
+  }
+  for (int64_t i = tid; i < h; i += nthreads) hist_byte(status[i], c);
+  for (int64_t i = h + nvec * 16 + tid; i < n; i += nthreads) hist_byte(status[i], c);
+#pragma unroll
+  for (int k = 0; k < 6; ++k) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c[k] += __shfl_down_sync(0xffffffffu, c[k], d);
+    if ((threadIdx.x & 31) == 0 && c[k]) atomicAdd(out + k, c[k]);
+  }
+}
+
 inline int ew_blocks(int64_t n) {
   int dev = 0, sms = 0;   // per call: the current device may differ between calls (cudaDeviceGetAttribute is a cached lookup)
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
@@ -393,6 +435,15 @@ int pivot_iv_black_price(const pivot_iv_inputs* in, const double* sigma, int64_t
     black_price_kernel<true><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma, n, price, vega);
   else
     black_price_kernel<false><<<ew_blocks(n), kEwThreads, 0, st>>>(*in, sigma, n, price, vega);
+  return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
+}
+
+int pivot_iv_status_histogram(const uint8_t* status, int64_t n, unsigned long long* counts6, pivot_iv_stream stream) {
+  if (n < 0) return PIVOT_ERR_BAD_N;
+  if (!counts6) return PIVOT_ERR_NULL;
+  if (n == 0) return PIVOT_OK;
+  if (!status) return PIVOT_ERR_NULL;
+  status_histogram_kernel<<<ew_blocks((n + 15) / 16), kEwThreads, 0, reinterpret_cast<cudaStream_t>(stream)>>>(status, n, counts6);
   return cudaGetLastError() == cudaSuccess ? PIVOT_OK : PIVOT_ERR_CUDA;
 }
 

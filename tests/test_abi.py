@@ -66,6 +66,10 @@ def test_argument_validation_without_gpu(lib):
     assert lib.pivot_iv_pipeline_create(ctypes.byref(h), 0, i64(16), 9) == -7
     assert lib.pivot_iv_pipeline_destroy(None) == 0
     assert lib.pivot_iv_pipeline_set_host_access(None, 0) == -1
+    assert lib.pivot_iv_status_histogram(8, i64(-1), 8, None) == -2
+    assert lib.pivot_iv_status_histogram(8, i64(4), None, None) == -1
+    assert lib.pivot_iv_status_histogram(None, i64(4), 8, None) == -1
+    assert lib.pivot_iv_status_histogram(None, i64(0), 8, None) == 0
     assert lib.pivot_iv_pipeline_last_host_path(None) == -1
     assert lib.pivot_iv_pipeline_set_forward_kernel(None, 0) == -1
 

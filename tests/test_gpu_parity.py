@@ -215,6 +215,26 @@ def test_full_size_headline_sampled():
     assert st["ok"] > 0.2 * idx.numel()
 
 
+def test_status_histogram_matches_the_oracle_counts():
+    """pivot_iv_status_histogram (diagnostics) on the status bytes of the forward pass: the counts per status code are those of
+    the ORACLE's status array (bit-exact integers), for sizes and pointer offsets around the 16-byte vector path, an empty
+    array, bytes outside 0..4 in the last bin, and accumulation into a caller's tensor."""
+    cfg = wl.config4(300_007, seed=91)
+    d, c = to_device(cfg), to_numpy(cfg)
+    st = gpu_forward(d)[2]
+    ost = oracle_forward(c)[2]
+    for lo, hi in ((0, 300_007), (1, 300_007), (5, 299_990), (3, 10), (7, 7 + 16), (0, 15), (0, 16), (0, 17), (0, 0), (13, 13 + 65_536)):
+        got = pv.pivot_iv_status_histogram(st[lo:hi]).cpu().numpy()
+        ref = np.bincount(ost[lo:hi], minlength=6)[:6]
+        assert np.array_equal(got, ref), (lo, hi, got, ref)
+    assert got.sum() == 65_536
+    junk = torch.tensor([0, 1, 2, 3, 4, 5, 9, 255, 4, 4, 0] * 1000, dtype=torch.uint8, device="cuda")
+    acc = torch.zeros(6, dtype=torch.int64, device="cuda")
+    pv.pivot_iv_status_histogram(junk, out=acc)
+    pv.pivot_iv_status_histogram(junk, out=acc)
+    assert acc.cpu().tolist() == [4000, 2000, 2000, 2000, 6000, 6000]
+
+
 def test_host_pipeline_matches_device_path():
     """pivot_iv_forward_host / _forward_backward_host (chunked H2D -> kernels -> D2H) give the device path's bits."""
     cfg = wl.config3(300_001, seed=9)
