@@ -365,7 +365,7 @@ loss_roundtrip_kernel(pivot_iv_inputs in, const double* __restrict__ sigma_hat, 
 }
 
 // Status histogram (optional diagnostics): out[k] += rows with status k, k = 0..4; out[5] += any other byte.
-// 16 status bytes per load where the pointer allows it, four bytes compared at a time (__vcmpeq4 + popc), one warp reduction
+// 16 status bytes per load where the pointer allows it, four bytes classified at a time (bit-sliced masks + popc), one warp reduction
 // in shared memory and at most six 64-bit global atomics per CTA (per warp they cost 113 us of contention at 2^26 rows).
 __device__ __forceinline__ void hist_byte(unsigned st, unsigned long long (&c)[6]) {
 #pragma unroll
@@ -385,16 +385,26 @@ __global__ void __launch_bounds__(kEwThreads) status_histogram_kernel(const uint
     const uint4 w = __ldcs(v + i);
     const unsigned words[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      unsigned known = 0u;
+    unsigned p[5] = {0u, 0u, 0u, 0u, 0u};
 #pragma unroll
-      for (unsigned b = 0; b < 5; ++b) {
-        const unsigned m = (unsigned)__popc(__vcmpeq4(words[k], b * 0x01010101u) & 0x01010101u);
-        c[b] += m;
-        known += m;
-      }
-      c[5] += 4u - known;
+    for (int k = 0; k < 4; ++k) {
+      // bit-sliced: per byte b0, b1, b2 = the three low bits and hi = "any of bits 3..7" as one flag bit each (0x01 per byte);
+      // status 0..4 = 000, 001, 010, 011, 100 with hi clear
+      const unsigned w_ = words[k], m = 0x01010101u;
+      const unsigned b0 = w_ & m, b1 = (w_ >> 1) & m, b2 = (w_ >> 2) & m;
+      const unsigned t = (w_ >> 3) & 0x1f1f1f1fu;
+      const unsigned hi = ((t + 0x7f7f7f7fu) >> 7) & m;     // t <= 0x1f per byte: no carry into the next byte
+      const unsigned n12h = ~(b1 | b2 | hi), n0 = ~b0;
+      p[0] += (unsigned)__popc(n0 & n12h & m);
+      p[1] += (unsigned)__popc(b0 & n12h);
+      p[2] += (unsigned)__popc(b1 & n0 & ~(b2 | hi));
+      p[3] += (unsigned)__popc(b0 & b1 & ~(b2 | hi));
+      p[4] += (unsigned)__popc(b2 & n0 & ~(b1 | hi));
     }
+    const unsigned known = p[0] + p[1] + p[2] + p[3] + p[4];
+#pragma unroll
+    for (int b = 0; b < 5; ++b) c[b] += p[b];
+    c[5] += 16u - known;
   }
   for (int64_t i = tid; i < h; i += nthreads) hist_byte(status[i], c);
   for (int64_t i = h + nvec * 16 + tid; i < n; i += nthreads) hist_byte(status[i], c);
