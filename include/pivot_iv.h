@@ -9,8 +9,11 @@
  * Conventions for every entry point
  *   - plain C, no C++ exceptions cross the boundary; returns 0 (PIVOT_OK) or a negative PIVOT_ERR_* code;
  *   - per-row numerical problems are never error codes, they are `status` values;
- *   - the library never allocates, frees or retains caller memory, keeps no global mutable state (except inside an
- *     explicit pivot_iv_pipeline object), and the device entry points never synchronise the host:
+ *   - the library never allocates, frees or retains caller memory, keeps no global mutable state that changes a result
+ *     (state lives inside an explicit pivot_iv_pipeline object; per device ordinal it caches, thread-safely, what it would
+ *     otherwise look up on every call: kernel attributes, the SM count, the launch graph of the default forward call, the
+ *     address of the static staging array of pivot_iv_forward_host_static), reads no environment variable, and the device
+ *     entry points never synchronise the host:
  *     work is enqueued on `stream` (a cudaStream_t passed as an opaque pointer; NULL = the legacy default stream);
  *   - all arrays are SoA, contiguous, length n, fp64 unless stated; pointers need only their natural alignment
  *     (8 B for double): the forward kernel uses 8-byte accesses throughout, the backward kernel has a 16-B-aligned
