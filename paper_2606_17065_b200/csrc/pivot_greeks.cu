@@ -384,7 +384,6 @@ __global__ void __launch_bounds__(kEwThreads) status_histogram_kernel(const uint
   for (int64_t i = tid; i < nvec; i += nthreads) {
     const uint4 w = __ldcs(v + i);
     const unsigned words[4] = {w.x, w.y, w.z, w.w};
-#pragma unroll
     unsigned p[5] = {0u, 0u, 0u, 0u, 0u};
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
